@@ -1,0 +1,139 @@
+/*
+ * af.h — C ABI of the B200-native Cross-Request State Packed Forward over a Unified KV Ring Buffer
+ * (ActionFlow, arxiv 2512.20276).  Citations "P:<n>" are lines of /root/reference/PAPER.md.
+ *
+ * What the library computes
+ *   One call of af_packed_forward is Algorithm 2 "Cross-Request State Packed Forward" applied
+ *   for every layer l = 0..n_layers-1 (Alg. 1 line 3 "PackedForwardEachLayer") to the packed
+ *   Cross-Request State H_CRS of Eq. 1: the rows of all segments (one prefill segment of L_P rows
+ *   and K-1 single-row decode segments in the paper's schedule) stacked along the sequence dimension.
+ *   Per layer: RMSNorm -> QKV projection -> RoPE at the token's logical position in its own request and append
+ *   of K/V into the Unified KV Ring Buffer -> segment-wise causal attention, every row
+ *   attending to positions 0..own position of its own request only -> output projection + residual
+ *   -> RMSNorm -> SwiGLU MLP + residual (P:185 read as the standard Llama pre-norm block, reading A1).
+ *   af_logits_rows is LMHead(Norm(H[s])) of Alg. 1 lines 5/8 on a caller-chosen row list.
+ *   The paper's InPlaceShiftKV moves no bytes here: regions are keyed by req_id and the stage
+ *   shift is a relabelling (reading A7); af_ring_reset_slot recycles an evicted request's region.
+ *
+ * Conventions
+ *   - All "device" pointers are CUDA device memory of the current device, owned by the caller.
+ *     All "host" pointers are ordinary host memory, read (or written) before the call returns.
+ *   - bf16 = IEEE bfloat16 stored as uint16.  Weights are [out_features, in_features] row-major (y = x W^T).
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t cast to void*) and return without host synchronisation
+ *     (the af_debug_* and af_ring_read_* calls synchronise; they are test/bench helpers, not the hot path).
+ *   - Return value: 0 on success, a negative AF_ERR_* otherwise.  On any error raised by argument validation
+ *     no kernel has been launched and the ring bookkeeping is unchanged.  af_last_error() gives a message.
+ *   - One af_ring is not thread-safe; the caller serialises calls on it.
+ *   - There is no CPU fallback anywhere in this library.
+ *
+ * Ring geometry (reading A6).  One allocation `kv_mem` holds, for every layer, all R = n_regions
+ *   request regions of C = capacity token slots each ("single, circular, physically contiguous memory region ...
+ *   logically partitioned per request").  The token at logical position pos of request r lives in
+ *       slot      = (base_r + pos) mod C                       (slot inside region r)
+ *       row_slot  = r * C + slot                               (the global slot id reported by af_debug_row_map)
+ *   and its K (after RoPE) and V vectors of head h are the head_dim contiguous bf16 values at element offset
+ *       (((layer * 2 + kv) * R + r) * n_heads + h) * C * head_dim + slot * head_dim,     kv = 0 for K, 1 for V.
+ *   A request's live range is positions 0..len_r-1; slots outside it are never read.
+ */
+#ifndef AF_H_
+#define AF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AF_OK               0
+#define AF_ERR_ARG         (-1)  /* null pointer, non-positive size, misaligned pointer */
+#define AF_ERR_SEGMENT     (-2)  /* bad or duplicate req_id, len < 1, decode segment with len != 1, too many segments */
+#define AF_ERR_POSITION    (-3)  /* start_pos != current length of the request (appends must be contiguous) */
+#define AF_ERR_CAPACITY    (-4)  /* start_pos + len > capacity: a live token would be overwritten */
+#define AF_ERR_WORKSPACE   (-5)  /* workspace / kv_mem too small */
+#define AF_ERR_CUDA        (-6)  /* a CUDA runtime/driver call failed */
+#define AF_ERR_UNSUPPORTED (-7)  /* shape outside what the sm_100a kernels handle */
+
+#define AF_PHASE_PREFILL 0
+#define AF_PHASE_DECODE  1
+#define AF_MAX_SEGS      64      /* segments per packed step */
+
+typedef struct af_ring af_ring;  /* opaque, library-owned */
+
+typedef struct {
+  int32_t d_model, n_layers, n_heads, head_dim, ffn, vocab;  /* d_model == n_heads*head_dim; head_dim in {64,128} */
+  float   rms_eps, rope_theta;
+} af_model_cfg;
+
+typedef struct { int32_t n_regions, capacity; } af_ring_cfg;
+
+/* One segment of the packed step = "append len tokens at positions start_pos..start_pos+len-1 of request req_id"
+ * (the segment lengths L_s of Alg. 2).  Rows of packed_embeds follow the segment-table order. */
+typedef struct { int32_t req_id, phase, start_pos, len; } af_segment;
+
+typedef struct {                 /* all device bf16 */
+  const void *wq, *wk, *wv, *wo; /* [d_model, d_model] */
+  const void *w_gate, *w_up;     /* [ffn, d_model] */
+  const void *w_down;            /* [d_model, ffn] */
+  const void *g_attn, *g_mlp;    /* RMSNorm gains [d_model] */
+} af_layer_weights;
+
+typedef struct {
+  af_model_cfg cfg;
+  const af_layer_weights* layers; /* HOST array [n_layers] of device pointers */
+  const void* g_final;            /* device bf16 [d_model] */
+  const void* w_lm;               /* device bf16 [vocab, d_model] */
+} af_weights;
+
+/* Bytes of kv_mem needed for (cfg, ring): 2 * n_layers * R * n_heads * C * head_dim * 2. */
+size_t af_ring_bytes(const af_model_cfg* cfg, const af_ring_cfg* ring);
+/* Bytes of workspace needed by af_packed_forward / af_logits_rows for up to max_rows packed rows. */
+size_t af_workspace_bytes(const af_model_cfg* cfg, int32_t max_rows, int32_t max_segs);
+
+/* Create the ring bookkeeping over caller-owned device memory kv_mem (256-byte aligned, >= af_ring_bytes).
+ * All regions start with base = 0, len = 0.  kv_mem is not touched (stale bytes are unreachable).
+ * The library allocates only small device metadata of its own (RoPE table, segment tables). */
+int af_ring_create(const af_model_cfg* cfg, const af_ring_cfg* ring, void* kv_mem, size_t kv_bytes, af_ring** out);
+
+/* Recycle region req_id for a new request ("overwriting the evicted oldest request", with no copy):
+ * len = 0 and base = new_base mod C if new_base >= 0, else base = (base + len) mod C (keep rotating). O(1), host only. */
+int af_ring_reset_slot(af_ring* ring, int32_t req_id, int32_t new_base);
+
+/* Algorithm 2 for all layers on one packed step.
+ *   packed_embeds : device bf16 [T, d_model], T = sum of segment lens, rows in segment-table order (H_CRS, Eq. 1)
+ *   segs          : HOST array [n_segs]; each req_id at most once; start_pos == current len of that request;
+ *                   start_pos + len <= capacity; phase == AF_PHASE_DECODE requires len == 1.  n_segs == 0 is a no-op.
+ *   hidden_out    : device fp32 [T, d_model], the residual stream after the last layer (before the final norm)
+ *   workspace     : device, 256-byte aligned, >= af_workspace_bytes(cfg, T, n_segs)
+ * On success the ring lengths advance: len_r = start_pos + len for every segment (the "ring commit"). */
+int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
+                      af_ring* ring, float* hidden_out, void* workspace, size_t ws_bytes, void* cuda_stream);
+
+/* logits_out[i, :] = RMSNorm(hidden[rows[i], :]; g_final) W_lm^T   (Alg. 1 l.5/l.8).
+ *   hidden : device fp32 [>= max(rows)+1, d_model];  rows : HOST int32 [n_rows], n_rows <= 256
+ *   logits_out : device fp32 [n_rows, vocab] */
+int af_logits_rows(const af_weights* w, const float* hidden, const int32_t* rows, int32_t n_rows,
+                   float* logits_out, void* workspace, size_t ws_bytes, void* cuda_stream);
+
+int af_ring_destroy(af_ring* ring); /* frees the handle and its own metadata; never frees caller memory */
+
+/* ---- introspection for bit-exact bookkeeping parity; these synchronise, they are not hot path ---- */
+int af_ring_get_state(const af_ring* ring, int32_t req_id, int32_t* base, int32_t* len);
+/* Row map of the LAST af_packed_forward, copied back from the DEVICE tables the kernels used.
+ * Each output is a HOST int32 [n] array (n <= T of that step) or NULL. */
+int af_debug_row_map(const af_ring* ring, int32_t* row_req, int32_t* row_pos, int32_t* row_slot, int32_t n);
+/* Bench/test only: rewind (or set) the bookkeeping length of a region; moves no data. */
+int af_debug_set_len(af_ring* ring, int32_t req_id, int32_t len);
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+int64_t af_debug_launch_count(void);
+/* Plain C = A B^T through the same tcgen05 GEMM kernel the forward uses (unit tests / roofline probes).
+ * a: device bf16 [n_tok, k] (activations), w: device bf16 [n_out, k]; out: device fp32 [n_tok, n_out]. */
+int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32_t n_out, int32_t k,
+                  void* workspace, size_t ws_bytes, void* cuda_stream);
+
+const char* af_last_error(void); /* thread-local message of the last failing call */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AF_H_ */
