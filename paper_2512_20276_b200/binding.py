@@ -1,0 +1,207 @@
+"""Thin ctypes binding of include/af.h — argument marshalling only; every step of the path runs in the CUDA kernels.
+
+PyTorch is used for device memory (tensor.data_ptr()) and streams only.  Loading fails loudly when the CUDA
+library has not been built (python -m paper_2512_20276_b200.build, or __graft_entry__.build()).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaf_b200.so")
+
+AF_OK, AF_ERR_ARG, AF_ERR_SEGMENT, AF_ERR_POSITION = 0, -1, -2, -3
+AF_ERR_CAPACITY, AF_ERR_WORKSPACE, AF_ERR_CUDA, AF_ERR_UNSUPPORTED = -4, -5, -6, -7
+ERR_NAMES = {0: "AF_OK", -1: "AF_ERR_ARG", -2: "AF_ERR_SEGMENT", -3: "AF_ERR_POSITION", -4: "AF_ERR_CAPACITY",
+             -5: "AF_ERR_WORKSPACE", -6: "AF_ERR_CUDA", -7: "AF_ERR_UNSUPPORTED"}
+
+
+class AfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+        self.name = ERR_NAMES.get(code, str(code))
+
+
+class af_model_cfg(C.Structure):
+    _fields_ = [("d_model", C.c_int32), ("n_layers", C.c_int32), ("n_heads", C.c_int32), ("head_dim", C.c_int32),
+                ("ffn", C.c_int32), ("vocab", C.c_int32), ("rms_eps", C.c_float), ("rope_theta", C.c_float)]
+
+
+class af_ring_cfg(C.Structure):
+    _fields_ = [("n_regions", C.c_int32), ("capacity", C.c_int32)]
+
+
+class af_segment(C.Structure):
+    _fields_ = [("req_id", C.c_int32), ("phase", C.c_int32), ("start_pos", C.c_int32), ("len", C.c_int32)]
+
+
+class af_layer_weights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("wq", "wk", "wv", "wo", "w_gate", "w_up", "w_down", "g_attn", "g_mlp")]
+
+
+class af_weights(C.Structure):
+    _fields_ = [("cfg", af_model_cfg), ("layers", C.POINTER(af_layer_weights)), ("g_final", C.c_void_p),
+                ("w_lm", C.c_void_p)]
+
+
+EXPORTS = ["af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+           "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
+           "af_debug_launch_count", "af_debug_gemm", "af_last_error"]
+
+_lib = None
+
+
+def load_library():
+    """dlopen the C-ABI library and declare its prototypes.  Raises if the library is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build the CUDA library first "
+                           "(python -m paper_2512_20276_b200.build). There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, sz = C.c_void_p, C.c_int32, C.c_size_t
+    L.af_ring_bytes.restype = sz
+    L.af_ring_bytes.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg)]
+    L.af_workspace_bytes.restype = sz
+    L.af_workspace_bytes.argtypes = [C.POINTER(af_model_cfg), i32, i32]
+    L.af_ring_create.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg), vp, sz, C.POINTER(vp)]
+    L.af_ring_reset_slot.argtypes = [vp, i32, i32]
+    L.af_packed_forward.argtypes = [C.POINTER(af_weights), vp, C.POINTER(af_segment), i32, vp, vp, vp, sz, vp]
+    L.af_logits_rows.argtypes = [C.POINTER(af_weights), vp, C.POINTER(i32), i32, vp, vp, sz, vp]
+    L.af_ring_destroy.argtypes = [vp]
+    L.af_ring_get_state.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32)]
+    L.af_debug_row_map.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), i32]
+    L.af_debug_set_len.argtypes = [vp, i32, i32]
+    L.af_debug_launch_count.restype = C.c_int64
+    L.af_debug_launch_count.argtypes = []
+    L.af_debug_gemm.argtypes = [vp, vp, vp, i32, i32, i32, vp, sz, vp]
+    L.af_last_error.restype = C.c_char_p
+    L.af_last_error.argtypes = []
+    for n in ("af_ring_create", "af_ring_reset_slot", "af_packed_forward", "af_logits_rows", "af_ring_destroy",
+              "af_ring_get_state", "af_debug_row_map", "af_debug_set_len", "af_debug_gemm"):
+        getattr(L, n).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        raise AfError(rc, load_library().af_last_error().decode())
+
+
+def _cfg_struct(cfg) -> af_model_cfg:
+    return af_model_cfg(cfg.d_model, cfg.n_layers, cfg.n_heads, cfg.head_dim, cfg.ffn, cfg.vocab,
+                        cfg.rms_eps, cfg.rope_theta)
+
+
+def _stream_ptr(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class Weights:
+    """Device copies of the bf16 weights + the af_weights struct pointing at them."""
+
+    def __init__(self, cfg, host_weights: dict, device="cuda"):
+        self.cfg = cfg
+        self.tensors = []          # keep alive
+        self._layers = (af_layer_weights * cfg.n_layers)()
+        for l, L in enumerate(host_weights["layers"]):
+            for name, _ in af_layer_weights._fields_:
+                t = L[name].to(torch.bfloat16).contiguous().to(device)
+                self.tensors.append(t)
+                setattr(self._layers[l], name, t.data_ptr())
+        self.g_final = host_weights["g_final"].to(torch.bfloat16).contiguous().to(device)
+        self.w_lm = host_weights["w_lm"].to(torch.bfloat16).contiguous().to(device)
+        self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr())
+
+
+class Ring:
+    """af_ring_create / af_ring_reset_slot / af_packed_forward / af_logits_rows / af_ring_destroy."""
+
+    def __init__(self, cfg, n_regions: int, capacity: int, max_rows: int, device="cuda"):
+        L = load_library()
+        self.cfg, self.R, self.Cap = cfg, n_regions, capacity
+        self._c = _cfg_struct(cfg)
+        self._r = af_ring_cfg(n_regions, capacity)
+        nbytes = L.af_ring_bytes(C.byref(self._c), C.byref(self._r))
+        self.kv_mem = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        self.max_rows = max_rows
+        self.ws_bytes = L.af_workspace_bytes(C.byref(self._c), max_rows, 64)
+        self.workspace = torch.empty(self.ws_bytes, dtype=torch.uint8, device=device)
+        h = C.c_void_p()
+        _check(L.af_ring_create(C.byref(self._c), C.byref(self._r), self.kv_mem.data_ptr(), nbytes, C.byref(h)))
+        self.handle = h
+
+    def kv_view(self) -> torch.Tensor:
+        """The ring as bf16 [n_layers, 2, R, H, C, hd] (layout documented in include/af.h)."""
+        c = self.cfg
+        return self.kv_mem.view(torch.bfloat16).view(c.n_layers, 2, self.R, c.n_heads, self.Cap, c.head_dim)
+
+    def reset_slot(self, req_id: int, new_base: int = -1):
+        _check(load_library().af_ring_reset_slot(self.handle, req_id, new_base))
+
+    def get_state(self, req_id: int):
+        b, n = C.c_int32(), C.c_int32()
+        _check(load_library().af_ring_get_state(self.handle, req_id, C.byref(b), C.byref(n)))
+        return b.value, n.value
+
+    def set_len(self, req_id: int, n: int):
+        _check(load_library().af_debug_set_len(self.handle, req_id, n))
+
+    def packed_forward(self, weights: Weights, packed_embeds: torch.Tensor, segs, hidden_out: torch.Tensor = None,
+                       stream=None) -> torch.Tensor:
+        T = sum(s[3] for s in segs)
+        arr = (af_segment * max(1, len(segs)))(*[af_segment(*s) for s in segs])
+        if hidden_out is None:
+            hidden_out = torch.empty(T, self.cfg.d_model, dtype=torch.float32, device=packed_embeds.device)
+        _check(load_library().af_packed_forward(C.byref(weights.struct), packed_embeds.data_ptr(), arr, len(segs),
+                                                self.handle, hidden_out.data_ptr(), self.workspace.data_ptr(),
+                                                self.ws_bytes, _stream_ptr(stream)))
+        return hidden_out
+
+    def logits_rows(self, weights: Weights, hidden: torch.Tensor, rows, logits_out: torch.Tensor = None, stream=None):
+        n = len(rows)
+        arr = (C.c_int32 * max(1, n))(*rows)
+        if logits_out is None:
+            logits_out = torch.empty(n, self.cfg.vocab, dtype=torch.float32, device=hidden.device)
+        _check(load_library().af_logits_rows(C.byref(weights.struct), hidden.data_ptr(), arr, n, logits_out.data_ptr(),
+                                             self.workspace.data_ptr(), self.ws_bytes, _stream_ptr(stream)))
+        return logits_out
+
+    def row_map(self, n: int):
+        a, b, c = (C.c_int32 * max(1, n))(), (C.c_int32 * max(1, n))(), (C.c_int32 * max(1, n))()
+        _check(load_library().af_debug_row_map(self.handle, a, b, c, n))
+        return list(a)[:n], list(b)[:n], list(c)[:n]
+
+    def destroy(self):
+        if self.handle is not None:
+            load_library().af_ring_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def debug_gemm(a: torch.Tensor, w: torch.Tensor) -> torch.Tensor:
+    """out[n_tok, n_out] fp32 = a[n_tok, k] @ w[n_out, k]^T through the tcgen05 GEMM kernel."""
+    L = load_library()
+    n_tok, k = a.shape
+    n_out = w.shape[0]
+    out = torch.empty(n_tok, n_out, dtype=torch.float32, device=a.device)
+    ws = torch.empty(160 * 288 * 128 * 4, dtype=torch.uint8, device=a.device)
+    _check(L.af_debug_gemm(a.data_ptr(), w.data_ptr(), out.data_ptr(), n_tok, n_out, k, ws.data_ptr(), ws.numel(),
+                           _stream_ptr()))
+    return out
+
+
+def launch_count() -> int:
+    return int(load_library().af_debug_launch_count())

@@ -1,0 +1,444 @@
+// Host side of the C ABI in include/af.h: ring bookkeeping + validation (a0, a9), tensor-map cache, workspace carve
+// and the launch sequence of Algorithm 2 per layer.  Links only libcudart; the driver's
+// cuTensorMapEncodeTiled is fetched through cudaGetDriverEntryPoint.  No CPU fallback: every step is a kernel.
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "../../include/af.h"
+
+namespace af { constexpr int AF_MAX_SEGS_K = AF_MAX_SEGS; }
+#include "gemm_tcgen05.cuh"
+#include "elementwise.cuh"
+
+using namespace af;
+
+// ------------------------------------------------------------------------------------------------ errors
+static thread_local std::string g_err;
+static int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+#define CUDA_TRY(expr)                                                                              \
+  do {                                                                                              \
+    cudaError_t e_ = (expr);                                                                        \
+    if (e_ != cudaSuccess) return fail(AF_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+static std::atomic<int64_t> g_launches{0};
+static int check_launch(const char* what) {
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+  return AF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static std::mutex g_mu;
+static EncodeTiledFn g_encode = nullptr;
+static std::map<std::tuple<const void*, int, int, int>, CUtensorMap> g_maps;
+
+// bf16 row-major [rows, cols] matrix, box = [box_rows, 64 cols], 128-byte swizzle, zero fill out of bounds.
+static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  auto key = std::make_tuple(ptr, rows, cols, box_rows);
+  auto it = g_maps.find(key);
+  if (it != g_maps.end()) { *out = it->second; return AF_OK; }
+  if (!g_encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+  }
+  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || (cols % 8))
+    return fail(AF_ERR_ARG, "matrix %p [%d,%d] must be 16-byte aligned with a 16-byte row pitch", ptr, rows, cols);
+  CUtensorMap m;
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(cols) * 2};
+  cuuint32_t box[2] = {static_cast<cuuint32_t>(GEMM_BK), static_cast<cuuint32_t>(box_rows)};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled([%d,%d], box %d) -> %d", rows, cols, box_rows, (int)r);
+  if (g_maps.size() > 8192) g_maps.clear();
+  g_maps[key] = m;
+  *out = m;
+  return AF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ GEMM launch
+static int g_num_sms = 0;
+static int* g_flags = nullptr;  // [256] stream-K epoch flags
+static int g_epoch = 0;
+constexpr int GEMM_MAX_GRID = 160;
+
+static int gemm_global_init() {
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (g_flags) return AF_OK;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
+  g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
+  CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
+  CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448 - 1024));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 128 * 2));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 64 * 2));
+  return AF_OK;
+}
+
+static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
+
+// out[tok, part*part_rows + f] (op)= sum_k x[tok, k] * w[part][f, k]
+static int launch_gemm(cudaStream_t st, const void* x, int x_rows_cap, int K, const void* const* w, int n_parts,
+                       int part_rows, int T, int epi, void* out, int ld_out, float* partial) {
+  int rc = gemm_global_init();
+  if (rc) return rc;
+  if (T <= 0) return AF_OK;
+  const int n_chunks = (T + GEMM_MAX_TOK - 1) / GEMM_MAX_TOK;
+  const int chunk = (T + n_chunks - 1) / n_chunks;
+  for (int tok0 = 0; tok0 < T; tok0 += chunk) {
+    const int Tc = (T - tok0 < chunk) ? (T - tok0) : chunk;
+    GemmParams p{};
+    int n_pad = (Tc + 15) / 16 * 16;
+    if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
+    else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
+    p.n_parts = n_parts; p.part_rows = part_rows; p.tiles_per_part = (part_rows + GEMM_BM - 1) / GEMM_BM;
+    p.K = K; p.num_kb = (K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
+    p.total_units = n_parts * p.tiles_per_part * p.num_kb;
+    int grid = p.total_units < g_num_sms ? p.total_units : g_num_sms;
+    p.units_per_cta = (p.total_units + grid - 1) / grid;
+    grid = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+    const int stage_bytes = GEMM_BM * GEMM_BK * 2 + n_pad * GEMM_BK * 2;
+    int stages = (232448 - 1024 - 1024) / stage_bytes;
+    if (stages > 12) stages = 12;
+    if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
+    p.stages = stages; p.epi = epi; p.out = out; p.ld_out = ld_out; p.partial = partial; p.flags = g_flags;
+    p.epoch = ++g_epoch;
+    CUtensorMap mw[3], mx;
+    for (int i = 0; i < 3; ++i) {
+      rc = get_map(w[i < n_parts ? i : 0], part_rows, K, GEMM_BM, &mw[i]);
+      if (rc) return rc;
+    }
+    rc = get_map(x, x_rows_cap, K, p.n1, &mx);
+    if (rc) return rc;
+    const size_t smem = static_cast<size_t>(stages) * stage_bytes + 1024;
+    gemm_tcgen05_kernel<<<grid, GEMM_THREADS, smem, st>>>(mw[0], mw[1], mw[2], mx, p);
+    rc = check_launch("gemm_tcgen05_kernel");
+    if (rc) return rc;
+  }
+  return AF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ ring handle
+struct af_ring {
+  af_model_cfg cfg;
+  af_ring_cfg rc;
+  __nv_bfloat16* kv;            // caller-owned
+  std::vector<int> base, len;   // host mirror, authoritative for validation (a0, a9)
+  int* tables = nullptr;        // library-owned device ints backing StepTables
+  StepTables tb{};
+  int* n_items_dev = nullptr;
+  float2* rope_tab = nullptr;   // [C][hd/2]
+  int max_rows = 0;
+  int last_T = 0;
+};
+
+static int check_cfg(const af_model_cfg* c) {
+  if (!c) return fail(AF_ERR_ARG, "null model cfg");
+  if (c->d_model <= 0 || c->n_layers <= 0 || c->n_heads <= 0 || c->ffn <= 0 || c->vocab <= 0)
+    return fail(AF_ERR_ARG, "non-positive model dimension");
+  if (c->head_dim != 64 && c->head_dim != 128) return fail(AF_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", c->head_dim);
+  if (c->d_model != c->n_heads * c->head_dim) return fail(AF_ERR_UNSUPPORTED, "d_model != n_heads*head_dim");
+  if (c->d_model % 8 || c->ffn % 8) return fail(AF_ERR_UNSUPPORTED, "d_model and ffn must be multiples of 8");
+  return AF_OK;
+}
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+extern "C" size_t af_ring_bytes(const af_model_cfg* c, const af_ring_cfg* r) {
+  if (!c || !r) return 0;
+  return static_cast<size_t>(2) * c->n_layers * r->n_regions * c->n_heads * r->capacity * c->head_dim * 2;
+}
+
+// workspace = fixed part (stream-K partials) + per-row part; the carve depends only on (pointer, bytes)
+static size_t ws_per_row(const af_model_cfg* c) {
+  const size_t D = c->d_model, F = c->ffn;
+  return align_up((D + 3 * D + D + D + 2 * F + F) * 2, 256);  // xn, qkv, q_rot, attn, gate|up, h  (bf16)
+}
+static size_t ws_fixed() { return align_up(gemm_partial_bytes(), 256) + 6 * 256; }
+
+extern "C" size_t af_workspace_bytes(const af_model_cfg* c, int32_t max_rows, int32_t max_segs) {
+  (void)max_segs;
+  if (!c || max_rows < 0) return 0;
+  const size_t rows = align_up(static_cast<size_t>(max_rows < 16 ? 16 : max_rows), 16);
+  return ws_fixed() + rows * ws_per_row(c);
+}
+
+struct Workspace {
+  float* partial;
+  __nv_bfloat16 *xn, *qkv, *q_rot, *attn, *gu, *h;
+  int max_rows;
+};
+static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, Workspace* o) {
+  if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255)) return fail(AF_ERR_ARG, "workspace must be 256-byte aligned");
+  if (bytes < ws_fixed() + 16 * ws_per_row(c)) return fail(AF_ERR_WORKSPACE, "workspace of %zu bytes is too small", bytes);
+  size_t rows = (bytes - ws_fixed()) / ws_per_row(c);
+  rows = rows / 16 * 16;
+  if (rows > 65536) rows = 65536;
+  if (static_cast<size_t>(need_rows) > rows)
+    return fail(AF_ERR_WORKSPACE, "workspace holds %zu rows, %d needed (use af_workspace_bytes)", rows, need_rows);
+  uint8_t* p = reinterpret_cast<uint8_t*>(ws);
+  const size_t D = c->d_model, F = c->ffn;
+  auto take = [&](size_t n) { uint8_t* q = p; p += align_up(n, 256); return q; };
+  o->partial = reinterpret_cast<float*>(take(gemm_partial_bytes()));
+  o->xn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
+  o->qkv = reinterpret_cast<__nv_bfloat16*>(take(rows * 3 * D * 2));
+  o->q_rot = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
+  o->attn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
+  o->gu = reinterpret_cast<__nv_bfloat16*>(take(rows * 2 * F * 2));
+  o->h = reinterpret_cast<__nv_bfloat16*>(take(rows * F * 2));
+  o->max_rows = static_cast<int>(rows);
+  return AF_OK;
+}
+
+extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void* kv_mem, size_t kv_bytes, af_ring** out) {
+  int rc = check_cfg(c);
+  if (rc) return rc;
+  if (!r || !out || !kv_mem) return fail(AF_ERR_ARG, "null argument");
+  if (r->n_regions <= 0 || r->capacity <= 0) return fail(AF_ERR_ARG, "ring needs n_regions > 0 and capacity > 0");
+  if (reinterpret_cast<uintptr_t>(kv_mem) & 255) return fail(AF_ERR_ARG, "kv_mem must be 256-byte aligned");
+  if (kv_bytes < af_ring_bytes(c, r)) return fail(AF_ERR_WORKSPACE, "kv_mem of %zu bytes < af_ring_bytes %zu", kv_bytes, af_ring_bytes(c, r));
+  rc = gemm_global_init();
+  if (rc) return rc;
+  af_ring* g = new af_ring();
+  g->cfg = *c; g->rc = *r; g->kv = reinterpret_cast<__nv_bfloat16*>(kv_mem);
+  g->base.assign(r->n_regions, 0); g->len.assign(r->n_regions, 0);
+  const long long cap_rows = static_cast<long long>(r->n_regions) * r->capacity;
+  g->max_rows = static_cast<int>(cap_rows > 65536 ? 65536 : cap_rows);
+  const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 2 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1;
+  cudaError_t e = cudaMalloc(&g->tables, n_int * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&g->rope_tab, static_cast<size_t>(r->capacity) * (c->head_dim / 2) * sizeof(float2));
+  if (e != cudaSuccess) { cudaFree(g->tables); delete g; return fail(AF_ERR_CUDA, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  int* p = g->tables;
+  g->tb.seg_req = p; p += AF_MAX_SEGS; g->tb.seg_start = p; p += AF_MAX_SEGS; g->tb.seg_len = p; p += AF_MAX_SEGS;
+  g->tb.seg_row0 = p; p += AF_MAX_SEGS; g->tb.seg_base = p; p += AF_MAX_SEGS;
+  g->tb.row_req = p; p += g->max_rows; g->tb.row_pos = p; p += g->max_rows; g->tb.row_slot = p; p += g->max_rows;
+  const int max_items = g->max_rows / ATT_BQ + AF_MAX_SEGS;
+  g->tb.item_seg = p; p += max_items; g->tb.item_q0 = p; p += max_items;
+  g->n_items_dev = p;
+  const int n = r->capacity * (c->head_dim / 2);
+  rope_table_kernel<<<(n + 255) / 256, 256>>>(g->rope_tab, r->capacity, c->head_dim, static_cast<double>(c->rope_theta));
+  rc = check_launch("rope_table_kernel");
+  if (rc == AF_OK && cudaDeviceSynchronize() != cudaSuccess) rc = fail(AF_ERR_CUDA, "rope table build failed");
+  if (rc) { cudaFree(g->tables); cudaFree(g->rope_tab); delete g; return rc; }
+  *out = g;
+  return AF_OK;
+}
+
+extern "C" int af_ring_destroy(af_ring* g) {
+  if (!g) return AF_OK;
+  cudaFree(g->tables);
+  cudaFree(g->rope_tab);
+  delete g;
+  return AF_OK;
+}
+
+extern "C" int af_ring_reset_slot(af_ring* g, int32_t req, int32_t new_base) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  if (req < 0 || req >= g->rc.n_regions) return fail(AF_ERR_SEGMENT, "req_id %d outside [0,%d)", req, g->rc.n_regions);
+  const int C = g->rc.capacity;
+  g->base[req] = new_base >= 0 ? new_base % C : (g->base[req] + g->len[req]) % C;
+  g->len[req] = 0;
+  return AF_OK;
+}
+
+extern "C" int af_ring_get_state(const af_ring* g, int32_t req, int32_t* base, int32_t* len) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  if (req < 0 || req >= g->rc.n_regions) return fail(AF_ERR_SEGMENT, "req_id %d outside [0,%d)", req, g->rc.n_regions);
+  if (base) *base = g->base[req];
+  if (len) *len = g->len[req];
+  return AF_OK;
+}
+
+extern "C" int af_debug_set_len(af_ring* g, int32_t req, int32_t len) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  if (req < 0 || req >= g->rc.n_regions) return fail(AF_ERR_SEGMENT, "req_id %d outside [0,%d)", req, g->rc.n_regions);
+  if (len < 0 || len > g->rc.capacity) return fail(AF_ERR_CAPACITY, "len %d outside [0,%d]", len, g->rc.capacity);
+  g->len[req] = len;
+  return AF_OK;
+}
+
+extern "C" int af_debug_row_map(const af_ring* g, int32_t* row_req, int32_t* row_pos, int32_t* row_slot, int32_t n) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  if (n < 0 || n > g->last_T) return fail(AF_ERR_ARG, "n = %d but the last step had %d rows", n, g->last_T);
+  CUDA_TRY(cudaDeviceSynchronize());
+  if (row_req) CUDA_TRY(cudaMemcpy(row_req, g->tb.row_req, n * sizeof(int), cudaMemcpyDeviceToHost));
+  if (row_pos) CUDA_TRY(cudaMemcpy(row_pos, g->tb.row_pos, n * sizeof(int), cudaMemcpyDeviceToHost));
+  if (row_slot) CUDA_TRY(cudaMemcpy(row_slot, g->tb.row_slot, n * sizeof(int), cudaMemcpyDeviceToHost));
+  return AF_OK;
+}
+
+extern "C" int64_t af_debug_launch_count(void) { return g_launches.load(); }
+extern "C" const char* af_last_error(void) { return g_err.c_str(); }
+
+// ------------------------------------------------------------------------------------------------ the packed step
+static int check_weights(const af_weights* w, bool need_lm) {
+  if (!w || !w->layers) return fail(AF_ERR_ARG, "null weights");
+  int rc = check_cfg(&w->cfg);
+  if (rc) return rc;
+  for (int l = 0; l < w->cfg.n_layers; ++l) {
+    const af_layer_weights& L = w->layers[l];
+    if (!L.wq || !L.wk || !L.wv || !L.wo || !L.w_gate || !L.w_up || !L.w_down || !L.g_attn || !L.g_mlp)
+      return fail(AF_ERR_ARG, "null weight pointer in layer %d", l);
+  }
+  if (need_lm && (!w->g_final || !w->w_lm)) return fail(AF_ERR_ARG, "null g_final / w_lm");
+  return AF_OK;
+}
+
+extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
+                                 af_ring* g, float* hidden_out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  if (n_segs < 0) return fail(AF_ERR_ARG, "n_segs < 0");
+  if (n_segs == 0) { g->last_T = 0; return AF_OK; }  // legal no-op
+  if (!segs) return fail(AF_ERR_ARG, "null segment table");
+  if (n_segs > AF_MAX_SEGS) return fail(AF_ERR_SEGMENT, "%d segments > AF_MAX_SEGS", n_segs);
+  int rc = check_weights(w, false);
+  if (rc) return rc;
+  const af_model_cfg& c = w->cfg;
+  if (memcmp(&c, &g->cfg, sizeof c) != 0) return fail(AF_ERR_ARG, "weights cfg differs from the ring's cfg");
+  const int R = g->rc.n_regions, C = g->rc.capacity;
+  // ---- a0 validation on the host mirror, before any launch; same order of checks as the index model ----
+  std::vector<char> seen(R, 0);
+  long long T64 = 0;
+  for (int s = 0; s < n_segs; ++s) {
+    const af_segment& sg = segs[s];
+    if (sg.req_id < 0 || sg.req_id >= R) return fail(AF_ERR_SEGMENT, "segment %d: req_id %d outside [0,%d)", s, sg.req_id, R);
+    if (seen[sg.req_id]) return fail(AF_ERR_SEGMENT, "segment %d: req_id %d appears twice in one step", s, sg.req_id);
+    seen[sg.req_id] = 1;
+    if (sg.len < 1) return fail(AF_ERR_SEGMENT, "segment %d: len %d < 1", s, sg.len);
+    if (sg.phase != AF_PHASE_PREFILL && sg.phase != AF_PHASE_DECODE) return fail(AF_ERR_SEGMENT, "segment %d: phase %d", s, sg.phase);
+    if (sg.phase == AF_PHASE_DECODE && sg.len != 1) return fail(AF_ERR_SEGMENT, "segment %d: decode with len %d", s, sg.len);
+    T64 += sg.len;
+  }
+  for (int s = 0; s < n_segs; ++s)
+    if (segs[s].start_pos != g->len[segs[s].req_id])
+      return fail(AF_ERR_POSITION, "segment %d: start_pos %d != current length %d of request %d", s, segs[s].start_pos,
+                  g->len[segs[s].req_id], segs[s].req_id);
+  for (int s = 0; s < n_segs; ++s)
+    if (static_cast<long long>(segs[s].start_pos) + segs[s].len > C)
+      return fail(AF_ERR_CAPACITY, "segment %d: start_pos %d + len %d > capacity %d", s, segs[s].start_pos, segs[s].len, C);
+  if (T64 > g->max_rows) return fail(AF_ERR_CAPACITY, "%lld packed rows > ring rows %d", T64, g->max_rows);
+  const int T = static_cast<int>(T64);
+  if (!packed_embeds || !hidden_out) return fail(AF_ERR_ARG, "null embeds / hidden_out");
+  if ((reinterpret_cast<uintptr_t>(packed_embeds) & 15) || (reinterpret_cast<uintptr_t>(hidden_out) & 15))
+    return fail(AF_ERR_ARG, "embeds / hidden_out must be 16-byte aligned");
+  Workspace ws;
+  rc = carve(&c, workspace, ws_bytes, T, &ws);
+  if (rc) return rc;
+
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const int D = c.d_model, F = c.ffn, H = c.n_heads, hd = c.head_dim;
+  SegTableArg sta{};
+  sta.n_segs = n_segs; sta.R = R; sta.C = C;
+  int n_items = 0;
+  for (int s = 0; s < n_segs; ++s) {
+    sta.req[s] = segs[s].req_id; sta.start[s] = segs[s].start_pos; sta.len[s] = segs[s].len;
+    sta.base[s] = g->base[segs[s].req_id];
+    n_items += (segs[s].len + ATT_BQ - 1) / ATT_BQ;
+  }
+  rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
+  if ((rc = check_launch("rowmap_kernel"))) return rc;
+  {
+    const size_t n = static_cast<size_t>(T) * D;
+    embed_to_residual_kernel<<<static_cast<unsigned>((n / 4 + 255) / 256), 256, 0, st>>>(
+        reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
+    if ((rc = check_launch("embed_to_residual_kernel"))) return rc;
+  }
+  const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
+  const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
+  for (int l = 0; l < c.n_layers; ++l) {
+    const af_layer_weights& L = w->layers[l];
+    __nv_bfloat16* kvl = g->kv + layer_elems * l;
+    rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, nullptr, D, c.rms_eps);
+    if ((rc = check_launch("rmsnorm_kernel"))) return rc;
+    const void* wqkv[3] = {L.wq, L.wk, L.wv};
+    if ((rc = launch_gemm(st, ws.xn, ws.max_rows, D, wqkv, 3, D, T, EPI_STORE_BF16, ws.qkv, 3 * D, ws.partial))) return rc;
+    rope_append_kernel<<<T, 256, 0, st>>>(ws.qkv, ws.q_rot, kvl, g->rope_tab, g->tb, H, hd, R, C);
+    if ((rc = check_launch("rope_append_kernel"))) return rc;
+    if (hd == 128)
+      attention_kernel<128><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 128 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
+    else
+      attention_kernel<64><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 64 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
+    if ((rc = check_launch("attention_kernel"))) return rc;
+    const void* wo[3] = {L.wo, nullptr, nullptr};
+    if ((rc = launch_gemm(st, ws.attn, ws.max_rows, D, wo, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+    rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, nullptr, D, c.rms_eps);
+    if ((rc = check_launch("rmsnorm_kernel"))) return rc;
+    const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
+    if ((rc = launch_gemm(st, ws.xn, ws.max_rows, D, wgu, 2, F, T, EPI_STORE_BF16, ws.gu, 2 * F, ws.partial))) return rc;
+    {
+      const size_t n = static_cast<size_t>(T) * (F / 8);
+      silu_mul_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(ws.gu, ws.h, T, F);
+      if ((rc = check_launch("silu_mul_kernel"))) return rc;
+    }
+    const void* wd[3] = {L.w_down, nullptr, nullptr};
+    if ((rc = launch_gemm(st, ws.h, ws.max_rows, F, wd, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+  }
+  // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----
+  for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;
+  g->last_T = T;
+  return AF_OK;
+}
+
+extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const int32_t* rows, int32_t n_rows,
+                              float* logits_out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  int rc = check_weights(w, true);
+  if (rc) return rc;
+  if (n_rows == 0) return AF_OK;
+  if (!hidden || !rows || !logits_out || n_rows < 0) return fail(AF_ERR_ARG, "null/negative argument");
+  if (n_rows > 256) return fail(AF_ERR_UNSUPPORTED, "n_rows %d > 256", n_rows);
+  for (int i = 0; i < n_rows; ++i)
+    if (rows[i] < 0) return fail(AF_ERR_ARG, "rows[%d] = %d < 0", i, rows[i]);
+  const af_model_cfg& c = w->cfg;
+  Workspace ws;
+  rc = carve(&c, workspace, ws_bytes, n_rows, &ws);
+  if (rc) return rc;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  // the row list rides in the (otherwise unused here) head of the gate|up buffer; xn holds the normed rows
+  int* rows_dev = reinterpret_cast<int*>(ws.gu);
+  CUDA_TRY(cudaMemcpyAsync(rows_dev, rows, n_rows * sizeof(int), cudaMemcpyHostToDevice, st));
+  rmsnorm_kernel<<<n_rows, 256, 0, st>>>(hidden, reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, rows_dev,
+                                         c.d_model, c.rms_eps);
+  if ((rc = check_launch("rmsnorm_kernel"))) return rc;
+  const void* wl[3] = {w->w_lm, nullptr, nullptr};
+  return launch_gemm(st, ws.xn, ws.max_rows, c.d_model, wl, 1, c.vocab, n_rows, EPI_STORE_F32, logits_out, c.vocab, ws.partial);
+}
+
+extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_t n_tok, int32_t n_out, int32_t k,
+                             void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (!a || !wmat || !out || !workspace) return fail(AF_ERR_ARG, "null argument");
+  if (n_tok <= 0 || n_out <= 0 || k <= 0 || (k % 8)) return fail(AF_ERR_ARG, "bad GEMM shape");
+  if (ws_bytes < gemm_partial_bytes()) return fail(AF_ERR_WORKSPACE, "workspace < %zu bytes", gemm_partial_bytes());
+  const void* wl[3] = {wmat, nullptr, nullptr};
+  return launch_gemm(reinterpret_cast<cudaStream_t>(cuda_stream), a, n_tok, k, wl, 1, n_out, n_tok, EPI_STORE_F32, out,
+                     n_out, reinterpret_cast<float*>(workspace));
+}

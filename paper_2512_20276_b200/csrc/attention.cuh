@@ -1,0 +1,240 @@
+// Segment-masked causal attention over the Unified KV Ring Buffer (step a4; Alg. 2 line 4, P:183,
+// P:194-200).  Each work item is (segment, 64-row query tile) x head.  The tile's rows attend to positions
+// 0..own position of THEIR OWN request only; K/V rows are gathered from the ring at slot (base_r + j) mod C
+// (wrap included) with 128-bit cp.async loads into XOR-swizzled shared memory, S = QK^T and O = PV run on
+// mma.sync.m16n8k16 (bf16 in, fp32 accumulate), and the online softmax reduces across the 4 lanes that share a row
+// with warp shuffles.  KV tiles are walked in LOGICAL position order, so results do not depend on base_r.
+#pragma once
+#include "ptx.cuh"
+
+namespace af {
+
+constexpr int ATT_BQ = 64;
+constexpr int ATT_BKV = 64;
+constexpr int ATT_THREADS = 128;
+
+struct StepTables {      // device arrays written by rowmap_kernel (elementwise.cuh), one set per ring
+  int* seg_req;          // [n_segs]
+  int* seg_start;        // [n_segs] start_pos
+  int* seg_len;          // [n_segs]
+  int* seg_row0;         // [n_segs] first packed row
+  int* seg_base;         // [n_segs] base_r of the segment's region
+  int* row_req;          // [T]
+  int* row_pos;          // [T]
+  int* row_slot;         // [T] global slot id req*C + (base+pos) mod C
+  int* item_seg;         // [n_items] attention work items
+  int* item_q0;          // [n_items]
+};
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid) {
+  const int sz = valid ? 16 : 0;  // src-size 0 => 16 bytes of zeros
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_u32(smem)), "l"(gmem), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void mma_bf16_16816(float* c, const uint32_t* a, uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// byte offset of 16-byte chunk `chunk` of row `row` in a [rows][HD] bf16 tile with XOR swizzle
+template <int HD>
+__device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
+  return static_cast<uint32_t>(row * (HD * 2) + ((chunk ^ (row & 7)) << 4));
+}
+
+template <int HD>
+__global__ void __launch_bounds__(ATT_THREADS)
+attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated queries
+                 const __nv_bfloat16* __restrict__ kv,    // ring, layer base: [2][R][H][C][HD]
+                 __nv_bfloat16* __restrict__ out,         // [T, H*HD]
+                 StepTables tb, int H, int R, int C, float scale_log2) {
+  constexpr int CH = HD / 8;                  // 16-byte chunks per row
+  constexpr int TILE_BYTES = ATT_BKV * HD * 2;
+  extern __shared__ __align__(128) uint8_t att_smem[];
+  uint8_t* sQ = att_smem;
+  uint8_t* sK = sQ + ATT_BQ * HD * 2;         // 2 stages
+  uint8_t* sV = sK + 2 * TILE_BYTES;          // 2 stages
+
+  const int item = blockIdx.x, h = blockIdx.y;
+  const int seg = tb.item_seg[item], q0 = tb.item_q0[item];
+  const int req = tb.seg_req[seg], start = tb.seg_start[seg], len = tb.seg_len[seg];
+  const int row0 = tb.seg_row0[seg], base = tb.seg_base[seg];
+  const int nq = min(ATT_BQ, len - q0);
+  const int kv_end = start + q0 + nq;         // positions [0, kv_end) are visible to the tile's last row
+  const int n_tiles = (kv_end + ATT_BKV - 1) / ATT_BKV;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;
+
+  const size_t head_stride = static_cast<size_t>(C) * HD;
+  const __nv_bfloat16* kbase = kv + (static_cast<size_t>(0 * R + req) * H + h) * head_stride;
+  const __nv_bfloat16* vbase = kv + (static_cast<size_t>(1 * R + req) * H + h) * head_stride;
+
+  // ---- async loads: Q tile, then KV tile 0 ----
+  for (int i = tid; i < ATT_BQ * CH; i += ATT_THREADS) {
+    const int r = i / CH, c = i % CH;
+    const bool ok = r < nq;
+    const __nv_bfloat16* src = q + static_cast<size_t>(row0 + q0 + (ok ? r : 0)) * (H * HD) + h * HD + c * 8;
+    cp_async16(sQ + sw_off<HD>(r, c), src, ok);
+  }
+  auto load_kv = [&](int tile, int stage) {
+    const int j0 = tile * ATT_BKV;
+    for (int i = tid; i < ATT_BKV * CH; i += ATT_THREADS) {
+      const int r = i / CH, c = i % CH;
+      const int j = j0 + r;
+      const bool ok = j < kv_end;
+      int slot = base + (ok ? j : 0);
+      slot = slot >= C ? slot - C : slot;   // (base + j) mod C, base < C and j < C
+      const size_t off = static_cast<size_t>(slot) * HD + c * 8;
+      cp_async16(sK + stage * TILE_BYTES + sw_off<HD>(r, c), kbase + off, ok);
+      cp_async16(sV + stage * TILE_BYTES + sw_off<HD>(r, c), vbase + off, ok);
+    }
+  };
+  load_kv(0, 0);
+  cp_async_commit();
+
+  float o_acc[HD / 8][4];
+#pragma unroll
+  for (int i = 0; i < HD / 8; ++i) { o_acc[i][0] = o_acc[i][1] = o_acc[i][2] = o_acc[i][3] = 0.f; }
+  float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
+  uint32_t qf[HD / 16][4];
+
+  const bool warp_active = warp * 16 < nq;
+  const int p_lo = start + q0 + warp * 16 + g;   // position of this thread's first row (second = +8)
+  const int warp_pmax = start + q0 + warp * 16 + 15;
+
+  for (int tile = 0; tile < n_tiles; ++tile) {
+    const int stage = tile & 1;
+    if (tile + 1 < n_tiles) load_kv(tile + 1, stage ^ 1);
+    cp_async_commit();
+    cp_async_wait<1>();
+    __syncthreads();
+    if (tile == 0) {
+#pragma unroll
+      for (int kk = 0; kk < HD / 16; ++kk) {
+        const int r = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const int c = kk * 2 + (lane >> 4);
+        ldsm_x4(smem_u32(sQ + sw_off<HD>(r, c)), qf[kk][0], qf[kk][1], qf[kk][2], qf[kk][3]);
+      }
+    }
+    const int j0 = tile * ATT_BKV;
+    if (warp_active && j0 <= warp_pmax) {
+      const uint8_t* cK = sK + stage * TILE_BYTES;
+      const uint8_t* cV = sV + stage * TILE_BYTES;
+      float s[ATT_BKV / 8][4];
+#pragma unroll
+      for (int i = 0; i < ATT_BKV / 8; ++i) { s[i][0] = s[i][1] = s[i][2] = s[i][3] = 0.f; }
+#pragma unroll
+      for (int kk = 0; kk < HD / 16; ++kk) {
+#pragma unroll
+        for (int nb = 0; nb < ATT_BKV / 8; nb += 2) {
+          uint32_t b0, b1, b2, b3;
+          const int r = nb * 8 + (lane & 7) + (lane >> 4) * 8;
+          const int c = kk * 2 + ((lane >> 3) & 1);
+          ldsm_x4(smem_u32(cK + sw_off<HD>(r, c)), b0, b1, b2, b3);
+          mma_bf16_16816(s[nb], qf[kk], b0, b1);
+          mma_bf16_16816(s[nb + 1], qf[kk], b2, b3);
+        }
+      }
+      // ---- causal mask within the request + online softmax (base-2 exponent) ----
+      float mx[2] = {-INFINITY, -INFINITY};
+#pragma unroll
+      for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int j = j0 + nb * 8 + 2 * t + (e & 1);
+          const int p = p_lo + (e >> 1) * 8;
+          const float v = (j <= p) ? s[nb][e] * scale_log2 : -INFINITY;
+          s[nb][e] = v;
+          mx[e >> 1] = fmaxf(mx[e >> 1], v);
+        }
+      }
+      float alpha[2];
+#pragma unroll
+      for (int r = 0; r < 2; ++r) {
+        mx[r] = fmaxf(mx[r], __shfl_xor_sync(0xffffffffu, mx[r], 1));
+        mx[r] = fmaxf(mx[r], __shfl_xor_sync(0xffffffffu, mx[r], 2));
+        const float m_new = fmaxf(m_run[r], mx[r]);
+        alpha[r] = (m_new == -INFINITY) ? 1.f : exp2f(m_run[r] - m_new);
+        m_run[r] = m_new;
+        mx[r] = (m_new == -INFINITY) ? 0.f : m_new;  // rows with nothing visible yet
+      }
+      float rs[2] = {0.f, 0.f};
+#pragma unroll
+      for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float pv = exp2f(s[nb][e] - mx[e >> 1]);
+          s[nb][e] = pv;
+          rs[e >> 1] += pv;
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 2; ++r) l_run[r] = l_run[r] * alpha[r] + rs[r];
+#pragma unroll
+      for (int i = 0; i < HD / 8; ++i) {
+        o_acc[i][0] *= alpha[0]; o_acc[i][1] *= alpha[0];
+        o_acc[i][2] *= alpha[1]; o_acc[i][3] *= alpha[1];
+      }
+      // ---- O += P V ----
+#pragma unroll
+      for (int kk = 0; kk < ATT_BKV / 16; ++kk) {
+        uint32_t a[4];
+        a[0] = pack_bf16(s[2 * kk][0], s[2 * kk][1]);
+        a[1] = pack_bf16(s[2 * kk][2], s[2 * kk][3]);
+        a[2] = pack_bf16(s[2 * kk + 1][0], s[2 * kk + 1][1]);
+        a[3] = pack_bf16(s[2 * kk + 1][2], s[2 * kk + 1][3]);
+#pragma unroll
+        for (int db = 0; db < HD / 8; db += 2) {
+          uint32_t b0, b1, b2, b3;
+          const int r = kk * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+          const int c = db + (lane >> 4);
+          ldsm_x4_trans(smem_u32(cV + sw_off<HD>(r, c)), b0, b1, b2, b3);
+          mma_bf16_16816(o_acc[db], a, b0, b1);
+          mma_bf16_16816(o_acc[db + 1], a, b2, b3);
+        }
+      }
+    }
+    __syncthreads();  // everyone is done with this stage before it is refilled
+  }
+  cp_async_wait<0>();
+
+  if (warp_active) {
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 1);
+      l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 2);
+    }
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      const int qi = warp * 16 + g + r * 8;
+      if (qi < nq) {
+        const float inv = 1.f / l_run[r];
+        __nv_bfloat16* dst = out + static_cast<size_t>(row0 + q0 + qi) * (H * HD) + h * HD;
+#pragma unroll
+        for (int db = 0; db < HD / 8; ++db) {
+          *reinterpret_cast<uint32_t*>(dst + db * 8 + 2 * t) =
+              pack_bf16(o_acc[db][2 * r] * inv, o_acc[db][2 * r + 1] * inv);
+        }
+      }
+    }
+  }
+}
+
+}  // namespace af

@@ -1,0 +1,186 @@
+// Row-wise kernels of the packed forward: segment-table ingest (a0), RMSNorm (a1/a6), RoPE + ring append (a3),
+// SiLU*mul (a7 epilogue), logits-row gather + final norm (a10).  SURVEY.md 8(a); Alg. 2 lines 1 and 3.
+#pragma once
+#include "attention.cuh"
+
+namespace af {
+
+struct SegTableArg {  // the host segment table, passed by value as a kernel parameter (no staging copy)
+  int n_segs;
+  int R, C;
+  int req[AF_MAX_SEGS_K], start[AF_MAX_SEGS_K], len[AF_MAX_SEGS_K], base[AF_MAX_SEGS_K];
+};
+
+// a0: every packed row i -> (req, pos = start_pos + i - row0(seg), slot = req*C + (base_r + pos) mod C), plus the
+// per-segment arrays and the attention work list.  One block; all integer, bit-exact by construction (P:208
+// "precomputed physical address").
+__global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_out) {
+  __shared__ int row0[AF_MAX_SEGS_K + 1], item0[AF_MAX_SEGS_K + 1];
+  if (threadIdx.x == 0) {
+    int r = 0, it = 0;
+    for (int s = 0; s < st.n_segs; ++s) {
+      row0[s] = r; item0[s] = it;
+      r += st.len[s];
+      it += (st.len[s] + ATT_BQ - 1) / ATT_BQ;
+    }
+    row0[st.n_segs] = r; item0[st.n_segs] = it;
+    *n_items_out = it;
+  }
+  __syncthreads();
+  for (int s = threadIdx.x; s < st.n_segs; s += blockDim.x) {
+    tb.seg_req[s] = st.req[s]; tb.seg_start[s] = st.start[s]; tb.seg_len[s] = st.len[s];
+    tb.seg_row0[s] = row0[s]; tb.seg_base[s] = st.base[s];
+    const int n_it = item0[s + 1] - item0[s];
+    for (int k = 0; k < n_it; ++k) { tb.item_seg[item0[s] + k] = s; tb.item_q0[item0[s] + k] = k * ATT_BQ; }
+  }
+  const int T = row0[st.n_segs];
+  for (int i = threadIdx.x; i < T; i += blockDim.x) {
+    int s = 0;
+    while (i >= row0[s + 1]) ++s;
+    const int pos = st.start[s] + (i - row0[s]);
+    tb.row_req[i] = st.req[s];
+    tb.row_pos[i] = pos;
+    tb.row_slot[i] = st.req[s] * st.C + (st.base[s] + pos) % st.C;
+  }
+}
+
+// bf16 embeddings -> fp32 residual stream
+__global__ void embed_to_residual_kernel(const __nv_bfloat16* __restrict__ e, float* __restrict__ x, size_t n) {
+  const size_t i = (static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x) * 4;
+  if (i + 3 < n) {
+    const uint2 raw = *reinterpret_cast<const uint2*>(e + i);
+    const __nv_bfloat162 a = *reinterpret_cast<const __nv_bfloat162*>(&raw.x);
+    const __nv_bfloat162 b = *reinterpret_cast<const __nv_bfloat162*>(&raw.y);
+    *reinterpret_cast<float4*>(x + i) =
+        make_float4(__low2float(a), __high2float(a), __low2float(b), __high2float(b));
+  } else {
+    for (size_t k = i; k < n; ++k) x[k] = __bfloat162float(e[k]);
+  }
+}
+
+__device__ __forceinline__ float block_sum(float v, float* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) red[w] = v;
+  __syncthreads();
+  const int nw = blockDim.x >> 5;
+  float t = (l < nw) ? red[l] : 0.f;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+  __syncthreads();
+  return t;
+}
+
+// a1/a6 (and a10's norm when rows != nullptr): y[i,:] = bf16( x[src,:] * g / sqrt(mean(x^2) + eps) ), one block per row.
+__global__ void __launch_bounds__(256)
+rmsnorm_kernel(const float* __restrict__ x, const __nv_bfloat16* __restrict__ g, __nv_bfloat16* __restrict__ y,
+               const int* __restrict__ rows, int D, float eps) {
+  __shared__ float red[32];
+  const int i = blockIdx.x;
+  const int src = rows ? rows[i] : i;
+  const float* xr = x + static_cast<size_t>(src) * D;
+  float ss = 0.f;
+  for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
+    const float4 v = *reinterpret_cast<const float4*>(xr + c);
+    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+  }
+  ss = block_sum(ss, red);
+  const float inv = rsqrtf(ss / D + eps);
+  __nv_bfloat16* yr = y + static_cast<size_t>(i) * D;
+  for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
+    const float4 v = *reinterpret_cast<const float4*>(xr + c);
+    const uint2 graw = *reinterpret_cast<const uint2*>(g + c);
+    const __nv_bfloat162 g0 = *reinterpret_cast<const __nv_bfloat162*>(&graw.x);
+    const __nv_bfloat162 g1 = *reinterpret_cast<const __nv_bfloat162*>(&graw.y);
+    uint2 o;
+    o.x = pack_bf16(v.x * inv * __low2float(g0), v.y * inv * __high2float(g0));
+    o.y = pack_bf16(v.z * inv * __low2float(g1), v.w * inv * __high2float(g1));
+    *reinterpret_cast<uint2*>(yr + c) = o;
+  }
+}
+
+// a3 FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q and k of every (row, head) at the row's logical
+// position in its own request (rotate-half pairing, table built in fp64), write q to the query buffer and
+// k (rotated), v straight to the row's ring slot.  One block per row, 8 elements (16 bytes) per thread-iteration.
+__global__ void __launch_bounds__(256)
+rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q | k | v)
+                   __nv_bfloat16* __restrict__ q_out,       // [T, H*hd]
+                   __nv_bfloat16* __restrict__ kv_layer,    // [2][R][H][C][hd]
+                   const float2* __restrict__ rope_tab,     // [C][hd/2] (cos, sin)
+                   StepTables tb, int H, int hd, int R, int C) {
+  const int i = blockIdx.x;
+  const int pos = tb.row_pos[i], gslot = tb.row_slot[i];
+  const int req = gslot / C, slot = gslot - req * C;
+  const int D = H * hd, half = hd >> 1;
+  const __nv_bfloat16* src = qkv + static_cast<size_t>(i) * 3 * D;
+  const float2* tab = rope_tab + static_cast<size_t>(pos) * half;
+  const int per_head = half / 8;  // 16-byte groups of the low half of a head
+  // q and k: thread handles 8 low-half elements c..c+7 and their partners c+half..
+  for (int w = threadIdx.x; w < 2 * H * per_head; w += blockDim.x) {
+    const int which = w / (H * per_head);           // 0 = q, 1 = k
+    const int rem = w - which * H * per_head;
+    const int h = rem / per_head, c = (rem - h * per_head) * 8;
+    const __nv_bfloat16* s = src + which * D + h * hd + c;
+    const uint4 lo_raw = *reinterpret_cast<const uint4*>(s);
+    const uint4 hi_raw = *reinterpret_cast<const uint4*>(s + half);
+    const __nv_bfloat16* lo = reinterpret_cast<const __nv_bfloat16*>(&lo_raw);
+    const __nv_bfloat16* hi = reinterpret_cast<const __nv_bfloat16*>(&hi_raw);
+    uint4 out_lo, out_hi;
+    uint32_t* ol = reinterpret_cast<uint32_t*>(&out_lo);
+    uint32_t* oh = reinterpret_cast<uint32_t*>(&out_hi);
+#pragma unroll
+    for (int e = 0; e < 8; e += 2) {
+      const float2 cs0 = tab[c + e], cs1 = tab[c + e + 1];
+      const float l0 = __bfloat162float(lo[e]), l1 = __bfloat162float(lo[e + 1]);
+      const float h0 = __bfloat162float(hi[e]), h1 = __bfloat162float(hi[e + 1]);
+      ol[e >> 1] = pack_bf16(l0 * cs0.x - h0 * cs0.y, l1 * cs1.x - h1 * cs1.y);
+      oh[e >> 1] = pack_bf16(h0 * cs0.x + l0 * cs0.y, h1 * cs1.x + l1 * cs1.y);
+    }
+    __nv_bfloat16* dst = (which == 0)
+        ? q_out + static_cast<size_t>(i) * D + h * hd + c
+        : kv_layer + ((static_cast<size_t>(0 * R + req) * H + h) * C + slot) * hd + c;
+    *reinterpret_cast<uint4*>(dst) = out_lo;
+    *reinterpret_cast<uint4*>(dst + half) = out_hi;
+  }
+  // v: plain copy into the ring
+  for (int w = threadIdx.x; w < D / 8; w += blockDim.x) {
+    const int h = (w * 8) / hd, c = (w * 8) - h * hd;
+    const uint4 v = *reinterpret_cast<const uint4*>(src + 2 * D + w * 8);
+    *reinterpret_cast<uint4*>(kv_layer + ((static_cast<size_t>(1 * R + req) * H + h) * C + slot) * hd + c) = v;
+  }
+}
+
+// h[i, f] = bf16( silu(gate[i, f]) * up[i, f] ),  gu = [T, 2F] (gate | up)
+__global__ void silu_mul_kernel(const __nv_bfloat16* __restrict__ gu, __nv_bfloat16* __restrict__ hbuf, int T, int F) {
+  const int per_row = F / 8;
+  const size_t idx = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (idx >= static_cast<size_t>(T) * per_row) return;
+  const int i = static_cast<int>(idx / per_row), c = static_cast<int>(idx - static_cast<size_t>(i) * per_row) * 8;
+  const uint4 graw = *reinterpret_cast<const uint4*>(gu + static_cast<size_t>(i) * 2 * F + c);
+  const uint4 uraw = *reinterpret_cast<const uint4*>(gu + static_cast<size_t>(i) * 2 * F + F + c);
+  const __nv_bfloat16* gp = reinterpret_cast<const __nv_bfloat16*>(&graw);
+  const __nv_bfloat16* up = reinterpret_cast<const __nv_bfloat16*>(&uraw);
+  uint4 o;
+  uint32_t* op = reinterpret_cast<uint32_t*>(&o);
+#pragma unroll
+  for (int e = 0; e < 8; e += 2) {
+    const float g0 = __bfloat162float(gp[e]), g1 = __bfloat162float(gp[e + 1]);
+    const float s0 = g0 / (1.f + __expf(-g0)), s1 = g1 / (1.f + __expf(-g1));
+    op[e >> 1] = pack_bf16(s0 * __bfloat162float(up[e]), s1 * __bfloat162float(up[e + 1]));
+  }
+  *reinterpret_cast<uint4*>(hbuf + static_cast<size_t>(i) * F + c) = o;
+}
+
+// RoPE table in fp64: tab[pos][c] = (cos, sin)(pos * theta^(-2c/hd))
+__global__ void rope_table_kernel(float2* tab, int C, int hd, double theta) {
+  const int half = hd / 2;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= C * half) return;
+  const int pos = idx / half, c = idx - pos * half;
+  const double f = exp2(-2.0 * c / hd * log2(theta));
+  const double a = pos * f;
+  tab[idx] = make_float2(static_cast<float>(cos(a)), static_cast<float>(sin(a)));
+}
+
+}  // namespace af
