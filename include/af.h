@@ -131,6 +131,13 @@ int64_t af_debug_launch_count(void);
 int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32_t n_out, int32_t k,
                   void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* Per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline leg; adds event records
+ * between kernels, so it is switched on only for a separate profiling pass).  Classes, in order: gemm_qkv, gemm_o,
+ * gemm_gateup, gemm_down, gemm_lm, attention, rope_append, rmsnorm, silu_mul, other (10 slots).
+ * af_debug_profile_read synchronises, returns summed milliseconds and launch counts since the last read, and clears. */
+int af_debug_profile(int enable);
+int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
+
 const char* af_last_error(void); /* thread-local message of the last failing call */
 
 #ifdef __cplusplus

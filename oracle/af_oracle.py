@@ -74,13 +74,22 @@ def attend_row(q: torch.Tensor, Kc: torch.Tensor, Vc: torch.Tensor) -> torch.Ten
 class Oracle:
     """Runs each micro-request separately, unpacked, with a private contiguous KV cache per (layer, request)."""
 
-    def __init__(self, cfg, weights: dict, dtype=torch.float64):
+    def __init__(self, cfg, weights: dict, dtype=torch.float64, cache_widened: bool = True):
         self.cfg = cfg
-        self.w = weights            # bf16 (or float) CPU tensors; widened per use
+        self.w = weights            # bf16 (or float) CPU tensors, widened to the working dtype on use
         self.dtype = dtype
+        self._wide = {} if cache_widened else None   # id(tensor) -> widened copy (same values, kept between calls)
         self.K = {}                 # (layer, req) -> [pos, H, hd]
         self.V = {}
         self.len = {}               # req -> tokens cached
+
+    def _widen(self, t: torch.Tensor, dtype) -> torch.Tensor:
+        if self._wide is None or t.dtype == dtype:
+            return t.to(dtype)
+        k = id(t)
+        if k not in self._wide:
+            self._wide[k] = t.to(dtype)
+        return self._wide[k]
 
     # -- request lifecycle -------------------------------------------------------------------------------
     def reset(self, req: int):
@@ -98,8 +107,9 @@ class Oracle:
         cfg, dt = self.cfg, self.dtype
         H, hd = cfg.n_heads, cfg.head_dim
         n = x_in.shape[0]
+        _w = self._widen
         assert start_pos == self.ctx_len(req), "appends must be contiguous (O0)"
-        x = _w(x_in, dt)                                                   # O0
+        x = x_in.to(dt)                                                    # O0
         pos = torch.arange(start_pos, start_pos + n)
         for l in range(cfg.n_layers):
             L = self.w["layers"][l]
@@ -142,6 +152,7 @@ class Oracle:
     def logits(self, hidden: torch.Tensor, rows) -> torch.Tensor:
         """O9 (Alg. 1 l.5/l.8): RMSNorm(hidden[rows]; g_final) W_lm^T."""
         dt = self.dtype
+        _w = self._widen
         h = hidden[list(rows)].to(dt)
         hn = rmsnorm(h, _w(self.w["g_final"], dt), self.cfg.rms_eps)
         return hn @ _w(self.w["w_lm"], dt).T

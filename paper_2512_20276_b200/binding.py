@@ -50,7 +50,10 @@ class af_weights(C.Structure):
 
 EXPORTS = ["af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
-           "af_debug_launch_count", "af_debug_gemm", "af_last_error"]
+           "af_debug_launch_count", "af_debug_gemm", "af_debug_profile", "af_debug_profile_read", "af_last_error"]
+
+PROFILE_CLASSES = ["gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm", "attention", "rope_append",
+                   "rmsnorm", "silu_mul", "other"]
 
 _lib = None
 
@@ -80,6 +83,10 @@ def load_library():
     L.af_debug_launch_count.restype = C.c_int64
     L.af_debug_launch_count.argtypes = []
     L.af_debug_gemm.argtypes = [vp, vp, vp, i32, i32, i32, vp, sz, vp]
+    L.af_debug_profile.argtypes = [C.c_int]
+    L.af_debug_profile.restype = C.c_int
+    L.af_debug_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), i32]
+    L.af_debug_profile_read.restype = C.c_int
     L.af_last_error.restype = C.c_char_p
     L.af_last_error.argtypes = []
     for n in ("af_ring_create", "af_ring_reset_slot", "af_packed_forward", "af_logits_rows", "af_ring_destroy",
@@ -205,3 +212,15 @@ def debug_gemm(a: torch.Tensor, w: torch.Tensor) -> torch.Tensor:
 
 def launch_count() -> int:
     return int(load_library().af_debug_launch_count())
+
+
+def profile(enable: bool):
+    _check(load_library().af_debug_profile(1 if enable else 0))
+
+
+def profile_read() -> dict:
+    """{class: (sum_ms, launches)} since the last read (CUDA events on the launching stream)."""
+    n = len(PROFILE_CLASSES)
+    ms, cnt = (C.c_double * n)(), (C.c_int64 * n)()
+    _check(load_library().af_debug_profile_read(ms, cnt, n))
+    return {k: (ms[i], cnt[i]) for i, k in enumerate(PROFILE_CLASSES)}

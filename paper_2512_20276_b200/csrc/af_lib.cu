@@ -44,6 +44,36 @@ static int check_launch(const char* what) {
   return AF_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ per-kernel timing
+// Optional CUDA-event timing of every launch, by kernel class, on the launching stream (bench.py's roofline leg).
+enum ProfCat { PC_GEMM_QKV = 0, PC_GEMM_O, PC_GEMM_GATEUP, PC_GEMM_DOWN, PC_GEMM_LM, PC_ATTENTION, PC_ROPE_APPEND,
+               PC_RMSNORM, PC_SILU_MUL, PC_OTHER, PC_COUNT };
+struct ProfRec { cudaEvent_t a, b; int cat; };
+static bool g_prof_on = false;
+static std::vector<ProfRec> g_prof;
+struct ProfScope {
+  cudaStream_t st; ProfRec r; bool on;
+  ProfScope(int cat, cudaStream_t s) : st(s), on(g_prof_on) {
+    if (!on) return;
+    r.cat = cat; cudaEventCreate(&r.a); cudaEventCreate(&r.b); cudaEventRecord(r.a, st);
+  }
+  ~ProfScope() { if (on) { cudaEventRecord(r.b, st); g_prof.push_back(r); } }
+};
+extern "C" int af_debug_profile(int enable) { g_prof_on = enable != 0; return AF_OK; }
+extern "C" int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n) {
+  if (!ms_sum || !counts || n < PC_COUNT) return fail(AF_ERR_ARG, "need %d slots", (int)PC_COUNT);
+  CUDA_TRY(cudaDeviceSynchronize());
+  for (int i = 0; i < n; ++i) { ms_sum[i] = 0; counts[i] = 0; }
+  for (auto& r : g_prof) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, r.a, r.b);
+    ms_sum[r.cat] += ms; counts[r.cat] += 1;
+    cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+  }
+  g_prof.clear();
+  return AF_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ tensor maps
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -108,7 +138,7 @@ static int gemm_global_init() {
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
 // out[tok, part*part_rows + f] (op)= sum_k x[tok, k] * w[part][f, k]
-static int launch_gemm(cudaStream_t st, const void* x, int x_rows_cap, int K, const void* const* w, int n_parts,
+static int launch_gemm(int cat, cudaStream_t st, const void* x, int x_rows_cap, int K, const void* const* w, int n_parts,
                        int part_rows, int T, int epi, void* out, int ld_out, float* partial) {
   int rc = gemm_global_init();
   if (rc) return rc;
@@ -141,7 +171,10 @@ static int launch_gemm(cudaStream_t st, const void* x, int x_rows_cap, int K, co
     rc = get_map(x, x_rows_cap, K, p.n1, &mx);
     if (rc) return rc;
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + 1024;
-    gemm_tcgen05_kernel<<<grid, GEMM_THREADS, smem, st>>>(mw[0], mw[1], mw[2], mx, p);
+    {
+      ProfScope ps(cat, st);
+      gemm_tcgen05_kernel<<<grid, GEMM_THREADS, smem, st>>>(mw[0], mw[1], mw[2], mx, p);
+    }
     rc = check_launch("gemm_tcgen05_kernel");
     if (rc) return rc;
   }
@@ -365,12 +398,16 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     sta.base[s] = g->base[segs[s].req_id];
     n_items += (segs[s].len + ATT_BQ - 1) / ATT_BQ;
   }
+  { ProfScope ps_(PC_OTHER, st);
   rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
+  }
   if ((rc = check_launch("rowmap_kernel"))) return rc;
   {
     const size_t n = static_cast<size_t>(T) * D;
+    { ProfScope ps_(PC_OTHER, st);
     embed_to_residual_kernel<<<static_cast<unsigned>((n / 4 + 255) / 256), 256, 0, st>>>(
         reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
+    }
     if ((rc = check_launch("embed_to_residual_kernel"))) return rc;
   }
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
@@ -378,30 +415,42 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   for (int l = 0; l < c.n_layers; ++l) {
     const af_layer_weights& L = w->layers[l];
     __nv_bfloat16* kvl = g->kv + layer_elems * l;
+    { ProfScope ps_(PC_RMSNORM, st);
     rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, nullptr, D, c.rms_eps);
+    }
     if ((rc = check_launch("rmsnorm_kernel"))) return rc;
     const void* wqkv[3] = {L.wq, L.wk, L.wv};
-    if ((rc = launch_gemm(st, ws.xn, ws.max_rows, D, wqkv, 3, D, T, EPI_STORE_BF16, ws.qkv, 3 * D, ws.partial))) return rc;
+    if ((rc = launch_gemm(PC_GEMM_QKV, st, ws.xn, ws.max_rows, D, wqkv, 3, D, T, EPI_STORE_BF16, ws.qkv, 3 * D, ws.partial))) return rc;
+    { ProfScope ps_(PC_ROPE_APPEND, st);
     rope_append_kernel<<<T, 256, 0, st>>>(ws.qkv, ws.q_rot, kvl, g->rope_tab, g->tb, H, hd, R, C);
+    }
     if ((rc = check_launch("rope_append_kernel"))) return rc;
     if (hd == 128)
+      { ProfScope ps_(PC_ATTENTION, st);
       attention_kernel<128><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 128 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
+      }
     else
+      { ProfScope ps_(PC_ATTENTION, st);
       attention_kernel<64><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 64 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
+      }
     if ((rc = check_launch("attention_kernel"))) return rc;
     const void* wo[3] = {L.wo, nullptr, nullptr};
-    if ((rc = launch_gemm(st, ws.attn, ws.max_rows, D, wo, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+    if ((rc = launch_gemm(PC_GEMM_O, st, ws.attn, ws.max_rows, D, wo, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+    { ProfScope ps_(PC_RMSNORM, st);
     rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, nullptr, D, c.rms_eps);
+    }
     if ((rc = check_launch("rmsnorm_kernel"))) return rc;
     const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
-    if ((rc = launch_gemm(st, ws.xn, ws.max_rows, D, wgu, 2, F, T, EPI_STORE_BF16, ws.gu, 2 * F, ws.partial))) return rc;
+    if ((rc = launch_gemm(PC_GEMM_GATEUP, st, ws.xn, ws.max_rows, D, wgu, 2, F, T, EPI_STORE_BF16, ws.gu, 2 * F, ws.partial))) return rc;
     {
       const size_t n = static_cast<size_t>(T) * (F / 8);
+      { ProfScope ps_(PC_SILU_MUL, st);
       silu_mul_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(ws.gu, ws.h, T, F);
+      }
       if ((rc = check_launch("silu_mul_kernel"))) return rc;
     }
     const void* wd[3] = {L.w_down, nullptr, nullptr};
-    if ((rc = launch_gemm(st, ws.h, ws.max_rows, F, wd, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+    if ((rc = launch_gemm(PC_GEMM_DOWN, st, ws.h, ws.max_rows, F, wd, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
   }
   // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----
   for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;
@@ -426,11 +475,13 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   // the row list rides in the (otherwise unused here) head of the gate|up buffer; xn holds the normed rows
   int* rows_dev = reinterpret_cast<int*>(ws.gu);
   CUDA_TRY(cudaMemcpyAsync(rows_dev, rows, n_rows * sizeof(int), cudaMemcpyHostToDevice, st));
+  { ProfScope ps_(PC_RMSNORM, st);
   rmsnorm_kernel<<<n_rows, 256, 0, st>>>(hidden, reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, rows_dev,
                                          c.d_model, c.rms_eps);
+  }
   if ((rc = check_launch("rmsnorm_kernel"))) return rc;
   const void* wl[3] = {w->w_lm, nullptr, nullptr};
-  return launch_gemm(st, ws.xn, ws.max_rows, c.d_model, wl, 1, c.vocab, n_rows, EPI_STORE_F32, logits_out, c.vocab, ws.partial);
+  return launch_gemm(PC_GEMM_LM, st, ws.xn, ws.max_rows, c.d_model, wl, 1, c.vocab, n_rows, EPI_STORE_F32, logits_out, c.vocab, ws.partial);
 }
 
 extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_t n_tok, int32_t n_out, int32_t k,
@@ -439,6 +490,6 @@ extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_
   if (n_tok <= 0 || n_out <= 0 || k <= 0 || (k % 8)) return fail(AF_ERR_ARG, "bad GEMM shape");
   if (ws_bytes < gemm_partial_bytes()) return fail(AF_ERR_WORKSPACE, "workspace < %zu bytes", gemm_partial_bytes());
   const void* wl[3] = {wmat, nullptr, nullptr};
-  return launch_gemm(reinterpret_cast<cudaStream_t>(cuda_stream), a, n_tok, k, wl, 1, n_out, n_tok, EPI_STORE_F32, out,
+  return launch_gemm(PC_OTHER, reinterpret_cast<cudaStream_t>(cuda_stream), a, n_tok, k, wl, 1, n_out, n_tok, EPI_STORE_F32, out,
                      n_out, reinterpret_cast<float*>(workspace));
 }
