@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <string>
@@ -80,12 +81,21 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static std::mutex g_mu;
 static EncodeTiledFn g_encode = nullptr;
-static std::map<std::tuple<const void*, int, int, int>, CUtensorMap> g_maps;
+struct MapKey {
+  const void* ptr; int elem; unsigned long long d[3], st[2]; unsigned b[3]; int rank, swz;
+  bool operator<(const MapKey& o) const { return memcmp(this, &o, sizeof(MapKey)) < 0; }
+};
+static std::map<MapKey, CUtensorMap> g_maps;
 
-// bf16 row-major [rows, cols] matrix, box = [box_rows, 64 cols], 128-byte swizzle, zero fill out of bounds.
-static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+// Cached cuTensorMapEncodeTiled.  dims / box innermost first; strides (bytes) of dims 1..rank-1.
+static int get_map_nd(const void* ptr, int elem_bytes, int rank, const unsigned long long* dims,
+                      const unsigned long long* strides, const unsigned* box, bool swizzle128, CUtensorMap* out) {
   std::lock_guard<std::mutex> lk(g_mu);
-  auto key = std::make_tuple(ptr, rows, cols, box_rows);
+  MapKey key;
+  memset(&key, 0, sizeof key);
+  key.ptr = ptr; key.elem = elem_bytes; key.rank = rank; key.swz = swizzle128;
+  for (int i = 0; i < rank; ++i) { key.d[i] = dims[i]; key.b[i] = box[i]; }
+  for (int i = 0; i + 1 < rank; ++i) key.st[i] = strides[i];
   auto it = g_maps.find(key);
   if (it != g_maps.end()) { *out = it->second; return AF_OK; }
   if (!g_encode) {
@@ -95,28 +105,65 @@ static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
     if (!fn || qres != cudaDriverEntryPointSuccess) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled not available");
     g_encode = reinterpret_cast<EncodeTiledFn>(fn);
   }
-  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || (cols % 8))
-    return fail(AF_ERR_ARG, "matrix %p [%d,%d] must be 16-byte aligned with a 16-byte row pitch", ptr, rows, cols);
+  if (reinterpret_cast<uintptr_t>(ptr) & 15) return fail(AF_ERR_ARG, "matrix %p must be 16-byte aligned", ptr);
+  for (int i = 0; i + 1 < rank; ++i)
+    if (strides[i] % 16) return fail(AF_ERR_ARG, "matrix %p: stride %llu is not a multiple of 16 bytes", ptr, strides[i]);
   CUtensorMap m;
-  cuuint64_t dims[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
-  cuuint64_t strides[1] = {static_cast<cuuint64_t>(cols) * 2};
-  cuuint32_t box[2] = {static_cast<cuuint32_t>(GEMM_BK), static_cast<cuuint32_t>(box_rows)};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled([%d,%d], box %d) -> %d", rows, cols, box_rows, (int)r);
+  cuuint64_t d[3], st[2];
+  cuuint32_t bx[3], estr[3] = {1, 1, 1};
+  for (int i = 0; i < rank; ++i) { d[i] = dims[i]; bx[i] = box[i]; }
+  for (int i = 0; i + 1 < rank; ++i) st[i] = strides[i];
+  const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  CUresult r = g_encode(&m, dt, rank, const_cast<void*>(ptr), d, st, bx, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled(%p, rank %d) -> %d", ptr, rank, (int)r);
   if (g_maps.size() > 8192) g_maps.clear();
   g_maps[key] = m;
   *out = m;
   return AF_OK;
 }
 
-// ------------------------------------------------------------------------------------------------ GEMM launch
+// bf16 row-major [rows, cols] operand matrix, box = [box_rows, 64 cols], 128-byte swizzle, zero fill out of bounds.
+static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+  if (cols % 8) return fail(AF_ERR_ARG, "matrix %p [%d,%d] needs a 16-byte row pitch", ptr, rows, cols);
+  const unsigned long long dims[2] = {static_cast<unsigned long long>(cols), static_cast<unsigned long long>(rows)};
+  const unsigned long long strides[1] = {static_cast<unsigned long long>(cols) * 2};
+  const unsigned box[2] = {static_cast<unsigned>(GEMM_BK), static_cast<unsigned>(box_rows)};
+  return get_map_nd(ptr, 2, 2, dims, strides, box, true, out);
+}
+
+// Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
+struct OutView { void* ptr; int elem_bytes; int features, n_mid, tokens; long long ld_mid, ld_tok; };
+static int get_out_map(const OutView& o, CUtensorMap* out) {
+  const unsigned long long dims[3] = {static_cast<unsigned long long>(o.features), static_cast<unsigned long long>(o.n_mid),
+                                      static_cast<unsigned long long>(o.tokens)};
+  const unsigned long long strides[2] = {static_cast<unsigned long long>(o.ld_mid) * o.elem_bytes,
+                                         static_cast<unsigned long long>(o.ld_tok) * o.elem_bytes};
+  const unsigned box[3] = {32u, 1u, o.elem_bytes == 2 ? 16u : 8u};
+  return get_map_nd(o.ptr, o.elem_bytes, 3, dims, strides, box, false, out);
+}
+
+// ------------------------------------------------------------------------------------------------ launches
+// Every kernel of the step is launched with programmatic dependent launch: its prologue (barrier init, TMEM
+// allocation, tensor-map prefetch, the first weight tiles) overlaps the previous kernel's tail, and each kernel
+// executes griddepcontrol.wait before it touches anything the previous kernel wrote.
+static bool g_use_pdl = true;
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = g_use_pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 static int g_num_sms = 0;
-static int* g_flags = nullptr;  // [256] stream-K epoch flags
-static int g_epoch = 0;
+static int* g_flags = nullptr;  // [GEMM_MAX_GRID] stream-K ready flags (0/1)
 constexpr int GEMM_MAX_GRID = 160;
+constexpr int GEMM_MAX_SPLITS = 4;
 
 static int gemm_global_init() {
   std::lock_guard<std::mutex> lk(g_mu);
@@ -127,19 +174,45 @@ static int gemm_global_init() {
   CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
   if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
   g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
+  if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
   CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448 - 1024));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 128 * 2));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 64 * 2));
   return AF_OK;
 }
 
+// debug timeline of the last TRACE_LAUNCHES GEMM launches (globaltimer stamps per CTA), off unless af_debug_trace(1)
+constexpr int TRACE_LAUNCHES = 16;
+static long long* g_trace = nullptr;
+static int g_trace_n = 0;
+struct TraceMeta { int cat, grid; };
+static TraceMeta g_trace_meta[TRACE_LAUNCHES];
+extern "C" int af_debug_trace(int enable) {
+  if (enable && !g_trace) {
+    CUDA_TRY(cudaMalloc(&g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32));
+    CUDA_TRY(cudaMemset(g_trace, 0, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32));
+  }
+  if (!enable && g_trace) { cudaFree(g_trace); g_trace = nullptr; }
+  g_trace_n = 0;
+  return AF_OK;
+}
+// out: [TRACE_LAUNCHES][160][32] int64 stamps; meta: [TRACE_LAUNCHES][2] (class, grid); returns launches recorded
+extern "C" int af_debug_trace_read(long long* out, int* meta) {
+  if (!g_trace || !out || !meta) return fail(AF_ERR_ARG, "trace is off");
+  CUDA_TRY(cudaDeviceSynchronize());
+  CUDA_TRY(cudaMemcpy(out, g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < TRACE_LAUNCHES; ++i) { meta[2 * i] = g_trace_meta[i].cat; meta[2 * i + 1] = g_trace_meta[i].grid; }
+  return g_trace_n;
+}
+
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
-// out[tok, part*part_rows + f] (op)= sum_k x[tok, k] * w[part][f, k]
-static int launch_gemm(int cat, cudaStream_t st, const void* x, int x_rows_cap, int K, const void* const* w, int n_parts,
-                       int part_rows, int T, int epi, void* out, int ld_out, float* partial) {
+// One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
+// layout (n_parts / part_rows / a_pair), the split mode and the epilogue fields; the decomposition is filled here.
+static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView& ov, const void* x, int x_rows_cap,
+                       const void* const* w, int T) {
   int rc = gemm_global_init();
   if (rc) return rc;
   if (T <= 0) return AF_OK;
@@ -147,33 +220,58 @@ static int launch_gemm(int cat, cudaStream_t st, const void* x, int x_rows_cap, 
   const int chunk = (T + n_chunks - 1) / n_chunks;
   for (int tok0 = 0; tok0 < T; tok0 += chunk) {
     const int Tc = (T - tok0 < chunk) ? (T - tok0) : chunk;
-    GemmParams p{};
+    GemmParams p = proto;
     int n_pad = (Tc + 15) / 16 * 16;
     if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
     else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
-    p.n_parts = n_parts; p.part_rows = part_rows; p.tiles_per_part = (part_rows + GEMM_BM - 1) / GEMM_BM;
-    p.K = K; p.num_kb = (K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
-    p.total_units = n_parts * p.tiles_per_part * p.num_kb;
-    int grid = p.total_units < g_num_sms ? p.total_units : g_num_sms;
-    p.units_per_cta = (p.total_units + grid - 1) / grid;
-    grid = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+    const int box_rows = p.a_pair ? 64 : GEMM_BM;
+    const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
+    p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
+    p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
+    p.total_units = n_tiles * p.num_kb;
+    int grid;
+    if (p.split == SPLIT_K) {
+      int s = g_num_sms / n_tiles;
+      if (s > GEMM_MAX_SPLITS) s = GEMM_MAX_SPLITS;
+      if (s > p.num_kb) s = p.num_kb;
+      if (s < 1) s = 1;
+      p.splits = s; p.units_per_cta = 0;
+      grid = n_tiles * s;
+    } else {
+      grid = p.total_units < g_num_sms ? p.total_units : g_num_sms;
+      p.units_per_cta = (p.total_units + grid - 1) / grid;
+      grid = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+      p.splits = 1;
+    }
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + n_pad * GEMM_BK * 2;
-    int stages = (232448 - 1024 - 1024) / stage_bytes;
-    if (stages > 12) stages = 12;
+    int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_XCH_BYTES) / stage_bytes;
+    if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
     if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
-    p.stages = stages; p.epi = epi; p.out = out; p.ld_out = ld_out; p.partial = partial; p.flags = g_flags;
-    p.epoch = ++g_epoch;
+    p.stages = stages; p.flags = g_flags;
+    { const char* d = getenv("AF_DBG"); p.dbg = d ? atoi(d) : 0; }
+    if (g_trace) { p.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * 32; g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {cat, grid}; ++g_trace_n; }
     CUtensorMap mw[3], mx;
     for (int i = 0; i < 3; ++i) {
-      rc = get_map(w[i < n_parts ? i : 0], part_rows, K, GEMM_BM, &mw[i]);
+      const int n_w = p.a_pair ? 2 : p.n_parts;
+      rc = get_map(w[i < n_w ? i : 0], p.part_rows, p.K, box_rows, &mw[i]);
       if (rc) return rc;
     }
-    rc = get_map(x, x_rows_cap, K, p.n1, &mx);
+    rc = get_map(x, x_rows_cap, p.K, p.n1, &mx);
     if (rc) return rc;
-    const size_t smem = static_cast<size_t>(stages) * stage_bytes + 1024;
+    CUtensorMap mo, mp;
+    p.out_bf16 = ov.elem_bytes == 2;
+    if ((rc = get_out_map(ov, &mo))) return rc;
+    {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
+      const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
+      const unsigned long long strides[2] = {GEMM_BM * 4ull, GEMM_BM * 4ull * GEMM_MAX_TOK};
+      const unsigned box[3] = {32u, 8u, 1u};
+      if ((rc = get_map_nd(p.partial, 4, 3, dims, strides, box, false, &mp))) return rc;
+    }
+    const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_XCH_BYTES + 1024;
     {
       ProfScope ps(cat, st);
-      gemm_tcgen05_kernel<<<grid, GEMM_THREADS, smem, st>>>(mw[0], mw[1], mw[2], mx, p);
+      cudaError_t e = launch_k(gemm_tcgen05_kernel, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
+      if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gemm_tcgen05_kernel failed: %s", cudaGetErrorString(e));
     }
     rc = check_launch("gemm_tcgen05_kernel");
     if (rc) return rc;
@@ -215,9 +313,10 @@ extern "C" size_t af_ring_bytes(const af_model_cfg* c, const af_ring_cfg* r) {
 // workspace = fixed part (stream-K partials) + per-row part; the carve depends only on (pointer, bytes)
 static size_t ws_per_row(const af_model_cfg* c) {
   const size_t D = c->d_model, F = c->ffn;
-  return align_up((D + 3 * D + D + D + 2 * F + F) * 2, 256);  // xn, qkv, q_rot, attn, gate|up, h  (bf16)
+  // xn, qkv, q_rot, attn, h (bf16) + split-K partial slabs of the O / down projections (fp32)
+  return align_up((D + 3 * D + D + D + F) * 2 + GEMM_MAX_SPLITS * D * 4, 256);
 }
-static size_t ws_fixed() { return align_up(gemm_partial_bytes(), 256) + 6 * 256; }
+static size_t ws_fixed() { return align_up(gemm_partial_bytes(), 256) + 8 * 256; }
 
 extern "C" size_t af_workspace_bytes(const af_model_cfg* c, int32_t max_rows, int32_t max_segs) {
   (void)max_segs;
@@ -227,8 +326,9 @@ extern "C" size_t af_workspace_bytes(const af_model_cfg* c, int32_t max_rows, in
 }
 
 struct Workspace {
-  float* partial;
-  __nv_bfloat16 *xn, *qkv, *q_rot, *attn, *gu, *h;
+  float* partial;        // stream-K partials [grid][n_pad][128]
+  float* split;          // split-K slabs [GEMM_MAX_SPLITS][max_rows][D]
+  __nv_bfloat16 *xn, *qkv, *q_rot, *attn, *h;
   int max_rows;
 };
 static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, Workspace* o) {
@@ -243,11 +343,11 @@ static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, W
   const size_t D = c->d_model, F = c->ffn;
   auto take = [&](size_t n) { uint8_t* q = p; p += align_up(n, 256); return q; };
   o->partial = reinterpret_cast<float*>(take(gemm_partial_bytes()));
+  o->split = reinterpret_cast<float*>(take(GEMM_MAX_SPLITS * rows * D * 4));
   o->xn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
   o->qkv = reinterpret_cast<__nv_bfloat16*>(take(rows * 3 * D * 2));
   o->q_rot = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
   o->attn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
-  o->gu = reinterpret_cast<__nv_bfloat16*>(take(rows * 2 * F * 2));
   o->h = reinterpret_cast<__nv_bfloat16*>(take(rows * F * 2));
   o->max_rows = static_cast<int>(rows);
   return AF_OK;
@@ -398,60 +498,100 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     sta.base[s] = g->base[segs[s].req_id];
     n_items += (segs[s].len + ATT_BQ - 1) / ATT_BQ;
   }
+  cudaError_t le;
+#define AF_LAUNCH(cat, name, ...)                                                                              \
+  do {                                                                                                         \
+    { ProfScope ps_(cat, st); le = launch_k(__VA_ARGS__); }                                                    \
+    if (le != cudaSuccess) return fail(AF_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(le)); \
+    if ((rc = check_launch(name))) return rc;                                                                  \
+  } while (0)
   { ProfScope ps_(PC_OTHER, st);
   rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
   }
   if ((rc = check_launch("rowmap_kernel"))) return rc;
   {
     const size_t n = static_cast<size_t>(T) * D;
-    { ProfScope ps_(PC_OTHER, st);
-    embed_to_residual_kernel<<<static_cast<unsigned>((n / 4 + 255) / 256), 256, 0, st>>>(
-        reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
-    }
-    if ((rc = check_launch("embed_to_residual_kernel"))) return rc;
+    AF_LAUNCH(PC_OTHER, "embed_to_residual_kernel", embed_to_residual_kernel,
+              dim3(static_cast<unsigned>((n / 4 + 255) / 256)), dim3(256), 0, st,
+              reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
   }
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
+  const long long split_stride = static_cast<long long>(ws.max_rows) * D;
+  int prev_splits = 0;   // split-K slabs of the previous projection still to be added to the residual stream
+  auto split_count = [&](int n_tiles, int K) {
+    int s2 = g_num_sms / n_tiles, nkb = (K + GEMM_BK - 1) / GEMM_BK;
+    if (s2 > GEMM_MAX_SPLITS) s2 = GEMM_MAX_SPLITS;
+    if (s2 > nkb) s2 = nkb;
+    return s2 < 1 ? 1 : s2;
+  };
+  const int d_tiles = (D + GEMM_BM - 1) / GEMM_BM;
   for (int l = 0; l < c.n_layers; ++l) {
     const af_layer_weights& L = w->layers[l];
     __nv_bfloat16* kvl = g->kv + layer_elems * l;
-    { ProfScope ps_(PC_RMSNORM, st);
-    rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, nullptr, D, c.rms_eps);
-    }
-    if ((rc = check_launch("rmsnorm_kernel"))) return rc;
-    const void* wqkv[3] = {L.wq, L.wk, L.wv};
-    if ((rc = launch_gemm(PC_GEMM_QKV, st, ws.xn, ws.max_rows, D, wqkv, 3, D, T, EPI_STORE_BF16, ws.qkv, 3 * D, ws.partial))) return rc;
-    { ProfScope ps_(PC_ROPE_APPEND, st);
-    rope_append_kernel<<<T, 256, 0, st>>>(ws.qkv, ws.q_rot, kvl, g->rope_tab, g->tb, H, hd, R, C);
-    }
-    if ((rc = check_launch("rope_append_kernel"))) return rc;
-    if (hd == 128)
-      { ProfScope ps_(PC_ATTENTION, st);
-      attention_kernel<128><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 128 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
-      }
-    else
-      { ProfScope ps_(PC_ATTENTION, st);
-      attention_kernel<64><<<dim3(n_items, H), ATT_THREADS, 5 * ATT_BQ * 64 * 2, st>>>(ws.q_rot, kvl, ws.attn, g->tb, H, R, C, scale_log2);
-      }
-    if ((rc = check_launch("attention_kernel"))) return rc;
-    const void* wo[3] = {L.wo, nullptr, nullptr};
-    if ((rc = launch_gemm(PC_GEMM_O, st, ws.attn, ws.max_rows, D, wo, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
-    { ProfScope ps_(PC_RMSNORM, st);
-    rmsnorm_kernel<<<T, 256, 0, st>>>(hidden_out, reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, nullptr, D, c.rms_eps);
-    }
-    if ((rc = check_launch("rmsnorm_kernel"))) return rc;
-    const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
-    if ((rc = launch_gemm(PC_GEMM_GATEUP, st, ws.xn, ws.max_rows, D, wgu, 2, F, T, EPI_STORE_BF16, ws.gu, 2 * F, ws.partial))) return rc;
+    // a8(prev) + a1: x += down partials; xn = RMSNorm(x; g_attn)
+    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+              static_cast<const float*>(ws.split), prev_splits, split_stride,
+              reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, D, c.rms_eps);
+    // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
     {
-      const size_t n = static_cast<size_t>(T) * (F / 8);
-      { ProfScope ps_(PC_SILU_MUL, st);
-      silu_mul_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(ws.gu, ws.h, T, F);
-      }
-      if ((rc = check_launch("silu_mul_kernel"))) return rc;
+      GemmParams gp{};
+      gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
+      gp.partial = ws.partial;
+      const OutView ov{ws.qkv, 2, D, 3, T, D, 3LL * D};
+      const void* wqkv[3] = {L.wq, L.wk, L.wv};
+      if ((rc = launch_gemm(PC_GEMM_QKV, st, gp, ov, ws.xn, ws.max_rows, wqkv, T))) return rc;
     }
-    const void* wd[3] = {L.w_down, nullptr, nullptr};
-    if ((rc = launch_gemm(PC_GEMM_DOWN, st, ws.h, ws.max_rows, F, wd, 1, D, T, EPI_RESIDUAL_F32, hidden_out, D, ws.partial))) return rc;
+    // a3: FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q, k at the row's position; k, v go straight to the ring slot
+    AF_LAUNCH(PC_ROPE_APPEND, "rope_append_kernel", rope_append_kernel, dim3(T), dim3(256), 0, st,
+              static_cast<const __nv_bfloat16*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
+              H, hd, R, C);
+    // a4: segment-masked causal attention over the ring
+    if (hd == 128)
+      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(n_items, H), dim3(ATT_THREADS),
+                5 * ATT_BQ * 128 * 2, st, static_cast<const __nv_bfloat16*>(ws.q_rot),
+                static_cast<const __nv_bfloat16*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
+    else
+      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(n_items, H), dim3(ATT_THREADS),
+                5 * ATT_BQ * 64 * 2, st, static_cast<const __nv_bfloat16*>(ws.q_rot),
+                static_cast<const __nv_bfloat16*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
+    // a5: O projection, split-K slabs (added to the residual by the next kernel)
+    {
+      GemmParams gp{};
+      gp.n_parts = 1; gp.part_rows = D; gp.K = D; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
+      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D};
+      const void* wo[3] = {L.wo, nullptr, nullptr};
+      if ((rc = launch_gemm(PC_GEMM_O, st, gp, ov, ws.attn, ws.max_rows, wo, T))) return rc;
+      prev_splits = split_count(d_tiles, D);
+    }
+    // a5 residual + a6: x += O partials; xn = RMSNorm(x; g_mlp)
+    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+              static_cast<const float*>(ws.split), prev_splits, split_stride,
+              reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, D, c.rms_eps);
+    // a7: gate/up projection with the fused SiLU*mul epilogue
+    {
+      GemmParams gp{};
+      gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
+      gp.partial = ws.partial;
+      const OutView ov{ws.h, 2, F, 1, T, F, F};
+      const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
+      if ((rc = launch_gemm(PC_GEMM_GATEUP, st, gp, ov, ws.xn, ws.max_rows, wgu, T))) return rc;
+    }
+    // a8: down projection, split-K slabs
+    {
+      GemmParams gp{};
+      gp.n_parts = 1; gp.part_rows = D; gp.K = F; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
+      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D};
+      const void* wd[3] = {L.w_down, nullptr, nullptr};
+      if ((rc = launch_gemm(PC_GEMM_DOWN, st, gp, ov, ws.h, ws.max_rows, wd, T))) return rc;
+      prev_splits = split_count(d_tiles, F);
+    }
   }
+  // a8 of the last layer: x += down partials (no norm: hidden_out is the pre-final-norm residual stream)
+  AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+            static_cast<const float*>(ws.split), prev_splits, split_stride, static_cast<const __nv_bfloat16*>(nullptr),
+            static_cast<__nv_bfloat16*>(nullptr), D, c.rms_eps);
+#undef AF_LAUNCH
   // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----
   for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;
   g->last_T = T;
@@ -472,16 +612,22 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   rc = carve(&c, workspace, ws_bytes, n_rows, &ws);
   if (rc) return rc;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  // the row list rides in the (otherwise unused here) head of the gate|up buffer; xn holds the normed rows
-  int* rows_dev = reinterpret_cast<int*>(ws.gu);
-  CUDA_TRY(cudaMemcpyAsync(rows_dev, rows, n_rows * sizeof(int), cudaMemcpyHostToDevice, st));
-  { ProfScope ps_(PC_RMSNORM, st);
-  rmsnorm_kernel<<<n_rows, 256, 0, st>>>(hidden, reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, rows_dev,
-                                         c.d_model, c.rms_eps);
+  RowListArg rl{};
+  for (int i = 0; i < n_rows; ++i) rl.rows[i] = rows[i];
+  {
+    ProfScope ps_(PC_RMSNORM, st);
+    cudaError_t le = launch_k(gather_norm_kernel, dim3(n_rows), dim3(256), 0, st, rl, hidden,
+                              reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, c.d_model, c.rms_eps);
+    if (le != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gather_norm_kernel failed: %s", cudaGetErrorString(le));
   }
-  if ((rc = check_launch("rmsnorm_kernel"))) return rc;
+  if ((rc = check_launch("gather_norm_kernel"))) return rc;
+  GemmParams gp{};
+  gp.n_parts = 1; gp.part_rows = c.vocab; gp.K = c.d_model; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
+  gp.partial = ws.partial;
+  if (c.vocab % 4) return fail(AF_ERR_UNSUPPORTED, "vocab must be a multiple of 4 (16-byte logits rows)");
+  const OutView ov{logits_out, 4, c.vocab, 1, n_rows, c.vocab, c.vocab};
   const void* wl[3] = {w->w_lm, nullptr, nullptr};
-  return launch_gemm(PC_GEMM_LM, st, ws.xn, ws.max_rows, c.d_model, wl, 1, c.vocab, n_rows, EPI_STORE_F32, logits_out, c.vocab, ws.partial);
+  return launch_gemm(PC_GEMM_LM, st, gp, ov, ws.xn, ws.max_rows, wl, n_rows);
 }
 
 extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_t n_tok, int32_t n_out, int32_t k,
@@ -489,7 +635,11 @@ extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_
   if (!a || !wmat || !out || !workspace) return fail(AF_ERR_ARG, "null argument");
   if (n_tok <= 0 || n_out <= 0 || k <= 0 || (k % 8)) return fail(AF_ERR_ARG, "bad GEMM shape");
   if (ws_bytes < gemm_partial_bytes()) return fail(AF_ERR_WORKSPACE, "workspace < %zu bytes", gemm_partial_bytes());
+  GemmParams gp{};
+  gp.n_parts = 1; gp.part_rows = n_out; gp.K = k; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
+  gp.partial = reinterpret_cast<float*>(workspace);
+  if (n_out % 4) return fail(AF_ERR_ARG, "n_out must be a multiple of 4");
+  const OutView ov{out, 4, n_out, 1, n_tok, n_out, n_out};
   const void* wl[3] = {wmat, nullptr, nullptr};
-  return launch_gemm(PC_OTHER, reinterpret_cast<cudaStream_t>(cuda_stream), a, n_tok, k, wl, 1, n_out, n_tok, EPI_STORE_F32, out,
-                     n_out, reinterpret_cast<float*>(workspace));
+  return launch_gemm(PC_OTHER, reinterpret_cast<cudaStream_t>(cuda_stream), gp, ov, a, n_tok, wl, n_tok);
 }

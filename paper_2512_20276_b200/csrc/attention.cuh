@@ -72,6 +72,8 @@ attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated q
   uint8_t* sK = sQ + ATT_BQ * HD * 2;         // 2 stages
   uint8_t* sV = sK + 2 * TILE_BYTES;          // 2 stages
 
+  pdl_wait();
+  pdl_launch_dependents();
   const int item = blockIdx.x, h = blockIdx.y;
   const int seg = tb.item_seg[item], q0 = tb.item_q0[item];
   const int req = tb.seg_req[seg], start = tb.seg_start[seg], len = tb.seg_len[seg];

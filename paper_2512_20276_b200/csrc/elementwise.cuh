@@ -1,5 +1,6 @@
-// Row-wise kernels of the packed forward: segment-table ingest (a0), RMSNorm (a1/a6), RoPE + ring append (a3),
-// SiLU*mul (a7 epilogue), logits-row gather + final norm (a10).  SURVEY.md 8(a); Alg. 2 lines 1 and 3.
+// Row-wise kernels of the packed forward: segment-table ingest (a0), residual + RMSNorm (a5/a8 + a1/a6),
+// RoPE + ring append (a3), logits-row gather + final norm (a10), RoPE table.  SURVEY.md 8(a); Alg. 2 lines 1 and 3
+// (P:180-182).  SiLU*mul (a7) is an epilogue of the GEMM kernel (gemm_tcgen05.cuh).
 #pragma once
 #include "attention.cuh"
 
@@ -46,6 +47,8 @@ __global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_
 
 // bf16 embeddings -> fp32 residual stream
 __global__ void embed_to_residual_kernel(const __nv_bfloat16* __restrict__ e, float* __restrict__ x, size_t n) {
+  pdl_wait();
+  pdl_launch_dependents();
   const size_t i = (static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x) * 4;
   if (i + 3 < n) {
     const uint2 raw = *reinterpret_cast<const uint2*>(e + i);
@@ -72,24 +75,33 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
   return t;
 }
 
-// a1/a6 (and a10's norm when rows != nullptr): y[i,:] = bf16( x[src,:] * g / sqrt(mean(x^2) + eps) ), one block per row.
-__global__ void __launch_bounds__(256)
-rmsnorm_kernel(const float* __restrict__ x, const __nv_bfloat16* __restrict__ g, __nv_bfloat16* __restrict__ y,
-               const int* __restrict__ rows, int D, float eps) {
+// a5/a8 residual + a1/a6 RMSNorm in one pass (and a10's norm when rows != nullptr), one block per row:
+//   x[i,:] += sum_s parts[s][i,:]      the split-K partials of the preceding O / down projection, in split order
+//   y[i,:]  = bf16( x[src,:] * g / sqrt(mean(x^2) + eps) )          (skipped when g == nullptr: reduce only)
+__device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const float* __restrict__ parts, int n_parts,
+                                                  long long part_stride, const __nv_bfloat16* __restrict__ g,
+                                                  __nv_bfloat16* __restrict__ y, int i, int src, int D, float eps) {
   __shared__ float red[32];
-  const int i = blockIdx.x;
-  const int src = rows ? rows[i] : i;
-  const float* xr = x + static_cast<size_t>(src) * D;
+  float* xr = x + static_cast<size_t>(src) * D;
   float ss = 0.f;
   for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
-    const float4 v = *reinterpret_cast<const float4*>(xr + c);
+    float4 v = *reinterpret_cast<const float4*>(xr + c);
+    if (n_parts > 0) {
+      const float* pr = parts + static_cast<size_t>(src) * D + c;
+      for (int s = 0; s < n_parts; ++s) {
+        const float4 a = __ldcg(reinterpret_cast<const float4*>(pr + s * part_stride));
+        v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
+      }
+      *reinterpret_cast<float4*>(xr + c) = v;
+    }
     ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
   }
+  if (!g) return;
   ss = block_sum(ss, red);
   const float inv = rsqrtf(ss / D + eps);
   __nv_bfloat16* yr = y + static_cast<size_t>(i) * D;
   for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
-    const float4 v = *reinterpret_cast<const float4*>(xr + c);
+    const float4 v = *reinterpret_cast<const float4*>(xr + c);   // this thread's own writes (same addresses)
     const uint2 graw = *reinterpret_cast<const uint2*>(g + c);
     const __nv_bfloat162 g0 = *reinterpret_cast<const __nv_bfloat162*>(&graw.x);
     const __nv_bfloat162 g1 = *reinterpret_cast<const __nv_bfloat162*>(&graw.y);
@@ -98,6 +110,25 @@ rmsnorm_kernel(const float* __restrict__ x, const __nv_bfloat16* __restrict__ g,
     o.y = pack_bf16(v.z * inv * __low2float(g1), v.w * inv * __high2float(g1));
     *reinterpret_cast<uint2*>(yr + c) = o;
   }
+}
+
+__global__ void __launch_bounds__(256)
+residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int n_parts, long long part_stride,
+                     const __nv_bfloat16* __restrict__ g, __nv_bfloat16* __restrict__ y, int D, float eps) {
+  pdl_wait();
+  pdl_launch_dependents();
+  residual_norm_row(x, parts, n_parts, part_stride, g, y, blockIdx.x, blockIdx.x, D, eps);
+}
+
+struct RowListArg { int rows[256]; };  // a10: the caller's row list, passed by value (no staging copy)
+
+// a10: y[i,:] = bf16( RMSNorm(hidden[rows[i],:]; g_final) ), the input of the LM-head GEMM
+__global__ void __launch_bounds__(256)
+gather_norm_kernel(const RowListArg rl, const float* __restrict__ x, const __nv_bfloat16* __restrict__ g,
+                   __nv_bfloat16* __restrict__ y, int D, float eps) {
+  pdl_wait();
+  pdl_launch_dependents();
+  residual_norm_row(const_cast<float*>(x), nullptr, 0, 0, g, y, blockIdx.x, rl.rows[blockIdx.x], D, eps);
 }
 
 // a3 FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q and k of every (row, head) at the row's logical
@@ -109,6 +140,8 @@ rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q |
                    __nv_bfloat16* __restrict__ kv_layer,    // [2][R][H][C][hd]
                    const float2* __restrict__ rope_tab,     // [C][hd/2] (cos, sin)
                    StepTables tb, int H, int hd, int R, int C) {
+  pdl_wait();
+  pdl_launch_dependents();
   const int i = blockIdx.x;
   const int pos = tb.row_pos[i], gslot = tb.row_slot[i];
   const int req = gslot / C, slot = gslot - req * C;
@@ -149,27 +182,6 @@ rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q |
     const uint4 v = *reinterpret_cast<const uint4*>(src + 2 * D + w * 8);
     *reinterpret_cast<uint4*>(kv_layer + ((static_cast<size_t>(1 * R + req) * H + h) * C + slot) * hd + c) = v;
   }
-}
-
-// h[i, f] = bf16( silu(gate[i, f]) * up[i, f] ),  gu = [T, 2F] (gate | up)
-__global__ void silu_mul_kernel(const __nv_bfloat16* __restrict__ gu, __nv_bfloat16* __restrict__ hbuf, int T, int F) {
-  const int per_row = F / 8;
-  const size_t idx = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-  if (idx >= static_cast<size_t>(T) * per_row) return;
-  const int i = static_cast<int>(idx / per_row), c = static_cast<int>(idx - static_cast<size_t>(i) * per_row) * 8;
-  const uint4 graw = *reinterpret_cast<const uint4*>(gu + static_cast<size_t>(i) * 2 * F + c);
-  const uint4 uraw = *reinterpret_cast<const uint4*>(gu + static_cast<size_t>(i) * 2 * F + F + c);
-  const __nv_bfloat16* gp = reinterpret_cast<const __nv_bfloat16*>(&graw);
-  const __nv_bfloat16* up = reinterpret_cast<const __nv_bfloat16*>(&uraw);
-  uint4 o;
-  uint32_t* op = reinterpret_cast<uint32_t*>(&o);
-#pragma unroll
-  for (int e = 0; e < 8; e += 2) {
-    const float g0 = __bfloat162float(gp[e]), g1 = __bfloat162float(gp[e + 1]);
-    const float s0 = g0 / (1.f + __expf(-g0)), s1 = g1 / (1.f + __expf(-g1));
-    op[e >> 1] = pack_bf16(s0 * __bfloat162float(up[e]), s1 * __bfloat162float(up[e + 1]));
-  }
-  *reinterpret_cast<uint4*>(hbuf + static_cast<size_t>(i) * F + c) = o;
 }
 
 // RoPE table in fp64: tab[pos][c] = (cos, sin)(pos * theta^(-2c/hd))

@@ -1,0 +1,356 @@
+// Body of gemm_tcgen05.cuh (kept in a second file only to keep each file short); see the header for the design.
+
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_constant__ CUtensorMap map_w1,
+                    const __grid_constant__ CUtensorMap map_w2, const __grid_constant__ CUtensorMap map_x,
+                    const __grid_constant__ CUtensorMap map_out, const __grid_constant__ CUtensorMap map_part,
+                    const GemmParams p) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  // 1024-byte aligned tile area (the 128-byte swizzle pattern repeats every 1024 bytes)
+  uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int n_pad = p.n1 + p.n2;
+  const uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
+  const uint32_t b_bytes = static_cast<uint32_t>(n_pad) * GEMM_BK * 2;
+  const uint32_t stage_bytes = a_bytes + b_bytes;
+  float* xch = reinterpret_cast<float*>(tiles + static_cast<size_t>(p.stages) * stage_bytes);
+
+  __shared__ uint64_t full_bar[GEMM_MAX_STAGES], empty_bar[GEMM_MAX_STAGES], tmem_full_bar, tmem_empty_bar, fix_bar;
+  __shared__ uint32_t tmem_base_smem;
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int cta = blockIdx.x;
+  long long* trace = p.trace ? p.trace + static_cast<size_t>(cta) * 32 : nullptr;
+#define AF_TRACE(slot) do { if (trace) trace[slot] = static_cast<long long>(globaltimer_ns()); } while (0)
+  if (trace && threadIdx.x == 0) AF_TRACE(0);
+
+  if (warp == GEMM_EPI_WARPS && lane == 0) {
+    tma_prefetch_desc(&map_w0);
+    if (p.n_parts > 1 || p.a_pair) tma_prefetch_desc(&map_w1);
+    if (p.n_parts > 2) tma_prefetch_desc(&map_w2);
+    tma_prefetch_desc(&map_x);
+    tma_prefetch_desc(&map_out);
+    tma_prefetch_desc(&map_part);
+    for (int s = 0; s < p.stages; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], 1);
+    }
+    mbar_init(&tmem_full_bar, 1);
+    mbar_init(&tmem_empty_bar, GEMM_EPI_WARPS);
+    mbar_init(&fix_bar, 1);
+    fence_barrier_init();
+  }
+  if (warp == GEMM_EPI_WARPS + 1) tmem_alloc(&tmem_base_smem, GEMM_TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+  pdl_launch_dependents();  // dependents still wait (griddepcontrol.wait) for this whole grid before reading its output
+
+  int u_begin, u_end;
+  if (p.split == SPLIT_K) {
+    const int tile = cta / p.splits, s = cta - tile * p.splits;
+    u_begin = tile * p.num_kb + static_cast<int>(static_cast<long long>(s) * p.num_kb / p.splits);
+    u_end = tile * p.num_kb + static_cast<int>(static_cast<long long>(s + 1) * p.num_kb / p.splits);
+  } else {
+    u_begin = min(cta * p.units_per_cta, p.total_units);
+    u_end = min(u_begin + p.units_per_cta, p.total_units);
+  }
+
+  if (warp == GEMM_EPI_WARPS) {
+    // ================================ TMA producer ================================
+    if (lane == 0) {
+      const uint64_t pol_w = policy_evict_first();  // weights are streamed once per step
+      const uint64_t pol_x = policy_evict_last();   // the packed activations are re-read by every CTA
+      // SPLIT_K: CTAs of one split would sweep the same k-blocks in lockstep; rotate each tile's sweep instead
+      const int rot_lo = u_begin % p.num_kb, rot_len = u_end - u_begin;
+      const int rot = (p.split == SPLIT_K && (p.dbg & 16)) ? ((u_begin / p.num_kb) * 5) % rot_len : 0;
+      auto kb_of = [&](int u) {
+        const int kb = u % p.num_kb;
+        return rot ? rot_lo + (kb - rot_lo + rot) % rot_len : kb;
+      };
+      auto load_w = [&](int u, int stage) {
+        const int tile = u / p.num_kb, kb = kb_of(u);
+        uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
+        if (p.a_pair) {
+          tma_load_2d(sa, &map_w0, &full_bar[stage], kb * GEMM_BK, tile * 64, pol_w);
+          tma_load_2d(sa + a_bytes / 2, &map_w1, &full_bar[stage], kb * GEMM_BK, tile * 64, pol_w);
+        } else {
+          const int part = tile / p.tiles_per_part, tip = tile - part * p.tiles_per_part;
+          const CUtensorMap* mw = part == 0 ? &map_w0 : (part == 1 ? &map_w1 : &map_w2);
+          tma_load_2d(sa, mw, &full_bar[stage], kb * GEMM_BK, tip * GEMM_BM, pol_w);
+        }
+      };
+      auto load_x = [&](int u, int stage) {
+        const int kb = kb_of(u);
+        uint8_t* sb = tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes;
+        tma_load_2d(sb, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0, pol_x);
+        if (p.n2 > 0)
+          tma_load_2d(sb + static_cast<size_t>(p.n1) * GEMM_BK * 2, &map_x, &full_bar[stage], kb * GEMM_BK,
+                      p.tok0 + p.n1, pol_x);
+      };
+      // The weights do not depend on the previous kernel: start streaming them before the PDL dependency resolves.
+      const int n_pre = min(p.stages, u_end - u_begin);
+      for (int i = 0; i < n_pre; ++i) {
+        mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
+        load_w(u_begin + i, i);
+      }
+      AF_TRACE(24);
+      pdl_wait();
+      AF_TRACE(25);
+      for (int i = 0; i < n_pre; ++i) load_x(u_begin + i, i);
+      int stage = n_pre == p.stages ? 0 : n_pre;
+      uint32_t phase = n_pre == p.stages ? 1 : 0;
+      for (int u = u_begin + n_pre; u < u_end; ++u) {
+        mbar_wait(&empty_bar[stage], phase ^ 1);
+        mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
+        load_w(u, stage);
+        load_x(u, stage);
+        if (++stage == p.stages) { stage = 0; phase ^= 1; }
+      }
+      AF_TRACE(26);
+    }
+  } else if (warp == GEMM_EPI_WARPS + 1) {
+    // ================================ MMA issuer (one thread) ================================
+    if (lane == 0) {
+      const uint32_t idesc1 = umma_idesc_bf16(GEMM_BM, p.n1);
+      const uint32_t idesc2 = umma_idesc_bf16(GEMM_BM, p.n2 > 0 ? p.n2 : 16);
+      int stage = 0;
+      uint32_t phase = 0, acc_phase = 0;
+      int u = u_begin;
+      while (u < u_end) {
+        const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
+        const int kb1 = min(p.num_kb, kb0 + (u_end - u));
+        mbar_wait(&tmem_empty_bar, acc_phase ^ 1);  // epilogue has drained the accumulator
+        tc_fence_after();
+        for (int kb = kb0; kb < kb1; ++kb) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
+          const uint32_t sb = sa + a_bytes;
+          const uint64_t da = umma_smem_desc_sw128(sa);
+          const uint64_t db1 = umma_smem_desc_sw128(sb);
+          const uint64_t db2 = umma_smem_desc_sw128(sb + p.n1 * GEMM_BK * 2);
+#pragma unroll
+          for (int k = 0; k < GEMM_BK / 16; ++k) {
+            const uint32_t accum = (kb > kb0 || k > 0) ? 1u : 0u;
+            // advancing 16 bf16 = 32 bytes along K inside the swizzle row: +2 in the (addr >> 4) field
+            umma_bf16(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
+            if (p.n2 > 0) umma_bf16(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
+          }
+          umma_commit(&empty_bar[stage]);  // frees the smem slot when these MMAs have read it
+          if (++stage == p.stages) { stage = 0; phase ^= 1; }
+        }
+        umma_commit(&tmem_full_bar);  // accumulator complete -> epilogue
+        acc_phase ^= 1;
+        u += kb1 - kb0;
+      }
+    }
+  } else {
+    // ================================ epilogue warps 0..7 ================================
+    // Warp w reads TMEM lanes [32*(w%4), +32) = 32 output features; the two warps of a quadrant alternate 16-token
+    // chunks.  Per chunk: TMEM -> registers -> the warp's private, double-buffered 1 KB staging buffer -> global with
+    // a TMA tensor store ([tokens][32 features] box).  No epilogue warp waits for another (except the gate/up pairing
+    // of EPI_SWIGLU and the stream-K fix-up loads) and the LSU is not involved.
+    const int quad = warp & 3, par = warp >> 2;
+    const int row = quad * 32 + lane;
+    const int etid = threadIdx.x;  // 0..255
+    uint8_t* stg = reinterpret_cast<uint8_t*>(xch) + warp * 2048;
+    uint32_t n_st = 0;  // stores issued by this warp (buffer = n_st & 1)
+    auto stage_buf = [&]() { return stg + (n_st & 1) * 1024; };
+    auto stage_store = [&](const CUtensorMap* m, int c0_, int c1_, int c2_) {
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) {
+        tma_store_3d(m, stage_buf(), c0_, c1_, c2_);
+        bulk_commit();
+        bulk_wait_read<1>();  // the store before this one has finished reading the other buffer
+      }
+      ++n_st;
+      __syncwarp();
+    };
+    pdl_wait();
+    if (etid == 0) AF_TRACE(1);
+    int piece = 0;
+    const int stage_area = p.stages * static_cast<int>(stage_bytes);
+    uint32_t acc_phase = 0, fix_phase = 0, n_sub = 0;
+    int u = u_begin;
+    while (u < u_end) {
+      const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
+      const int kb1 = min(p.num_kb, kb0 + (u_end - u));
+      const bool streamk = p.split == SPLIT_STREAMK;
+      const bool contributor = streamk && kb0 > 0;
+      const bool owner_partial = streamk && (kb0 == 0) && (kb1 < p.num_kb);
+      int c_first = 0, n_contrib = 0;
+      if (owner_partial) {
+        // CTAs holding the rest of this tile: cta+1 .. while their range starts before the tile ends
+        c_first = cta + 1;
+        const int tile_end = (tile + 1) * p.num_kb;
+        const int c_last = min((tile_end - 1) / p.units_per_cta, static_cast<int>(gridDim.x) - 1);
+        n_contrib = c_last - c_first + 1;
+        if (etid < n_contrib) {
+          volatile int* f = p.flags + c_first + etid;
+          while (*f == 0) {
+          }
+          *f = 0;  // one consumer per flag: ready for the next launch (graph-replay safe)
+          __threadfence();
+        }
+        AF_EPI_BAR();
+      }
+      if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
+      mbar_wait(&tmem_full_bar, acc_phase);
+      tc_fence_after();
+      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
+      // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
+      int f0, mid;
+      if (p.a_pair) {
+        f0 = tile * 64 + (quad & 1) * 32; mid = 0;
+      } else {
+        const int part = tile / p.tiles_per_part;
+        f0 = (tile - part * p.tiles_per_part) * GEMM_BM + quad * 32;
+        mid = p.split == SPLIT_K ? cta % p.splits : part;
+      }
+      // column blocks: with contributors, their partial columns [b0, b1) are bulk-copied into the (now idle) stages,
+      // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 32-column blocks
+      int blk_cols = n_pad, grp = n_contrib, n_groups = n_contrib > 0 ? 1 : 0;
+      if (n_contrib > 0) {
+        const int grp_max = stage_area / (32 * GEMM_BM * 4);
+        if (n_contrib > grp_max) {
+          grp = grp_max; blk_cols = 32; n_groups = (n_contrib + grp - 1) / grp;
+        } else {
+          blk_cols = (stage_area / (n_contrib * GEMM_BM * 4)) / 32 * 32;
+          if (blk_cols > n_pad) blk_cols = n_pad;
+        }
+      }
+      const float* fix = reinterpret_cast<const float*>(tiles);
+      bool fix_used = false;
+      auto load_group = [&](int g0, int cnt, int b0, int b1) {
+        if (fix_used) AF_EPI_BAR();  // everyone is done reading what the buffer held
+        fix_used = true;
+        if (etid == 0) {
+          const uint32_t bytes = static_cast<uint32_t>(b1 - b0) * GEMM_BM * 4;
+          fence_proxy_async_all();
+          mbar_arrive_expect_tx(&fix_bar, bytes * cnt);
+          for (int c = 0; c < cnt; ++c)
+            bulk_load_1d(tiles + static_cast<size_t>(c) * bytes,
+                         p.partial + (static_cast<size_t>(c_first + g0 + c) * GEMM_MAX_TOK + b0) * GEMM_BM, bytes,
+                         &fix_bar);
+        }
+        mbar_wait(&fix_bar, fix_phase);
+        fix_phase ^= 1;
+      };
+      auto load_acc = [&](int c0, float* v) {
+        uint32_t r[16];
+        tmem_ld16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0, r);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) v[j] = __uint_as_float(r[j]);
+      };
+      auto add_fix = [&](int cnt, int b0, int b1, int c0, float* v) {
+        for (int c = 0; c < cnt; ++c) {
+          const float* q = fix + (static_cast<size_t>(c) * (b1 - b0) + (c0 - b0)) * GEMM_BM + row;
+#pragma unroll
+          for (int j = 0; j < 16; ++j) v[j] += q[j * GEMM_BM];
+        }
+      };
+      auto finish_chunk = [&](int c0, float* v) {
+        if (contributor) {  // fp32 partial [cta][token][128 features], two 8-token stores
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            float* sb = reinterpret_cast<float*>(stage_buf());
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sb[j * 32 + lane] = v[hh * 8 + j];
+            stage_store(&map_part, quad * 32, c0 + hh * 8, cta);
+          }
+        } else if (p.epi == EPI_STORE) {
+          if (p.out_bf16) {
+            __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stage_buf());
+#pragma unroll
+            for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = __float2bfloat16_rn(v[j]);
+            stage_store(&map_out, f0, mid, p.tok0 + c0);
+          } else {
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+              float* sb = reinterpret_cast<float*>(stage_buf());
+#pragma unroll
+              for (int j = 0; j < 8; ++j) sb[j * 32 + lane] = v[hh * 8 + j];
+              stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 8);
+            }
+          }
+        } else if (quad >= 2) {  // EPI_SWIGLU, up half: hand the values to the gate warp of the same features
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh, ++n_sub) {
+            float* xb = reinterpret_cast<float*>(stg + (n_sub & 1) * 1024);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) xb[j * 32 + lane] = v[hh * 8 + j];
+            asm volatile("bar.sync %0, 64;\n" ::"r"(2 + (quad & 1) + 2 * par) : "memory");
+          }
+        } else {                 // EPI_SWIGLU, gate half
+          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stage_buf());
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh, ++n_sub) {
+            asm volatile("bar.sync %0, 64;\n" ::"r"(2 + (quad & 1) + 2 * par) : "memory");
+            const float* xb = reinterpret_cast<const float*>(stg + 2 * 2048 + (n_sub & 1) * 1024);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const float g = v[hh * 8 + j];
+              sb[(hh * 8 + j) * 32 + lane] = __float2bfloat16_rn(g / (1.f + __expf(-g)) * xb[j * 32 + lane]);
+            }
+          }
+          stage_store(&map_out, f0, mid, p.tok0 + c0);
+        }
+      };
+      for (int b0 = 0; b0 < n_pad && b0 < p.T; b0 += blk_cols) {
+        const int b1 = min(b0 + blk_cols, n_pad);
+        float v[16];
+        if (n_groups <= 1) {
+          if (n_groups == 1) {
+            load_group(0, n_contrib, b0, b1);
+            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
+          }
+          for (int c0 = b0 + 16 * par; c0 < b1 && c0 < p.T; c0 += 32) {
+            load_acc(c0, v);
+            if (n_groups == 1) add_fix(n_contrib, b0, b1, c0, v);
+            finish_chunk(c0, v);
+          }
+        } else {  // 32-column block: at most one chunk per warp; every warp takes part in every group load
+          const int c0 = b0 + 16 * par;
+          const bool has = c0 < b1 && c0 < p.T;
+          if (has) load_acc(c0, v);
+          for (int g0 = 0; g0 < n_contrib; g0 += grp) {
+            const int cnt = min(grp, n_contrib - g0);
+            load_group(g0, cnt, b0, b1);
+            if (has) add_fix(cnt, b0, b1, c0, v);
+          }
+          if (has) finish_chunk(c0, v);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&tmem_empty_bar);
+      if (contributor) {
+        if (lane == 0) { bulk_wait<0>(); fence_proxy_async_all(); }  // this warp's partial stores are complete
+        __syncwarp();
+        __threadfence();
+        AF_EPI_BAR();
+        if (etid == 0) {
+          __threadfence();
+          atomicExch(p.flags + cta, 1);
+        }
+      }
+      if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
+      ++piece;
+      acc_phase ^= 1;
+      u += kb1 - kb0;
+    }
+    if (lane == 0) bulk_wait<0>();  // all output stores are complete before the CTA exits
+  }
+#undef AF_TRACE
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == GEMM_EPI_WARPS + 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, GEMM_TMEM_COLS);
+  }
+}
