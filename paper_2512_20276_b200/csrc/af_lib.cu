@@ -134,13 +134,13 @@ static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
 }
 
 // Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
-struct OutView { void* ptr; int elem_bytes; int features, n_mid, tokens; long long ld_mid, ld_tok; };
+struct OutView { void* ptr; int elem_bytes; int features, n_mid, tokens; long long ld_mid, ld_tok; int box_feat; };
 static int get_out_map(const OutView& o, CUtensorMap* out) {
   const unsigned long long dims[3] = {static_cast<unsigned long long>(o.features), static_cast<unsigned long long>(o.n_mid),
                                       static_cast<unsigned long long>(o.tokens)};
   const unsigned long long strides[2] = {static_cast<unsigned long long>(o.ld_mid) * o.elem_bytes,
                                          static_cast<unsigned long long>(o.ld_tok) * o.elem_bytes};
-  const unsigned box[3] = {32u, 1u, o.elem_bytes == 2 ? 16u : 8u};
+  const unsigned box[3] = {static_cast<unsigned>(o.box_feat), 1u, 32u};
   return get_map_nd(o.ptr, o.elem_bytes, 3, dims, strides, box, false, out);
 }
 
@@ -224,7 +224,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     int n_pad = (Tc + 15) / 16 * 16;
     if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
     else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
-    const int box_rows = p.a_pair ? 64 : GEMM_BM;
+    const int box_rows = p.a_pair ? 16 : GEMM_BM;
     const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
     p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
@@ -264,7 +264,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
       const unsigned long long strides[2] = {GEMM_BM * 4ull, GEMM_BM * 4ull * GEMM_MAX_TOK};
-      const unsigned box[3] = {32u, 8u, 1u};
+      const unsigned box[3] = {32u, 32u, 1u};
       if ((rc = get_map_nd(p.partial, 4, 3, dims, strides, box, false, &mp))) return rc;
     }
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_XCH_BYTES + 1024;
@@ -538,7 +538,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
       GemmParams gp{};
       gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
       gp.partial = ws.partial;
-      const OutView ov{ws.qkv, 2, D, 3, T, D, 3LL * D};
+      const OutView ov{ws.qkv, 2, D, 3, T, D, 3LL * D, 32};
       const void* wqkv[3] = {L.wq, L.wk, L.wv};
       if ((rc = launch_gemm(PC_GEMM_QKV, st, gp, ov, ws.xn, ws.max_rows, wqkv, T))) return rc;
     }
@@ -559,7 +559,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     {
       GemmParams gp{};
       gp.n_parts = 1; gp.part_rows = D; gp.K = D; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
-      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D};
+      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wo[3] = {L.wo, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_O, st, gp, ov, ws.attn, ws.max_rows, wo, T))) return rc;
       prev_splits = split_count(d_tiles, D);
@@ -573,7 +573,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
       GemmParams gp{};
       gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
       gp.partial = ws.partial;
-      const OutView ov{ws.h, 2, F, 1, T, F, F};
+      const OutView ov{ws.h, 2, F, 1, T, F, F, 16};
       const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
       if ((rc = launch_gemm(PC_GEMM_GATEUP, st, gp, ov, ws.xn, ws.max_rows, wgu, T))) return rc;
     }
@@ -581,7 +581,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     {
       GemmParams gp{};
       gp.n_parts = 1; gp.part_rows = D; gp.K = F; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
-      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D};
+      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wd[3] = {L.w_down, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_DOWN, st, gp, ov, ws.h, ws.max_rows, wd, T))) return rc;
       prev_splits = split_count(d_tiles, F);
@@ -625,7 +625,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   gp.n_parts = 1; gp.part_rows = c.vocab; gp.K = c.d_model; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
   gp.partial = ws.partial;
   if (c.vocab % 4) return fail(AF_ERR_UNSUPPORTED, "vocab must be a multiple of 4 (16-byte logits rows)");
-  const OutView ov{logits_out, 4, c.vocab, 1, n_rows, c.vocab, c.vocab};
+  const OutView ov{logits_out, 4, c.vocab, 1, n_rows, c.vocab, c.vocab, 32};
   const void* wl[3] = {w->w_lm, nullptr, nullptr};
   return launch_gemm(PC_GEMM_LM, st, gp, ov, ws.xn, ws.max_rows, wl, n_rows);
 }
@@ -639,7 +639,7 @@ extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_
   gp.n_parts = 1; gp.part_rows = n_out; gp.K = k; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
   gp.partial = reinterpret_cast<float*>(workspace);
   if (n_out % 4) return fail(AF_ERR_ARG, "n_out must be a multiple of 4");
-  const OutView ov{out, 4, n_out, 1, n_tok, n_out, n_out};
+  const OutView ov{out, 4, n_out, 1, n_tok, n_out, n_out, 32};
   const void* wl[3] = {wmat, nullptr, nullptr};
   return launch_gemm(PC_OTHER, reinterpret_cast<cudaStream_t>(cuda_stream), gp, ov, a, n_tok, wl, n_tok);
 }

@@ -17,11 +17,12 @@
 //                  [split][token][feature] and the NEXT kernel (residual + RMSNorm, elementwise.cuh) adds them in
 //                  split order.  No CTA ever waits on another.
 //
-// Epilogues (features sit on TMEM lanes, tokens on columns): every warp stages its 32 features x 16 tokens in shared
-// memory and writes them with one TMA tensor store, bf16 or fp32.
+// Epilogues (features sit on TMEM lanes, tokens on columns): every warp stages its 32 features x 32 tokens in shared
+// memory and writes them with TMA tensor stores, bf16 or fp32.
 //   EPI_STORE      plain store (q|k|v, split-K slabs, logits).
-//   EPI_SWIGLU     tile = 64 gate rows + 64 up rows of the same features; warps 2,3 hand their up values to warps 0,1
-//                  through shared memory, which write bf16(silu(gate) * up).
+//   EPI_SWIGLU     tile = 64 gate rows + 64 up rows of the same features, loaded so that every lane quadrant holds
+//                  16 gate + 16 up rows of the same 16 features: the pairing is a warp shuffle, the output is
+//                  bf16(silu(gate) * up).
 //
 // Warp roles (320 threads): warps 0-7 epilogue (TMEM lane quadrant = warp % 4, two warps per quadrant alternate
 // 16-token chunks), warp 8 TMA producer, warp 9 MMA issuer.
@@ -37,7 +38,7 @@ constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
-constexpr int GEMM_XCH_BYTES = GEMM_EPI_WARPS * 2 * 1024;  // per epilogue warp: two 1 KB staging buffers for the TMA stores
+constexpr int GEMM_XCH_BYTES = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB staging buffers for the TMA stores
 constexpr int GEMM_SMEM_BUDGET = 232448 - 1024;    // dynamic shared memory: 227 KB minus the static part
 
 enum GemmEpilogue : int { EPI_STORE = 0, EPI_SWIGLU = 1 };
@@ -50,7 +51,7 @@ struct GemmParams {
   int n_parts;         // weight matrices stacked along the feature axis (q|k|v): 1..3 (when a_pair == 0)
   int part_rows;       // output features per part (a_pair: rows of gate = rows of up)
   int tiles_per_part;  // ceil(part_rows / 128)
-  int a_pair;          // 1: tile t = rows [64t, 64t+64) of map_w0 (gate) on lanes 0-63 + of map_w1 (up) on lanes 64-127
+  int a_pair;          // 1: tile t = rows [64t, 64t+64) of map_w0 (gate) and of map_w1 (up), interleaved 16 + 16 per lane quadrant
   int K, num_kb;       // reduction length, ceil(K / 64)
   int T, tok0;         // valid tokens of this launch, first token row
   int n1, n2;          // UMMA N of the two token halves (multiples of 16, n2 may be 0)
@@ -59,7 +60,7 @@ struct GemmParams {
   int total_units, units_per_cta;  // SPLIT_STREAMK
   int stages;
   int epi;             // GemmEpilogue
-  int out_bf16;        // EPI_STORE: 1 = bf16 output (box 32 x 16 tokens), 0 = fp32 (box 32 x 8 tokens)
+  int out_bf16;        // EPI_STORE: 1 = bf16 output (box 32 features x 32 tokens), 0 = fp32 (same box)
   float* partial;      // [grid][288][128] fp32 stream-K partials (written through map_part)
   int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
   int dbg;

@@ -7,7 +7,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
                     const GemmParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // 1024-byte aligned tile area (the 128-byte swizzle pattern repeats every 1024 bytes)
-  uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  // (offset arithmetic on the __shared__ array, not an integer round trip, so the compiler keeps the shared address space)
+  uint8_t* tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   const int n_pad = p.n1 + p.n2;
   const uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
   const uint32_t b_bytes = static_cast<uint32_t>(n_pad) * GEMM_BK * 2;
@@ -72,9 +73,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       auto load_w = [&](int u, int stage) {
         const int tile = u / p.num_kb, kb = kb_of(u);
         uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
-        if (p.a_pair) {
-          tma_load_2d(sa, &map_w0, &full_bar[stage], kb * GEMM_BK, tile * 64, pol_w);
-          tma_load_2d(sa + a_bytes / 2, &map_w1, &full_bar[stage], kb * GEMM_BK, tile * 64, pol_w);
+        if (p.a_pair) {  // every TMEM lane quadrant = 16 gate rows + the 16 up rows of the same features
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            tma_load_2d(sa + q * 4096, &map_w0, &full_bar[stage], kb * GEMM_BK, tile * 64 + q * 16, pol_w);
+            tma_load_2d(sa + q * 4096 + 2048, &map_w1, &full_bar[stage], kb * GEMM_BK, tile * 64 + q * 16, pol_w);
+          }
         } else {
           const int part = tile / p.tiles_per_part, tip = tile - part * p.tiles_per_part;
           const CUtensorMap* mw = part == 0 ? &map_w0 : (part == 1 ? &map_w1 : &map_w2);
@@ -148,32 +152,41 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     }
   } else {
     // ================================ epilogue warps 0..7 ================================
-    // Warp w reads TMEM lanes [32*(w%4), +32) = 32 output features; the two warps of a quadrant alternate 16-token
-    // chunks.  Per chunk: TMEM -> registers -> the warp's private, double-buffered 1 KB staging buffer -> global with
-    // a TMA tensor store ([tokens][32 features] box).  No epilogue warp waits for another (except the gate/up pairing
-    // of EPI_SWIGLU and the stream-K fix-up loads) and the LSU is not involved.
+    // Warp w reads TMEM lanes [32*(w%4), +32) = 32 output features; the two warps of a quadrant alternate 32-token
+    // chunks.  Per chunk: TMEM -> registers -> the warp's private 2 KB staging buffer -> global with TMA tensor stores
+    // ([tokens][features] boxes).  No epilogue warp waits for another (except for the stream-K fix-up loads) and the
+    // LSU is not involved.  EPI_SWIGLU pairs gate and up inside the warp (lanes l and l+16) with shuffles.
     const int quad = warp & 3, par = warp >> 2;
     const int row = quad * 32 + lane;
     const int etid = threadIdx.x;  // 0..255
-    uint8_t* stg = reinterpret_cast<uint8_t*>(xch) + warp * 2048;
-    uint32_t n_st = 0;  // stores issued by this warp (buffer = n_st & 1)
-    auto stage_buf = [&]() { return stg + (n_st & 1) * 1024; };
+    uint8_t* stg_base = reinterpret_cast<uint8_t*>(xch) + warp * 8192;
+    uint32_t n_st = 0;  // TMA stores issued by this warp; buffer = n_st & 1
+#define stg (stg_base + (n_st & 1) * 4096)
+    long long tk[6] = {0, 0, 0, 0, 0, 0};
+    long long tk0 = 0;
+#define AF_TICK(i) do { if (trace) { const long long t_ = clock64(); tk[i] += t_ - tk0; tk0 = t_; } } while (0)
+    auto stage_free = [&]() {  // the TMA stores issued by this warp have finished reading the staging buffer
+      AF_TICK(2);
+      if (lane == 0) bulk_wait_read<1>();  // all but the latest store (which reads the other buffer) are done reading
+      __syncwarp();
+      AF_TICK(3);
+    };
     auto stage_store = [&](const CUtensorMap* m, int c0_, int c1_, int c2_) {
       fence_proxy_async();
       __syncwarp();
+      AF_TICK(4);
       if (lane == 0) {
-        tma_store_3d(m, stage_buf(), c0_, c1_, c2_);
+        tma_store_3d(m, stg, c0_, c1_, c2_);
         bulk_commit();
-        bulk_wait_read<1>();  // the store before this one has finished reading the other buffer
       }
       ++n_st;
-      __syncwarp();
+      AF_TICK(5);
     };
     pdl_wait();
     if (etid == 0) AF_TRACE(1);
     int piece = 0;
     const int stage_area = p.stages * static_cast<int>(stage_bytes);
-    uint32_t acc_phase = 0, fix_phase = 0, n_sub = 0;
+    uint32_t acc_phase = 0, fix_phase = 0;
     int u = u_begin;
     while (u < u_end) {
       const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
@@ -204,21 +217,21 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
       int f0, mid;
       if (p.a_pair) {
-        f0 = tile * 64 + (quad & 1) * 32; mid = 0;
+        f0 = tile * 64 + quad * 16; mid = 0;
       } else {
         const int part = tile / p.tiles_per_part;
         f0 = (tile - part * p.tiles_per_part) * GEMM_BM + quad * 32;
         mid = p.split == SPLIT_K ? cta % p.splits : part;
       }
       // column blocks: with contributors, their partial columns [b0, b1) are bulk-copied into the (now idle) stages,
-      // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 32-column blocks
+      // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 64-column blocks
       int blk_cols = n_pad, grp = n_contrib, n_groups = n_contrib > 0 ? 1 : 0;
       if (n_contrib > 0) {
-        const int grp_max = stage_area / (32 * GEMM_BM * 4);
+        const int grp_max = stage_area / (64 * GEMM_BM * 4);
         if (n_contrib > grp_max) {
-          grp = grp_max; blk_cols = 32; n_groups = (n_contrib + grp - 1) / grp;
+          grp = grp_max; blk_cols = 64; n_groups = (n_contrib + grp - 1) / grp;
         } else {
-          blk_cols = (stage_area / (n_contrib * GEMM_BM * 4)) / 32 * 32;
+          blk_cols = (stage_area / (n_contrib * GEMM_BM * 4)) / 64 * 64;
           if (blk_cols > n_pad) blk_cols = n_pad;
         }
       }
@@ -239,90 +252,86 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         mbar_wait(&fix_bar, fix_phase);
         fix_phase ^= 1;
       };
-      auto load_acc = [&](int c0, float* v) {
-        uint32_t r[16];
-        tmem_ld16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0, r);
+      auto load_acc = [&](int c0, int cw, float* v) {
+        uint32_t r[32];
+        if (trace) tk0 = clock64();
+        const uint32_t ta = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0;
+        tmem_ld16(ta, r);
+        if (cw > 16) tmem_ld16(ta + 16, r + 16);
         tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = __uint_as_float(r[j]);
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+        AF_TICK(0);
       };
       auto add_fix = [&](int cnt, int b0, int b1, int c0, float* v) {
+        // (a 16-wide last chunk over-reads 16 columns of the staging area; those columns are never stored)
         for (int c = 0; c < cnt; ++c) {
           const float* q = fix + (static_cast<size_t>(c) * (b1 - b0) + (c0 - b0)) * GEMM_BM + row;
 #pragma unroll
-          for (int j = 0; j < 16; ++j) v[j] += q[j * GEMM_BM];
+          for (int h2 = 0; h2 < 2; ++h2) {
+            float t[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) t[j] = q[(h2 * 16 + j) * GEMM_BM];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) v[h2 * 16 + j] += t[j];
+          }
         }
       };
-      auto finish_chunk = [&](int c0, float* v) {
-        if (contributor) {  // fp32 partial [cta][token][128 features], two 8-token stores
+      auto finish_chunk = [&](int c0, int cw, float* v) {
+        if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
+          // fp32, one 32-token box: stream-K partial [cta][token][128 features] or the fp32 output
+          stage_free();
+          float* sb = reinterpret_cast<float*>(stg);
 #pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
-            float* sb = reinterpret_cast<float*>(stage_buf());
+          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
+          if (contributor) stage_store(&map_part, quad * 32, c0, cta);
+          else stage_store(&map_out, f0, mid, p.tok0 + c0);
+        } else if (p.epi == EPI_STORE) {  // bf16, one 32-token box
+          stage_free();
+          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stg);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) sb[j * 32 + lane] = v[hh * 8 + j];
-            stage_store(&map_part, quad * 32, c0 + hh * 8, cta);
-          }
-        } else if (p.epi == EPI_STORE) {
-          if (p.out_bf16) {
-            __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stage_buf());
+          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __float2bfloat16_rn(v[j]);
+          stage_store(&map_out, f0, mid, p.tok0 + c0);
+        } else {
+          // EPI_SWIGLU: lanes 0-15 hold gate, lanes 16-31 hold up of the same 16 features.  Lanes 0-15 finish tokens
+          // 0-15 of the chunk, lanes 16-31 tokens 16-31; each gets the other half's operand with one shuffle.
+          stage_free();
+          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stg);
+          const bool lo = lane < 16;
 #pragma unroll
-            for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = __float2bfloat16_rn(v[j]);
-            stage_store(&map_out, f0, mid, p.tok0 + c0);
-          } else {
-#pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-              float* sb = reinterpret_cast<float*>(stage_buf());
-#pragma unroll
-              for (int j = 0; j < 8; ++j) sb[j * 32 + lane] = v[hh * 8 + j];
-              stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 8);
-            }
-          }
-        } else if (quad >= 2) {  // EPI_SWIGLU, up half: hand the values to the gate warp of the same features
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh, ++n_sub) {
-            float* xb = reinterpret_cast<float*>(stg + (n_sub & 1) * 1024);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) xb[j * 32 + lane] = v[hh * 8 + j];
-            asm volatile("bar.sync %0, 64;\n" ::"r"(2 + (quad & 1) + 2 * par) : "memory");
-          }
-        } else {                 // EPI_SWIGLU, gate half
-          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stage_buf());
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh, ++n_sub) {
-            asm volatile("bar.sync %0, 64;\n" ::"r"(2 + (quad & 1) + 2 * par) : "memory");
-            const float* xb = reinterpret_cast<const float*>(stg + 2 * 2048 + (n_sub & 1) * 1024);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const float g = v[hh * 8 + j];
-              sb[(hh * 8 + j) * 32 + lane] = __float2bfloat16_rn(g / (1.f + __expf(-g)) * xb[j * 32 + lane]);
-            }
+          for (int j = 0; j < 16; ++j) {
+            const float other = __shfl_xor_sync(0xffffffffu, lo ? v[j + 16] : v[j], 16);
+            const float g = lo ? v[j] : other, up = lo ? other : v[j + 16];
+            sb[(lo ? j : j + 16) * 16 + (lane & 15)] = __float2bfloat16_rn(__fdividef(g, 1.f + __expf(-g)) * up);
           }
           stage_store(&map_out, f0, mid, p.tok0 + c0);
         }
       };
       for (int b0 = 0; b0 < n_pad && b0 < p.T; b0 += blk_cols) {
         const int b1 = min(b0 + blk_cols, n_pad);
-        float v[16];
+        float v[32];
         if (n_groups <= 1) {
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
             if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
           }
-          for (int c0 = b0 + 16 * par; c0 < b1 && c0 < p.T; c0 += 32) {
-            load_acc(c0, v);
+          for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += 64) {
+            const int cw = min(32, b1 - c0);
+            load_acc(c0, cw, v);
             if (n_groups == 1) add_fix(n_contrib, b0, b1, c0, v);
-            finish_chunk(c0, v);
+            finish_chunk(c0, cw, v);
           }
-        } else {  // 32-column block: at most one chunk per warp; every warp takes part in every group load
-          const int c0 = b0 + 16 * par;
+        } else {  // 64-column block: at most one chunk per warp; every warp takes part in every group load
+          const int c0 = b0 + 32 * par;
           const bool has = c0 < b1 && c0 < p.T;
-          if (has) load_acc(c0, v);
+          const int cw = min(32, b1 - c0);
+          if (has) load_acc(c0, cw, v);
           for (int g0 = 0; g0 < n_contrib; g0 += grp) {
             const int cnt = min(grp, n_contrib - g0);
             load_group(g0, cnt, b0, b1);
             if (has) add_fix(cnt, b0, b1, c0, v);
           }
-          if (has) finish_chunk(c0, v);
+          if (has) finish_chunk(c0, cw, v);
         }
       }
       tc_fence_before();
@@ -339,6 +348,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
       }
       if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
+      if (etid == 0 && trace) { for (int i = 0; i < 6; ++i) trace[18 + i] = tk[i]; }
       ++piece;
       acc_phase ^= 1;
       u += kb1 - kb0;
@@ -346,6 +356,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     if (lane == 0) bulk_wait<0>();  // all output stores are complete before the CTA exits
   }
 #undef AF_TRACE
+#undef stg
 
   tc_fence_before();
   __syncthreads();
