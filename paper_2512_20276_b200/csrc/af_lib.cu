@@ -207,6 +207,9 @@ extern "C" int af_debug_trace_read(long long* out, int* meta) {
   return g_trace_n;
 }
 
+// threads of the one-block-per-row kernels: one 16-byte access per thread where the row allows it
+static int row_threads_for(int D) { int t = (D / 4 + 31) / 32 * 32; return t < 64 ? 64 : (t > 1024 ? 1024 : t); }
+
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
 // One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
@@ -515,6 +518,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
               dim3(static_cast<unsigned>((n / 4 + 255) / 256)), dim3(256), 0, st,
               reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
   }
+  const int row_threads = row_threads_for(D);
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   const long long split_stride = static_cast<long long>(ws.max_rows) * D;
@@ -530,7 +534,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     const af_layer_weights& L = w->layers[l];
     __nv_bfloat16* kvl = g->kv + layer_elems * l;
     // a8(prev) + a1: x += down partials; xn = RMSNorm(x; g_attn)
-    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
               static_cast<const float*>(ws.split), prev_splits, split_stride,
               reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, D, c.rms_eps);
     // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
@@ -543,7 +547,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
       if ((rc = launch_gemm(PC_GEMM_QKV, st, gp, ov, ws.xn, ws.max_rows, wqkv, T))) return rc;
     }
     // a3: FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q, k at the row's position; k, v go straight to the ring slot
-    AF_LAUNCH(PC_ROPE_APPEND, "rope_append_kernel", rope_append_kernel, dim3(T), dim3(256), 0, st,
+    AF_LAUNCH(PC_ROPE_APPEND, "rope_append_kernel", rope_append_kernel, dim3(T), dim3(row_threads), 0, st,
               static_cast<const __nv_bfloat16*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
               H, hd, R, C);
     // a4: segment-masked causal attention over the ring
@@ -565,7 +569,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
       prev_splits = split_count(d_tiles, D);
     }
     // a5 residual + a6: x += O partials; xn = RMSNorm(x; g_mlp)
-    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+    AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
               static_cast<const float*>(ws.split), prev_splits, split_stride,
               reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, D, c.rms_eps);
     // a7: gate/up projection with the fused SiLU*mul epilogue
@@ -588,7 +592,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     }
   }
   // a8 of the last layer: x += down partials (no norm: hidden_out is the pre-final-norm residual stream)
-  AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(256), 0, st, hidden_out,
+  AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
             static_cast<const float*>(ws.split), prev_splits, split_stride, static_cast<const __nv_bfloat16*>(nullptr),
             static_cast<__nv_bfloat16*>(nullptr), D, c.rms_eps);
 #undef AF_LAUNCH
@@ -616,7 +620,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   for (int i = 0; i < n_rows; ++i) rl.rows[i] = rows[i];
   {
     ProfScope ps_(PC_RMSNORM, st);
-    cudaError_t le = launch_k(gather_norm_kernel, dim3(n_rows), dim3(256), 0, st, rl, hidden,
+    cudaError_t le = launch_k(gather_norm_kernel, dim3(n_rows), dim3(row_threads_for(c.d_model)), 0, st, rl, hidden,
                               reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, c.d_model, c.rms_eps);
     if (le != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gather_norm_kernel failed: %s", cudaGetErrorString(le));
   }

@@ -1,0 +1,152 @@
+"""GPU parity at the full Llama-2-7B shapes of BASELINE.json configs[2..4], in the launch configuration bench.py times
+(T = 282 packed rows, ring 8 x 512, PDL launches), against the unpacked fp32 CPU oracle.  Oracle cost bounds what
+is compared: cfg3 compares pipeline steps 0..8 (fill, first steady steps, first region recycle) on every row; cfg5
+compares every grid point against two oracle forwards (packing independence makes each point a row selection);
+cfg4 runs the full wrap schedule on an 8-layer slice against the oracle and on all 32 layers GPU-vs-GPU (bitwise
+base invariance).  Run with `pytest -m gpu` on a B200."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import af_oracle as O
+from paper_2512_20276_b200 import inputs as I
+from af_harness import Pair, relmax, TOL
+
+pytestmark = pytest.mark.gpu
+
+L_P, K, R, C = 276, 7, 8, 512
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2512_20276_b200 import binding as b
+    b.load_library()
+    return b
+
+
+@pytest.fixture(scope="module")
+def w7b(binding):
+    cfg = I.CFG_7B
+    hw = I.make_weights(cfg, seed=2, threads=16)
+    return cfg, hw, binding.Weights(cfg, hw)
+
+
+def test_cfg3_pipeline_fill_steady_and_recycle(binding, w7b):
+    """BASELINE.json configs[2]: schedule P9 (req = step mod 8, reset_slot before each prefill), steps 0..8: pipeline
+    fill, steady steps with 6 decodes at contexts 277..282, and the first recycled region at step 8; logits on the
+    prediction rows (row 275 + the decode rows) from the first steady step on."""
+    cfg, hw, W = w7b
+    P = Pair(cfg, hw, R=R, C=C, max_rows=288, oracle_dtype=torch.float32, dev_weights=W)
+    worst_h, worst_l = 0.0, 0.0
+    for t in range(9):
+        P.reset(t % R, -1)
+        segs = I.steady_schedule(t, L_P, K, R)
+        e = I.make_embeds(cfg, 2, t, I.total_rows(segs))
+        hid, ref = P.step(segs, e)
+        worst_h = max(worst_h, relmax(hid, ref))
+        if t >= K - 1:
+            lg, ref_lg = P.check_logits(hid, ref, I.prediction_rows(segs))
+            worst_l = max(worst_l, relmax(lg, ref_lg))
+            assert torch.equal(lg.argmax(dim=1).cpu(), ref_lg.argmax(dim=1)) or worst_l <= TOL
+    assert P.len[8 % R] == L_P and P.base[8 % R] == (L_P + K - 1) % C      # region 0 was recycled and rotated
+    P.check_ring(list(range(R)), layers=[0, 15, 31])
+    print(f"cfg3: worst hidden {worst_h:.3e}, worst logits {worst_l:.3e}")
+
+
+def test_cfg3_steady_step_is_deterministic(binding, w7b):
+    """Two runs of the same 8 steps give bit-identical hidden states and logits (order-fixed reductions)."""
+    cfg, hw, W = w7b
+    outs = []
+    for _ in range(2):
+        ring = binding.Ring(cfg, R, C, max_rows=288)
+        for t in range(8):
+            ring.reset_slot(t % R, -1)
+            segs = I.steady_schedule(t, L_P, K, R)
+            hid = ring.packed_forward(W, I.make_embeds(cfg, 2, t, I.total_rows(segs)).cuda(), segs)
+        lg = ring.logits_rows(W, hid, I.prediction_rows(segs))
+        outs.append((hid.clone(), lg.clone()))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+
+
+def test_cfg5_scheduling_shape_sweep(binding, w7b):
+    """BASELINE.json configs[4]: n_dec in 0..15 x prefill in {0,128,276,512}; decode j's history is the first 276+j
+    rows of one stream H, the prefill is the first P rows of one stream E.  The oracle runs E (512 rows) and H
+    (291 rows) once; every grid point's rows are selections of those two results."""
+    cfg, hw, W = w7b
+    Rr, Cc = 17, 1024
+    E = I.make_embeds(cfg, 4, 0, 512)
+    H = I.make_embeds(cfg, 4, 1, 291)
+    orc = O.Oracle(cfg, hw, torch.float32)
+    ref_E = orc.step([(0, 0, 0, 512)], E)
+    ref_H = orc.step([(1, 0, 0, 291)], H)
+    ring = binding.Ring(cfg, Rr, Cc, max_rows=544)
+    for j in range(15):                      # histories: region j+1 holds the first 276+j rows of H
+        ring.packed_forward(W, H[:276 + j].cuda().contiguous(), [(j + 1, 0, 0, 276 + j)])
+    assert ring.packed_forward(W, E[:0].cuda(), []).shape[0] == 0          # the (0, 0) grid point is a legal no-op
+    worst = 0.0
+    points = [(n, p) for n in (0, 1, 6, 15) for p in (0, 128, 276, 512)] + [(n, 276) for n in range(2, 15)]
+    for n_dec, p_len in points:
+        if n_dec == 0 and p_len == 0:
+            continue
+        ring.reset_slot(0, 0)
+        for j in range(15):
+            ring.set_len(j + 1, 276 + j)
+        segs, rows, refs = [], [], []
+        if p_len:
+            segs.append((0, 0, 0, p_len)); rows.append(E[:p_len]); refs.append(ref_E[:p_len])
+        for j in range(n_dec):
+            segs.append((j + 1, 1, 276 + j, 1)); rows.append(H[276 + j:277 + j]); refs.append(ref_H[276 + j:277 + j])
+        hid = ring.packed_forward(W, torch.cat(rows).cuda().contiguous(), segs)
+        err = relmax(hid, torch.cat(refs))
+        worst = max(worst, err)
+        assert err <= TOL, f"n_dec={n_dec} prefill={p_len}: {err:.3e}"
+    print(f"cfg5: worst hidden {worst:.3e} over {len(points) - 1} grid points")
+
+
+def _cfg4_schedule(rng, Cc, n_req):
+    """Deterministic scheduler of BASELINE.json configs[3]: chunked prefills (U{128..512}, <= 4 chunks per step) until
+    len = 1015, then one decode token per step up to len = 1023."""
+    lens = [0] * n_req
+    steps = []
+    while any(n < Cc - 1 for n in lens):
+        segs, chunks = [], 0
+        for r in range(n_req):
+            n = lens[r]
+            if n >= Cc - 1:
+                continue
+            if n < 1015:
+                if chunks == 4:
+                    continue
+                ln = int(min(rng.integers(128, 513), 1015 - n))
+                segs.append((r, 0, n, ln)); chunks += 1
+            else:
+                ln = 1
+                segs.append((r, 1, n, 1))
+            lens[r] = n + ln
+        steps.append(segs)
+    return steps
+
+
+def test_cfg4_wraparound_long_context(binding):
+    """BASELINE.json configs[3] on an 8-layer slice against the oracle (every request's appends cross its wrap, prefill
+    chunks of 128..512 rows, decodes up to context 1023, ring read back in logical order), then the same schedule with
+    all bases 0: outputs must be bit-identical (KV tiles are walked in logical order)."""
+    cfg = I.cfg_7b_layers(8, vocab=512)
+    hw = I.make_weights(cfg, seed=3, threads=16)
+    W = binding.Weights(cfg, hw)
+    Rr, Cc = 8, 1024
+    rng = np.random.default_rng(3)
+    bases = [int(Cc - rng.integers(1, 601)) for _ in range(Rr)]
+    steps = _cfg4_schedule(np.random.default_rng(33), Cc, Rr)
+    P = Pair(cfg, hw, R=Rr, C=Cc, max_rows=2048, bases=bases, oracle_dtype=torch.float32, dev_weights=W)
+    ring0 = binding.Ring(cfg, Rr, Cc, max_rows=2048)
+    worst = 0.0
+    for t, segs in enumerate(steps):
+        e = I.make_embeds(cfg, 3, t, I.total_rows(segs))
+        hid, ref = P.step(segs, e)
+        worst = max(worst, relmax(hid, ref))
+        hid0 = ring0.packed_forward(W, e.cuda(), segs)
+        assert torch.equal(hid, hid0), f"step {t}: result depends on the ring rotation"
+    assert P.len == [Cc - 1] * Rr
+    P.check_ring(list(range(Rr)))
+    print(f"cfg4: {len(steps)} steps, worst hidden {worst:.3e}")
