@@ -18,7 +18,9 @@
  * Conventions
  *   - All "device" pointers are CUDA device memory of the current device, owned by the caller.
  *     All "host" pointers are ordinary host memory, read (or written) before the call returns.
- *   - bf16 = IEEE bfloat16 stored as uint16.  Weights are [out_features, in_features] row-major (y = x W^T).
+ *   - bf16 = bfloat16, fp16 = IEEE binary16, both stored as uint16.  Weights, gains and the packed embeddings are bf16;
+ *     weights are [out_features, in_features] row-major (y = x W^T).  The KV ring holds fp16 (same bytes as bf16, 3 more
+ *     mantissa bits: DESIGN.md "Precision"); all accumulation and the residual stream are fp32.
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t cast to void*) and return without host synchronisation
  *     (the af_debug_* and af_ring_read_* calls synchronise; they are test/bench helpers, not the hot path).
  *   - Return value: 0 on success, a negative AF_ERR_* otherwise.  On any error raised by argument validation
@@ -31,7 +33,7 @@
  *   logically partitioned per request").  The token at logical position pos of request r lives in
  *       slot      = (base_r + pos) mod C                       (slot inside region r)
  *       row_slot  = r * C + slot                               (the global slot id reported by af_debug_row_map)
- *   and its K (after RoPE) and V vectors of head h are the head_dim contiguous bf16 values at element offset
+ *   and its K (after RoPE) and V vectors of head h are the head_dim contiguous fp16 values at element offset
  *       (((layer * 2 + kv) * R + r) * n_heads + h) * C * head_dim + slot * head_dim,     kv = 0 for K, 1 for V.
  *   A request's live range is positions 0..len_r-1; slots outside it are never read.
  */
@@ -78,12 +80,21 @@ typedef struct {                 /* all device bf16 */
   const void *g_attn, *g_mlp;    /* RMSNorm gains [d_model] */
 } af_layer_weights;
 
+#define AF_WEIGHTS_BF16 0         /* projection matrices are bf16; every weight tile is converted to fp16 in shared memory */
+#define AF_WEIGHTS_FP16 1         /* projection matrices were prepared once with af_convert_bf16_to_fp16 (same values) */
+
 typedef struct {
   af_model_cfg cfg;
   const af_layer_weights* layers; /* HOST array [n_layers] of device pointers */
   const void* g_final;            /* device bf16 [d_model] */
-  const void* w_lm;               /* device bf16 [vocab, d_model] */
+  const void* w_lm;               /* device bf16 (or prepared fp16) [vocab, d_model] */
+  int32_t weight_format;          /* AF_WEIGHTS_BF16 or AF_WEIGHTS_FP16: format of wq..w_down and w_lm (gains stay bf16) */
 } af_weights;
+
+/* Load-time weight preparation: dst[i] = fp16(src[i]) for n_elems bf16 values (n_elems % 8 == 0,
+ * both device, 16-byte aligned, may not overlap).  Exact for every finite bf16 value with 2^-14 <= |w| <= 65504; smaller
+ * values round to fp16 subnormals (absolute error <= 2^-25).  Enqueued on cuda_stream. */
+int af_convert_bf16_to_fp16(const void* src_bf16, void* dst_fp16, size_t n_elems, void* cuda_stream);
 
 /* Bytes of kv_mem needed for (cfg, ring): 2 * n_layers * R * n_heads * C * head_dim * 2. */
 size_t af_ring_bytes(const af_model_cfg* cfg, const af_ring_cfg* ring);
@@ -127,7 +138,7 @@ int af_debug_set_len(af_ring* ring, int32_t req_id, int32_t len);
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t af_debug_launch_count(void);
 /* Plain C = A B^T through the same tcgen05 GEMM kernel the forward uses (unit tests / roofline probes).
- * a: device bf16 [n_tok, k] (activations), w: device bf16 [n_out, k]; out: device fp32 [n_tok, n_out]. */
+ * a: device fp16 [n_tok, k] (activations), w: device bf16 [n_out, k]; out: device fp32 [n_tok, n_out], n_out % 4 == 0. */
 int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32_t n_out, int32_t k,
                   void* workspace, size_t ws_bytes, void* cuda_stream);
 

@@ -45,10 +45,10 @@ class af_layer_weights(C.Structure):
 
 class af_weights(C.Structure):
     _fields_ = [("cfg", af_model_cfg), ("layers", C.POINTER(af_layer_weights)), ("g_final", C.c_void_p),
-                ("w_lm", C.c_void_p)]
+                ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
 
 
-EXPORTS = ["af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+EXPORTS = ["af_convert_bf16_to_fp16", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_profile", "af_debug_profile_read", "af_last_error"]
 
@@ -72,6 +72,8 @@ def load_library():
     L.af_ring_bytes.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg)]
     L.af_workspace_bytes.restype = sz
     L.af_workspace_bytes.argtypes = [C.POINTER(af_model_cfg), i32, i32]
+    L.af_convert_bf16_to_fp16.argtypes = [vp, vp, sz, vp]
+    L.af_convert_bf16_to_fp16.restype = C.c_int
     L.af_ring_create.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg), vp, sz, C.POINTER(vp)]
     L.af_ring_reset_slot.argtypes = [vp, i32, i32]
     L.af_packed_forward.argtypes = [C.POINTER(af_weights), vp, C.POINTER(af_segment), i32, vp, vp, vp, sz, vp]
@@ -112,20 +114,32 @@ def _stream_ptr(stream=None):
 
 
 class Weights:
-    """Device copies of the bf16 weights + the af_weights struct pointing at them."""
+    """Device copies of the bf16 weights + the af_weights struct pointing at them.  With prepared=True (default) the
+    projection matrices are rewritten once, on the device, as fp16 by af_convert_bf16_to_fp16 (AF_WEIGHTS_FP16: the
+    same values, no per-tile conversion in the GEMM); prepared=False keeps them bf16 (AF_WEIGHTS_BF16)."""
 
-    def __init__(self, cfg, host_weights: dict, device="cuda"):
+    def __init__(self, cfg, host_weights: dict, device="cuda", prepared=True):
         self.cfg = cfg
+        self.prepared = prepared
         self.tensors = []          # keep alive
         self._layers = (af_layer_weights * cfg.n_layers)()
         for l, L in enumerate(host_weights["layers"]):
             for name, _ in af_layer_weights._fields_:
-                t = L[name].to(torch.bfloat16).contiguous().to(device)
+                t = self._prep(L[name].to(torch.bfloat16).contiguous().to(device), name.startswith("w"))
                 self.tensors.append(t)
                 setattr(self._layers[l], name, t.data_ptr())
         self.g_final = host_weights["g_final"].to(torch.bfloat16).contiguous().to(device)
-        self.w_lm = host_weights["w_lm"].to(torch.bfloat16).contiguous().to(device)
-        self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr())
+        self.w_lm = self._prep(host_weights["w_lm"].to(torch.bfloat16).contiguous().to(device), True)
+        torch.cuda.synchronize()
+        self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr(),
+                                 1 if prepared else 0)
+
+    def _prep(self, t: torch.Tensor, is_matrix: bool) -> torch.Tensor:
+        if not (self.prepared and is_matrix):
+            return t
+        out = torch.empty(t.shape, dtype=torch.float16, device=t.device)
+        _check(load_library().af_convert_bf16_to_fp16(t.data_ptr(), out.data_ptr(), t.numel(), _stream_ptr()))
+        return out
 
 
 class Ring:
@@ -146,9 +160,9 @@ class Ring:
         self.handle = h
 
     def kv_view(self) -> torch.Tensor:
-        """The ring as bf16 [n_layers, 2, R, H, C, hd] (layout documented in include/af.h)."""
+        """The ring as fp16 [n_layers, 2, R, H, C, hd] (layout documented in include/af.h)."""
         c = self.cfg
-        return self.kv_mem.view(torch.bfloat16).view(c.n_layers, 2, self.R, c.n_heads, self.Cap, c.head_dim)
+        return self.kv_mem.view(torch.float16).view(c.n_layers, 2, self.R, c.n_heads, self.Cap, c.head_dim)
 
     def reset_slot(self, req_id: int, new_base: int = -1):
         _check(load_library().af_ring_reset_slot(self.handle, req_id, new_base))
@@ -199,8 +213,9 @@ class Ring:
 
 
 def debug_gemm(a: torch.Tensor, w: torch.Tensor) -> torch.Tensor:
-    """out[n_tok, n_out] fp32 = a[n_tok, k] @ w[n_out, k]^T through the tcgen05 GEMM kernel."""
+    """out[n_tok, n_out] fp32 = a[n_tok, k] (fp16 activations) @ w[n_out, k]^T (bf16 weights), tcgen05 GEMM kernel."""
     L = load_library()
+    assert a.dtype == torch.float16 and w.dtype == torch.bfloat16
     n_tok, k = a.shape
     n_out = w.shape[0]
     out = torch.empty(n_tok, n_out, dtype=torch.float32, device=a.device)

@@ -88,7 +88,7 @@ struct MapKey {
 static std::map<MapKey, CUtensorMap> g_maps;
 
 // Cached cuTensorMapEncodeTiled.  dims / box innermost first; strides (bytes) of dims 1..rank-1.
-static int get_map_nd(const void* ptr, int elem_bytes, int rank, const unsigned long long* dims,
+static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 2 = bf16, -2 = fp16, 4 = fp32 */ const unsigned long long* dims,
                       const unsigned long long* strides, const unsigned* box, bool swizzle128, CUtensorMap* out) {
   std::lock_guard<std::mutex> lk(g_mu);
   MapKey key;
@@ -113,7 +113,8 @@ static int get_map_nd(const void* ptr, int elem_bytes, int rank, const unsigned 
   cuuint32_t bx[3], estr[3] = {1, 1, 1};
   for (int i = 0; i < rank; ++i) { d[i] = dims[i]; bx[i] = box[i]; }
   for (int i = 0; i + 1 < rank; ++i) st[i] = strides[i];
-  const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                 : (elem_bytes == -2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32);
   CUresult r = g_encode(&m, dt, rank, const_cast<void*>(ptr), d, st, bx, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                         swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -125,23 +126,25 @@ static int get_map_nd(const void* ptr, int elem_bytes, int rank, const unsigned 
 }
 
 // bf16 row-major [rows, cols] operand matrix, box = [box_rows, 64 cols], 128-byte swizzle, zero fill out of bounds.
-static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out, bool fp16 = false) {
   if (cols % 8) return fail(AF_ERR_ARG, "matrix %p [%d,%d] needs a 16-byte row pitch", ptr, rows, cols);
   const unsigned long long dims[2] = {static_cast<unsigned long long>(cols), static_cast<unsigned long long>(rows)};
   const unsigned long long strides[1] = {static_cast<unsigned long long>(cols) * 2};
   const unsigned box[2] = {static_cast<unsigned>(GEMM_BK), static_cast<unsigned>(box_rows)};
-  return get_map_nd(ptr, 2, 2, dims, strides, box, true, out);
+  return get_map_nd(ptr, fp16 ? -2 : 2, 2, dims, strides, box, true, out);
 }
 
 // Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
-struct OutView { void* ptr; int elem_bytes; int features, n_mid, tokens; long long ld_mid, ld_tok; int box_feat; };
+struct OutView { void* ptr; int elem_bytes; /* 4 = fp32, 2 = bf16, -2 = fp16 */ int features, n_mid, tokens; long long ld_mid, ld_tok; int box_feat; };
 static int get_out_map(const OutView& o, CUtensorMap* out) {
   const unsigned long long dims[3] = {static_cast<unsigned long long>(o.features), static_cast<unsigned long long>(o.n_mid),
                                       static_cast<unsigned long long>(o.tokens)};
-  const unsigned long long strides[2] = {static_cast<unsigned long long>(o.ld_mid) * o.elem_bytes,
-                                         static_cast<unsigned long long>(o.ld_tok) * o.elem_bytes};
+  const int eb = o.elem_bytes < 0 ? -o.elem_bytes : o.elem_bytes;
+  const unsigned long long strides[2] = {static_cast<unsigned long long>(o.ld_mid) * eb,
+                                         static_cast<unsigned long long>(o.ld_tok) * eb};
+  const int et = o.elem_bytes;
   const unsigned box[3] = {static_cast<unsigned>(o.box_feat), 1u, 32u};
-  return get_map_nd(o.ptr, o.elem_bytes, 3, dims, strides, box, false, out);
+  return get_map_nd(o.ptr, et, 3, dims, strides, box, false, out);
 }
 
 // ------------------------------------------------------------------------------------------------ launches
@@ -214,7 +217,7 @@ static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) *
 
 // One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
 // layout (n_parts / part_rows / a_pair), the split mode and the epilogue fields; the decomposition is filled here.
-static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView& ov, const void* x, int x_rows_cap,
+static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView& ov, /* proto.w_fp16 set by the caller */ const void* x, int x_rows_cap,
                        const void* const* w, int T) {
   int rc = gemm_global_init();
   if (rc) return rc;
@@ -262,7 +265,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     rc = get_map(x, x_rows_cap, p.K, p.n1, &mx);
     if (rc) return rc;
     CUtensorMap mo, mp;
-    p.out_bf16 = ov.elem_bytes == 2;
+    p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
     if ((rc = get_out_map(ov, &mo))) return rc;
     {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
@@ -286,7 +289,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
 struct af_ring {
   af_model_cfg cfg;
   af_ring_cfg rc;
-  __nv_bfloat16* kv;            // caller-owned
+  act_t* kv;                    // caller-owned, fp16
   std::vector<int> base, len;   // host mirror, authoritative for validation (a0, a9)
   int* tables = nullptr;        // library-owned device ints backing StepTables
   StepTables tb{};
@@ -331,7 +334,7 @@ extern "C" size_t af_workspace_bytes(const af_model_cfg* c, int32_t max_rows, in
 struct Workspace {
   float* partial;        // stream-K partials [grid][n_pad][128]
   float* split;          // split-K slabs [GEMM_MAX_SPLITS][max_rows][D]
-  __nv_bfloat16 *xn, *qkv, *q_rot, *attn, *h;
+  act_t *xn, *qkv, *q_rot, *attn, *h;   // fp16 activations
   int max_rows;
 };
 static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, Workspace* o) {
@@ -347,11 +350,11 @@ static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, W
   auto take = [&](size_t n) { uint8_t* q = p; p += align_up(n, 256); return q; };
   o->partial = reinterpret_cast<float*>(take(gemm_partial_bytes()));
   o->split = reinterpret_cast<float*>(take(GEMM_MAX_SPLITS * rows * D * 4));
-  o->xn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
-  o->qkv = reinterpret_cast<__nv_bfloat16*>(take(rows * 3 * D * 2));
-  o->q_rot = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
-  o->attn = reinterpret_cast<__nv_bfloat16*>(take(rows * D * 2));
-  o->h = reinterpret_cast<__nv_bfloat16*>(take(rows * F * 2));
+  o->xn = reinterpret_cast<act_t*>(take(rows * D * 2));
+  o->qkv = reinterpret_cast<act_t*>(take(rows * 3 * D * 2));
+  o->q_rot = reinterpret_cast<act_t*>(take(rows * D * 2));
+  o->attn = reinterpret_cast<act_t*>(take(rows * D * 2));
+  o->h = reinterpret_cast<act_t*>(take(rows * F * 2));
   o->max_rows = static_cast<int>(rows);
   return AF_OK;
 }
@@ -366,7 +369,7 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   rc = gemm_global_init();
   if (rc) return rc;
   af_ring* g = new af_ring();
-  g->cfg = *c; g->rc = *r; g->kv = reinterpret_cast<__nv_bfloat16*>(kv_mem);
+  g->cfg = *c; g->rc = *r; g->kv = reinterpret_cast<act_t*>(kv_mem);
   g->base.assign(r->n_regions, 0); g->len.assign(r->n_regions, 0);
   const long long cap_rows = static_cast<long long>(r->n_regions) * r->capacity;
   g->max_rows = static_cast<int>(cap_rows > 65536 ? 65536 : cap_rows);
@@ -433,6 +436,16 @@ extern "C" int af_debug_row_map(const af_ring* g, int32_t* row_req, int32_t* row
   return AF_OK;
 }
 
+extern "C" int af_convert_bf16_to_fp16(const void* src, void* dst, size_t n, void* cuda_stream) {
+  if (!src || !dst || (n % 8)) return fail(AF_ERR_ARG, "null pointer or n_elems not a multiple of 8");
+  if ((reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst)) & 15) return fail(AF_ERR_ARG, "pointers must be 16-byte aligned");
+  if (n == 0) return AF_OK;
+  const size_t n_vec = n / 8;
+  convert_bf16_to_fp16_kernel<<<static_cast<unsigned>((n_vec + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(
+      reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst), n_vec);
+  return check_launch("convert_bf16_to_fp16_kernel");
+}
+
 extern "C" int64_t af_debug_launch_count(void) { return g_launches.load(); }
 extern "C" const char* af_last_error(void) { return g_err.c_str(); }
 
@@ -447,6 +460,8 @@ static int check_weights(const af_weights* w, bool need_lm) {
       return fail(AF_ERR_ARG, "null weight pointer in layer %d", l);
   }
   if (need_lm && (!w->g_final || !w->w_lm)) return fail(AF_ERR_ARG, "null g_final / w_lm");
+  if (w->weight_format != AF_WEIGHTS_BF16 && w->weight_format != AF_WEIGHTS_FP16)
+    return fail(AF_ERR_ARG, "weight_format %d is neither AF_WEIGHTS_BF16 nor AF_WEIGHTS_FP16", w->weight_format);
   return AF_OK;
 }
 
@@ -519,6 +534,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
               reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
   }
   const int row_threads = row_threads_for(D);
+  const int wfmt = w->weight_format == AF_WEIGHTS_FP16;
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   const long long split_stride = static_cast<long long>(ws.max_rows) * D;
@@ -532,7 +548,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   const int d_tiles = (D + GEMM_BM - 1) / GEMM_BM;
   for (int l = 0; l < c.n_layers; ++l) {
     const af_layer_weights& L = w->layers[l];
-    __nv_bfloat16* kvl = g->kv + layer_elems * l;
+    act_t* kvl = g->kv + layer_elems * l;
     // a8(prev) + a1: x += down partials; xn = RMSNorm(x; g_attn)
     AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
               static_cast<const float*>(ws.split), prev_splits, split_stride,
@@ -540,29 +556,29 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
     {
       GemmParams gp{};
-      gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
+      gp.w_fp16 = wfmt; gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
       gp.partial = ws.partial;
-      const OutView ov{ws.qkv, 2, D, 3, T, D, 3LL * D, 32};
+      const OutView ov{ws.qkv, -2, D, 3, T, D, 3LL * D, 32};
       const void* wqkv[3] = {L.wq, L.wk, L.wv};
       if ((rc = launch_gemm(PC_GEMM_QKV, st, gp, ov, ws.xn, ws.max_rows, wqkv, T))) return rc;
     }
     // a3: FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q, k at the row's position; k, v go straight to the ring slot
     AF_LAUNCH(PC_ROPE_APPEND, "rope_append_kernel", rope_append_kernel, dim3(T), dim3(row_threads), 0, st,
-              static_cast<const __nv_bfloat16*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
+              static_cast<const act_t*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
               H, hd, R, C);
     // a4: segment-masked causal attention over the ring
     if (hd == 128)
       AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(n_items, H), dim3(ATT_THREADS),
-                5 * ATT_BQ * 128 * 2, st, static_cast<const __nv_bfloat16*>(ws.q_rot),
-                static_cast<const __nv_bfloat16*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
+                5 * ATT_BQ * 128 * 2, st, static_cast<const act_t*>(ws.q_rot),
+                static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     else
       AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(n_items, H), dim3(ATT_THREADS),
-                5 * ATT_BQ * 64 * 2, st, static_cast<const __nv_bfloat16*>(ws.q_rot),
-                static_cast<const __nv_bfloat16*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
+                5 * ATT_BQ * 64 * 2, st, static_cast<const act_t*>(ws.q_rot),
+                static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     // a5: O projection, split-K slabs (added to the residual by the next kernel)
     {
       GemmParams gp{};
-      gp.n_parts = 1; gp.part_rows = D; gp.K = D; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
+      gp.w_fp16 = wfmt; gp.n_parts = 1; gp.part_rows = D; gp.K = D; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
       const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wo[3] = {L.wo, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_O, st, gp, ov, ws.attn, ws.max_rows, wo, T))) return rc;
@@ -575,16 +591,16 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a7: gate/up projection with the fused SiLU*mul epilogue
     {
       GemmParams gp{};
-      gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
+      gp.w_fp16 = wfmt; gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
       gp.partial = ws.partial;
-      const OutView ov{ws.h, 2, F, 1, T, F, F, 16};
+      const OutView ov{ws.h, -2, F, 1, T, F, F, 16};
       const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
       if ((rc = launch_gemm(PC_GEMM_GATEUP, st, gp, ov, ws.xn, ws.max_rows, wgu, T))) return rc;
     }
     // a8: down projection, split-K slabs
     {
       GemmParams gp{};
-      gp.n_parts = 1; gp.part_rows = D; gp.K = F; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
+      gp.w_fp16 = wfmt; gp.n_parts = 1; gp.part_rows = D; gp.K = F; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
       const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wd[3] = {L.w_down, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_DOWN, st, gp, ov, ws.h, ws.max_rows, wd, T))) return rc;
@@ -594,7 +610,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   // a8 of the last layer: x += down partials (no norm: hidden_out is the pre-final-norm residual stream)
   AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
             static_cast<const float*>(ws.split), prev_splits, split_stride, static_cast<const __nv_bfloat16*>(nullptr),
-            static_cast<__nv_bfloat16*>(nullptr), D, c.rms_eps);
+            static_cast<act_t*>(nullptr), D, c.rms_eps);
 #undef AF_LAUNCH
   // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----
   for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;
@@ -626,6 +642,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   }
   if ((rc = check_launch("gather_norm_kernel"))) return rc;
   GemmParams gp{};
+  gp.w_fp16 = w->weight_format == AF_WEIGHTS_FP16;
   gp.n_parts = 1; gp.part_rows = c.vocab; gp.K = c.d_model; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
   gp.partial = ws.partial;
   if (c.vocab % 4) return fail(AF_ERR_UNSUPPORTED, "vocab must be a multiple of 4 (16-byte logits rows)");

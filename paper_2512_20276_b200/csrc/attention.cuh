@@ -2,7 +2,7 @@
 // P:194-200).  Each work item is (segment, 64-row query tile) x head.  The tile's rows attend to positions
 // 0..own position of THEIR OWN request only; K/V rows are gathered from the ring at slot (base_r + j) mod C
 // (wrap included) with 128-bit cp.async loads into XOR-swizzled shared memory, S = QK^T and O = PV run on
-// mma.sync.m16n8k16 (bf16 in, fp32 accumulate), and the online softmax reduces across the 4 lanes that share a row
+// mma.sync.m16n8k16 (fp16 in, fp32 accumulate), and the online softmax reduces across the 4 lanes that share a row
 // with warp shuffles.  KV tiles are walked in LOGICAL position order, so results do not depend on base_r.
 #pragma once
 #include "ptx.cuh"
@@ -42,9 +42,9 @@ __device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint3
   asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
                : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
 }
-__device__ __forceinline__ void mma_bf16_16816(float* c, const uint32_t* a, uint32_t b0, uint32_t b1) {
+__device__ __forceinline__ void mma_f16_16816(float* c, const uint32_t* a, uint32_t b0, uint32_t b1) {
   asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
       : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
@@ -53,7 +53,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&h);
 }
 
-// byte offset of 16-byte chunk `chunk` of row `row` in a [rows][HD] bf16 tile with XOR swizzle
+// byte offset of 16-byte chunk `chunk` of row `row` in a [rows][HD] 16-bit tile with XOR swizzle
 template <int HD>
 __device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
   return static_cast<uint32_t>(row * (HD * 2) + ((chunk ^ (row & 7)) << 4));
@@ -61,9 +61,9 @@ __device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
 
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS)
-attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated queries
-                 const __nv_bfloat16* __restrict__ kv,    // ring, layer base: [2][R][H][C][HD]
-                 __nv_bfloat16* __restrict__ out,         // [T, H*HD]
+attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
+                 const act_t* __restrict__ kv,    // ring, layer base: [2][R][H][C][HD]
+                 act_t* __restrict__ out,         // [T, H*HD]
                  StepTables tb, int H, int R, int C, float scale_log2) {
   constexpr int CH = HD / 8;                  // 16-byte chunks per row
   constexpr int TILE_BYTES = ATT_BKV * HD * 2;
@@ -85,14 +85,14 @@ attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated q
   const int g = lane >> 2, t = lane & 3;
 
   const size_t head_stride = static_cast<size_t>(C) * HD;
-  const __nv_bfloat16* kbase = kv + (static_cast<size_t>(0 * R + req) * H + h) * head_stride;
-  const __nv_bfloat16* vbase = kv + (static_cast<size_t>(1 * R + req) * H + h) * head_stride;
+  const act_t* kbase = kv + (static_cast<size_t>(0 * R + req) * H + h) * head_stride;
+  const act_t* vbase = kv + (static_cast<size_t>(1 * R + req) * H + h) * head_stride;
 
   // ---- async loads: Q tile, then KV tile 0 ----
   for (int i = tid; i < ATT_BQ * CH; i += ATT_THREADS) {
     const int r = i / CH, c = i % CH;
     const bool ok = r < nq;
-    const __nv_bfloat16* src = q + static_cast<size_t>(row0 + q0 + (ok ? r : 0)) * (H * HD) + h * HD + c * 8;
+    const act_t* src = q + static_cast<size_t>(row0 + q0 + (ok ? r : 0)) * (H * HD) + h * HD + c * 8;
     cp_async16(sQ + sw_off<HD>(r, c), src, ok);
   }
   auto load_kv = [&](int tile, int stage) {
@@ -150,8 +150,8 @@ attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated q
           const int r = nb * 8 + (lane & 7) + (lane >> 4) * 8;
           const int c = kk * 2 + ((lane >> 3) & 1);
           ldsm_x4(smem_u32(cK + sw_off<HD>(r, c)), b0, b1, b2, b3);
-          mma_bf16_16816(s[nb], qf[kk], b0, b1);
-          mma_bf16_16816(s[nb + 1], qf[kk], b2, b3);
+          mma_f16_16816(s[nb], qf[kk], b0, b1);
+          mma_f16_16816(s[nb + 1], qf[kk], b2, b3);
         }
       }
       // ---- causal mask within the request + online softmax (base-2 exponent) ----
@@ -198,18 +198,18 @@ attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated q
 #pragma unroll
       for (int kk = 0; kk < ATT_BKV / 16; ++kk) {
         uint32_t a[4];
-        a[0] = pack_bf16(s[2 * kk][0], s[2 * kk][1]);
-        a[1] = pack_bf16(s[2 * kk][2], s[2 * kk][3]);
-        a[2] = pack_bf16(s[2 * kk + 1][0], s[2 * kk + 1][1]);
-        a[3] = pack_bf16(s[2 * kk + 1][2], s[2 * kk + 1][3]);
+        a[0] = pack_act(s[2 * kk][0], s[2 * kk][1]);
+        a[1] = pack_act(s[2 * kk][2], s[2 * kk][3]);
+        a[2] = pack_act(s[2 * kk + 1][0], s[2 * kk + 1][1]);
+        a[3] = pack_act(s[2 * kk + 1][2], s[2 * kk + 1][3]);
 #pragma unroll
         for (int db = 0; db < HD / 8; db += 2) {
           uint32_t b0, b1, b2, b3;
           const int r = kk * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
           const int c = db + (lane >> 4);
           ldsm_x4_trans(smem_u32(cV + sw_off<HD>(r, c)), b0, b1, b2, b3);
-          mma_bf16_16816(o_acc[db], a, b0, b1);
-          mma_bf16_16816(o_acc[db + 1], a, b2, b3);
+          mma_f16_16816(o_acc[db], a, b0, b1);
+          mma_f16_16816(o_acc[db + 1], a, b2, b3);
         }
       }
     }
@@ -228,11 +228,11 @@ attention_kernel(const __nv_bfloat16* __restrict__ q,     // [T, H*HD] rotated q
       const int qi = warp * 16 + g + r * 8;
       if (qi < nq) {
         const float inv = 1.f / l_run[r];
-        __nv_bfloat16* dst = out + static_cast<size_t>(row0 + q0 + qi) * (H * HD) + h * HD;
+        act_t* dst = out + static_cast<size_t>(row0 + q0 + qi) * (H * HD) + h * HD;
 #pragma unroll
         for (int db = 0; db < HD / 8; ++db) {
           *reinterpret_cast<uint32_t*>(dst + db * 8 + 2 * t) =
-              pack_bf16(o_acc[db][2 * r] * inv, o_acc[db][2 * r + 1] * inv);
+              pack_act(o_acc[db][2 * r] * inv, o_acc[db][2 * r + 1] * inv);
         }
       }
     }

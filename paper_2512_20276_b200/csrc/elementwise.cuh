@@ -77,10 +77,10 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 
 // a5/a8 residual + a1/a6 RMSNorm in one pass (and a10's norm when rows != nullptr), one block per row:
 //   x[i,:] += sum_s parts[s][i,:]      the split-K partials of the preceding O / down projection, in split order
-//   y[i,:]  = bf16( x[src,:] * g / sqrt(mean(x^2) + eps) )          (skipped when g == nullptr: reduce only)
+//   y[i,:]  = fp16( x[src,:] * g / sqrt(mean(x^2) + eps) )          (skipped when g == nullptr: reduce only)
 __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const float* __restrict__ parts, int n_parts,
                                                   long long part_stride, const __nv_bfloat16* __restrict__ g,
-                                                  __nv_bfloat16* __restrict__ y, int i, int src, int D, float eps) {
+                                                  act_t* __restrict__ y, int i, int src, int D, float eps) {
   __shared__ float red[32];
   float* xr = x + static_cast<size_t>(src) * D;
   float ss = 0.f;
@@ -99,22 +99,22 @@ __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const f
   if (!g) return;
   ss = block_sum(ss, red);
   const float inv = rsqrtf(ss / D + eps);
-  __nv_bfloat16* yr = y + static_cast<size_t>(i) * D;
+  act_t* yr = y + static_cast<size_t>(i) * D;
   for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
     const float4 v = *reinterpret_cast<const float4*>(xr + c);   // this thread's own writes (same addresses)
     const uint2 graw = *reinterpret_cast<const uint2*>(g + c);
     const __nv_bfloat162 g0 = *reinterpret_cast<const __nv_bfloat162*>(&graw.x);
     const __nv_bfloat162 g1 = *reinterpret_cast<const __nv_bfloat162*>(&graw.y);
     uint2 o;
-    o.x = pack_bf16(v.x * inv * __low2float(g0), v.y * inv * __high2float(g0));
-    o.y = pack_bf16(v.z * inv * __low2float(g1), v.w * inv * __high2float(g1));
+    o.x = pack_act(v.x * inv * __low2float(g0), v.y * inv * __high2float(g0));
+    o.y = pack_act(v.z * inv * __low2float(g1), v.w * inv * __high2float(g1));
     *reinterpret_cast<uint2*>(yr + c) = o;
   }
 }
 
 __global__ void __launch_bounds__(1024)
 residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int n_parts, long long part_stride,
-                     const __nv_bfloat16* __restrict__ g, __nv_bfloat16* __restrict__ y, int D, float eps) {
+                     const __nv_bfloat16* __restrict__ g, act_t* __restrict__ y, int D, float eps) {
   pdl_wait();
   pdl_launch_dependents();
   residual_norm_row(x, parts, n_parts, part_stride, g, y, blockIdx.x, blockIdx.x, D, eps);
@@ -122,10 +122,10 @@ residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int
 
 struct RowListArg { int rows[256]; };  // a10: the caller's row list, passed by value (no staging copy)
 
-// a10: y[i,:] = bf16( RMSNorm(hidden[rows[i],:]; g_final) ), the input of the LM-head GEMM
+// a10: y[i,:] = fp16( RMSNorm(hidden[rows[i],:]; g_final) ), the input of the LM-head GEMM
 __global__ void __launch_bounds__(1024)
 gather_norm_kernel(const RowListArg rl, const float* __restrict__ x, const __nv_bfloat16* __restrict__ g,
-                   __nv_bfloat16* __restrict__ y, int D, float eps) {
+                   act_t* __restrict__ y, int D, float eps) {
   pdl_wait();
   pdl_launch_dependents();
   residual_norm_row(const_cast<float*>(x), nullptr, 0, 0, g, y, blockIdx.x, rl.rows[blockIdx.x], D, eps);
@@ -135,9 +135,9 @@ gather_norm_kernel(const RowListArg rl, const float* __restrict__ x, const __nv_
 // position in its own request (rotate-half pairing, table built in fp64), write q to the query buffer and
 // k (rotated), v straight to the row's ring slot.  One block per row, 8 elements (16 bytes) per thread-iteration.
 __global__ void __launch_bounds__(1024)
-rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q | k | v)
-                   __nv_bfloat16* __restrict__ q_out,       // [T, H*hd]
-                   __nv_bfloat16* __restrict__ kv_layer,    // [2][R][H][C][hd]
+rope_append_kernel(const act_t* __restrict__ qkv,   // [T, 3*H*hd]  (q | k | v)
+                   act_t* __restrict__ q_out,       // [T, H*hd]
+                   act_t* __restrict__ kv_layer,    // [2][R][H][C][hd]
                    const float2* __restrict__ rope_tab,     // [C][hd/2] (cos, sin)
                    StepTables tb, int H, int hd, int R, int C) {
   pdl_wait();
@@ -146,7 +146,7 @@ rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q |
   const int pos = tb.row_pos[i], gslot = tb.row_slot[i];
   const int req = gslot / C, slot = gslot - req * C;
   const int D = H * hd, half = hd >> 1;
-  const __nv_bfloat16* src = qkv + static_cast<size_t>(i) * 3 * D;
+  const act_t* src = qkv + static_cast<size_t>(i) * 3 * D;
   const float2* tab = rope_tab + static_cast<size_t>(pos) * half;
   const int per_head = half / 8;  // 16-byte groups of the low half of a head
   // q and k: thread handles 8 low-half elements c..c+7 and their partners c+half..
@@ -154,23 +154,23 @@ rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q |
     const int which = w / (H * per_head);           // 0 = q, 1 = k
     const int rem = w - which * H * per_head;
     const int h = rem / per_head, c = (rem - h * per_head) * 8;
-    const __nv_bfloat16* s = src + which * D + h * hd + c;
+    const act_t* s = src + which * D + h * hd + c;
     const uint4 lo_raw = *reinterpret_cast<const uint4*>(s);
     const uint4 hi_raw = *reinterpret_cast<const uint4*>(s + half);
-    const __nv_bfloat16* lo = reinterpret_cast<const __nv_bfloat16*>(&lo_raw);
-    const __nv_bfloat16* hi = reinterpret_cast<const __nv_bfloat16*>(&hi_raw);
+    const act_t* lo = reinterpret_cast<const act_t*>(&lo_raw);
+    const act_t* hi = reinterpret_cast<const act_t*>(&hi_raw);
     uint4 out_lo, out_hi;
     uint32_t* ol = reinterpret_cast<uint32_t*>(&out_lo);
     uint32_t* oh = reinterpret_cast<uint32_t*>(&out_hi);
 #pragma unroll
     for (int e = 0; e < 8; e += 2) {
       const float2 cs0 = tab[c + e], cs1 = tab[c + e + 1];
-      const float l0 = __bfloat162float(lo[e]), l1 = __bfloat162float(lo[e + 1]);
-      const float h0 = __bfloat162float(hi[e]), h1 = __bfloat162float(hi[e + 1]);
-      ol[e >> 1] = pack_bf16(l0 * cs0.x - h0 * cs0.y, l1 * cs1.x - h1 * cs1.y);
-      oh[e >> 1] = pack_bf16(h0 * cs0.x + l0 * cs0.y, h1 * cs1.x + l1 * cs1.y);
+      const float l0 = act2f(lo[e]), l1 = act2f(lo[e + 1]);
+      const float h0 = act2f(hi[e]), h1 = act2f(hi[e + 1]);
+      ol[e >> 1] = pack_act(l0 * cs0.x - h0 * cs0.y, l1 * cs1.x - h1 * cs1.y);
+      oh[e >> 1] = pack_act(h0 * cs0.x + l0 * cs0.y, h1 * cs1.x + l1 * cs1.y);
     }
-    __nv_bfloat16* dst = (which == 0)
+    act_t* dst = (which == 0)
         ? q_out + static_cast<size_t>(i) * D + h * hd + c
         : kv_layer + ((static_cast<size_t>(0 * R + req) * H + h) * C + slot) * hd + c;
     *reinterpret_cast<uint4*>(dst) = out_lo;
@@ -182,6 +182,15 @@ rope_append_kernel(const __nv_bfloat16* __restrict__ qkv,   // [T, 3*H*hd]  (q |
     const uint4 v = *reinterpret_cast<const uint4*>(src + 2 * D + w * 8);
     *reinterpret_cast<uint4*>(kv_layer + ((static_cast<size_t>(1 * R + req) * H + h) * C + slot) * hd + c) = v;
   }
+}
+
+// Load-time weight preparation: bf16 -> fp16, exact for finite |w| in [2^-14, 65504] (8 elements per thread).
+__global__ void convert_bf16_to_fp16_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, size_t n_vec) {
+  const size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n_vec) return;
+  uint4 v = src[i];
+  v.x = bf16x2_to_f16x2(v.x); v.y = bf16x2_to_f16x2(v.y); v.z = bf16x2_to_f16x2(v.z); v.w = bf16x2_to_f16x2(v.w);
+  dst[i] = v;
 }
 
 // RoPE table in fp64: tab[pos][c] = (cos, sin)(pos * theta^(-2c/hd))

@@ -15,7 +15,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   const uint32_t stage_bytes = a_bytes + b_bytes;
   float* xch = reinterpret_cast<float*>(tiles + static_cast<size_t>(p.stages) * stage_bytes);
 
-  __shared__ uint64_t full_bar[GEMM_MAX_STAGES], empty_bar[GEMM_MAX_STAGES], tmem_full_bar, tmem_empty_bar, fix_bar;
+  __shared__ uint64_t full_bar[GEMM_MAX_STAGES], conv_bar[GEMM_MAX_STAGES], empty_bar[GEMM_MAX_STAGES], tmem_full_bar,
+      tmem_empty_bar, fix_bar;
   __shared__ uint32_t tmem_base_smem;
 
   const int warp = threadIdx.x >> 5;
@@ -34,6 +35,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     tma_prefetch_desc(&map_part);
     for (int s = 0; s < p.stages; ++s) {
       mbar_init(&full_bar[s], 1);
+      mbar_init(&conv_bar[s], GEMM_EPI_WARPS);
       mbar_init(&empty_bar[s], 1);
     }
     mbar_init(&tmem_full_bar, 1);
@@ -128,7 +130,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         mbar_wait(&tmem_empty_bar, acc_phase ^ 1);  // epilogue has drained the accumulator
         tc_fence_after();
         for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(&full_bar[stage], phase);
+          // the stage has landed (and, for bf16 weights, the epilogue warps have rewritten the W tile as fp16)
+          mbar_wait(p.w_fp16 ? &full_bar[stage] : &conv_bar[stage], phase);
           tc_fence_after();
           const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
           const uint32_t sb = sa + a_bytes;
@@ -186,7 +189,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     if (etid == 0) AF_TRACE(1);
     int piece = 0;
     const int stage_area = p.stages * static_cast<int>(stage_bytes);
-    uint32_t acc_phase = 0, fix_phase = 0;
+    uint32_t acc_phase = 0, fix_phase = 0, cphase = 0;
+    int cstage = 0;
     int u = u_begin;
     while (u < u_end) {
       const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
@@ -194,6 +198,23 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       const bool streamk = p.split == SPLIT_STREAMK;
       const bool contributor = streamk && kb0 > 0;
       const bool owner_partial = streamk && (kb0 == 0) && (kb1 < p.num_kb);
+      // ---- weight transform: this piece's W stages bf16 -> fp16, in place, as they land (exact for every finite
+      //      bf16 weight below 65504 in magnitude; values under 2^-14 keep 10 + e bits as fp16 subnormals) ----
+      for (int kb = p.w_fp16 ? kb1 : kb0; kb < kb1; ++kb) {
+        mbar_wait(&full_bar[cstage], cphase);
+        uint4* wst = reinterpret_cast<uint4*>(tiles + static_cast<size_t>(cstage) * stage_bytes);
+#pragma unroll
+        for (int i = 0; i < static_cast<int>(a_bytes / 16) / (GEMM_EPI_WARPS * 32); ++i) {
+          uint4 raw = wst[etid + i * GEMM_EPI_WARPS * 32];
+          raw.x = bf16x2_to_f16x2(raw.x); raw.y = bf16x2_to_f16x2(raw.y);
+          raw.z = bf16x2_to_f16x2(raw.z); raw.w = bf16x2_to_f16x2(raw.w);
+          wst[etid + i * GEMM_EPI_WARPS * 32] = raw;
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&conv_bar[cstage]);
+        if (++cstage == p.stages) { cstage = 0; cphase ^= 1; }
+      }
       int c_first = 0, n_contrib = 0;
       if (owner_partial) {
         // CTAs holding the rest of this tile: cta+1 .. while their range starts before the tile ends
@@ -286,23 +307,28 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
           if (contributor) stage_store(&map_part, quad * 32, c0, cta);
           else stage_store(&map_out, f0, mid, p.tok0 + c0);
-        } else if (p.epi == EPI_STORE) {  // bf16, one 32-token box
+        } else if (p.epi == EPI_STORE) {  // bf16 or fp16, one 32-token box
           stage_free();
-          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stg);
+          uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
+          if (p.out_bf16 == 2) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __float2bfloat16_rn(v[j]);
+            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __half_as_ushort(__float2half_rn(v[j]));
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __bfloat16_as_ushort(__float2bfloat16_rn(v[j]));
+          }
           stage_store(&map_out, f0, mid, p.tok0 + c0);
         } else {
           // EPI_SWIGLU: lanes 0-15 hold gate, lanes 16-31 hold up of the same 16 features.  Lanes 0-15 finish tokens
           // 0-15 of the chunk, lanes 16-31 tokens 16-31; each gets the other half's operand with one shuffle.
           stage_free();
-          __nv_bfloat16* sb = reinterpret_cast<__nv_bfloat16*>(stg);
+          act_t* sb = reinterpret_cast<act_t*>(stg);
           const bool lo = lane < 16;
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             const float other = __shfl_xor_sync(0xffffffffu, lo ? v[j + 16] : v[j], 16);
             const float g = lo ? v[j] : other, up = lo ? other : v[j + 16];
-            sb[(lo ? j : j + 16) * 16 + (lane & 15)] = __float2bfloat16_rn(__fdividef(g, 1.f + __expf(-g)) * up);
+            sb[(lo ? j : j + 16) * 16 + (lane & 15)] = __float2half_rn(fminf(fmaxf(__fdividef(g, 1.f + __expf(-g)) * up, -65504.f), 65504.f));
           }
           stage_store(&map_out, f0, mid, p.tok0 + c0);
         }

@@ -3,9 +3,20 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 
 namespace af {
+
+// Activations (normed rows, q/k/v, the KV ring, attention probabilities and outputs, the SwiGLU product) are fp16:
+// same bytes as bf16 with 3 more mantissa bits.  Weights are bf16 in global memory and are converted to fp16 (exactly)
+// tile by tile in shared memory; every accumulation is fp32.
+using act_t = __half;
+__device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
+  __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ float act2f(act_t v) { return __half2float(v); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -156,9 +167,17 @@ __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr) {
   d |= static_cast<uint64_t>(2) << 61;
   return d;
 }
-// Instruction descriptor, kind::f16: D = fp32, A = B = bf16, both K-major, M x N tile.
+// Instruction descriptor, kind::f16: D = fp32 (bits 4-5 = 1), A = B = fp16 (format 0 in bits 7-9 and 10-12; bf16
+// would be 1), both K-major, M x N tile.  A and B must share one format: a bf16 x fp16 mix raises an
+// illegal-instruction fault on sm_100a, which is why the bf16 weight tiles are converted to fp16 in shared memory.
 __device__ __forceinline__ uint32_t umma_idesc_bf16(uint32_t M, uint32_t N) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+  return (1u << 4) | (0u << 7) | (0u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+// two packed bf16 -> two packed fp16 (round to nearest; exact for finite |x| in [2^-14, 65504])
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t v) {
+  const float lo = __uint_as_float(v << 16), hi = __uint_as_float(v & 0xffff0000u);
+  __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
 }
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {

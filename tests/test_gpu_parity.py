@@ -29,7 +29,7 @@ def test_gemm_tcgen05_vs_fp64(binding, n_tok, n_out, k):
     """out = a w^T through the tcgen05/TMA stream-K kernel; odd shapes span several tiles, a ragged feature tail,
     a ragged k tail (688 = 10.75 k-blocks), both token halves and the multi-launch token chunking."""
     g = torch.Generator().manual_seed(n_tok * 7919 + n_out * 31 + k)
-    a = torch.randn(n_tok, k, generator=g).to(torch.bfloat16)
+    a = torch.randn(n_tok, k, generator=g).to(torch.float16)
     w = (0.05 * torch.randn(n_out, k, generator=g)).to(torch.bfloat16)
     ref = a.double() @ w.double().T
     got = binding.debug_gemm(a.cuda(), w.cuda())
@@ -40,7 +40,7 @@ def test_gemm_tcgen05_vs_fp64(binding, n_tok, n_out, k):
 
 def test_gemm_deterministic(binding):
     g = torch.Generator().manual_seed(5)
-    a = torch.randn(282, 4096, generator=g).to(torch.bfloat16).cuda()
+    a = torch.randn(282, 4096, generator=g).to(torch.float16).cuda()
     w = (0.02 * torch.randn(4096, 4096, generator=g)).to(torch.bfloat16).cuda()
     o1 = binding.debug_gemm(a, w).clone()
     o2 = binding.debug_gemm(a, w)
@@ -177,3 +177,26 @@ def test_cfg2_single_7b_layer(binding):
     hid, ref = P.step(segs, I.make_embeds(cfg, 1, 0, 282))
     P.check_ring(list(range(7)))
     P.check_logits(hid, ref, I.prediction_rows(segs))
+
+
+def test_bf16_weight_path_equals_prepared_fp16_path(binding):
+    """AF_WEIGHTS_BF16 (every weight tile converted bf16 -> fp16 in shared memory by the GEMM) and AF_WEIGHTS_FP16
+    (matrices prepared once by af_convert_bf16_to_fp16) hold the same values, so the two paths agree bit for bit."""
+    cfg = I.CFG_TINY
+    hw = I.make_weights(cfg, seed=0)
+    e = I.make_embeds(cfg, 0, 7, 100).cuda()
+    outs = []
+    for prepared in (True, False):
+        W = binding.Weights(cfg, hw, prepared=prepared)
+        ring = binding.Ring(cfg, 4, 128, max_rows=128)
+        hid = ring.packed_forward(W, e, [(0, 0, 0, 60), (3, 0, 0, 40)])
+        outs.append((hid.clone(), ring.logits_rows(W, hid, [59, 99]).clone()))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    w = (0.02 * torch.randn(256, 512)).to(torch.bfloat16).cuda()
+    w16 = torch.empty(256, 512, dtype=torch.float16, device="cuda")
+    L = binding.load_library()
+    assert L.af_convert_bf16_to_fp16(w.data_ptr(), w16.data_ptr(), w.numel(), None) == 0
+    torch.cuda.synchronize()
+    big = w.float().abs() >= 2.0 ** -14
+    assert torch.equal(w16.float()[big], w.float()[big])                   # exact in the fp16 normal range
+    assert float((w16.float() - w.float()).abs().max()) <= 2.0 ** -25        # fp16 subnormals below it
