@@ -259,8 +259,10 @@ def main():
     line = {
         "metric": "action_frames_per_s", "value": fps, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
         "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": "f16", "data": "synthetic",
         "config": {"workload": WORKLOAD if args.layers == 32 else f"DEBUG {args.layers}-layer slice of " + WORKLOAD,
+                   "precision": "bf16-valued weights stored as fp16 (af_convert_bf16_to_fp16 at load, exact), fp16 "
+                                "activations and KV ring, fp32 accumulate / residual / logits (tcgen05 kind::f16)",
                    "packed_rows": T, "ring": f"{R_REGIONS} regions x {CAPACITY}", "multi_gpu": "independent replicas",
                    "l2": "inputs larger than L2 (13.2 GB of weights streamed per step vs 126 MB L2)"},
         "packed_tok_per_s": fps * T,
