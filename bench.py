@@ -24,6 +24,9 @@ sys.path.insert(0, ROOT)
 
 L_P, K_STAGES, R_REGIONS, CAPACITY = 276, 7, 8, 512      # 256 patch + 20 prompt tokens, K = 7 action tokens
 SEED = 2
+# DRAM bytes per gemm_tcgen05_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, averaged over the launches of
+# a steady step; cold caches): profiles/launches_r1.md.  Algorithmic weight bytes per launch: 102.8 MB.
+GEMM_TRAFFIC_BYTES_PER_LAUNCH = 109.7e6
 WORKLOAD = "cfg3: 32-layer Llama-2-7B shape, steady pipelined step = 276-row prefill + 6 decodes (ctx 277..282) + LM head on 7 rows"
 
 
@@ -272,7 +275,8 @@ def main():
                           "peaks": peaks, "flops": work["flops"], "bytes": work["bytes"]},
         "roofline": {"kernel": "gemm_tcgen05_kernel (all packed projections + LM head)", "bound": "tensor",
                      "achieved": achieved_tf, "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
-                     "frac": achieved_tf / peaks["tf_sustained"], "traffic": None,
+                     "frac": achieved_tf / peaks["tf_sustained"],
+                     "traffic": GEMM_TRAFFIC_BYTES_PER_LAUNCH if args.layers == 32 else None,
                      "peak_source": peaks["source"] + " sustained bf16 (kernel timed inside a long step)",
                      "launches_per_step": gemm_n, "avg_launch_ms": gemm_ms / max(1, gemm_n),
                      "share_of_step": gemm_ms / all_ms,
