@@ -149,6 +149,14 @@ int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32
 int af_debug_profile(int enable);
 int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
 
+/* Debug timeline of the GEMM kernel: while enabled every gemm_tcgen05_kernel launch records %globaltimer / clock stamps
+ * per CTA (kernel start, PDL wait, per piece: accumulator ready / fix-up loaded / drained, producer and MMA-thread
+ * counters) into a library-owned device buffer that keeps the last 16 launches.  af_debug_trace_read synchronises and
+ * copies them out: stamps = HOST int64 [16][160][32], meta = HOST int32 [16][2] (kernel class as in af_debug_profile,
+ * grid size); returns the number of launches recorded since af_debug_trace(1), or a negative AF_ERR_*. */
+int af_debug_trace(int enable);
+int af_debug_trace_read(long long* stamps, int* meta);
+
 const char* af_last_error(void); /* thread-local message of the last failing call */
 
 #ifdef __cplusplus

@@ -152,14 +152,25 @@ static int get_out_map(const OutView& o, CUtensorMap* out) {
 // allocation, tensor-map prefetch, the first weight tiles) overlaps the previous kernel's tail, and each kernel
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
 static bool g_use_pdl = true;
+static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
+static int g_launch_cluster = 1;  // cluster size of the next launch_k call (set by launch_gemm, reset after the launch)
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = g_use_pdl ? 1 : 0;
+  cudaLaunchAttribute at[2];
+  int n = 0;
+  if (g_use_pdl) {
+    at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[n].val.programmaticStreamSerializationAllowed = 1;
+    ++n;
+  }
+  if (g_launch_cluster > 1) {
+    at[n].id = cudaLaunchAttributeClusterDimension;
+    at[n].val.clusterDim.x = g_launch_cluster; at[n].val.clusterDim.y = 1; at[n].val.clusterDim.z = 1;
+    ++n;
+  }
+  cfg.attrs = at; cfg.numAttrs = n;
   return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
@@ -178,6 +189,7 @@ static int gemm_global_init() {
   if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
   g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
   if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
+  if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
   CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
@@ -213,6 +225,16 @@ extern "C" int af_debug_trace_read(long long* out, int* meta) {
 // threads of the one-block-per-row kernels: one 16-byte access per thread where the row allows it
 static int row_threads_for(int D) { int t = (D / 4 + 31) / 32 * 32; return t < 64 ? 64 : (t > 1024 ? 1024 : t); }
 
+// split-K pieces per tile of the O / down projections (also the number of slabs the next residual kernel adds)
+static int gemm_split_count(int n_tiles, int K) {
+  const int cluster = (g_gemm_cluster > 1 && n_tiles >= 2) ? 2 : 1;
+  const int n_pairs = (n_tiles + cluster - 1) / cluster, nkb = (K + GEMM_BK - 1) / GEMM_BK;
+  int s = (g_num_sms / cluster) / n_pairs;
+  if (s > GEMM_MAX_SPLITS) s = GEMM_MAX_SPLITS;
+  if (s > nkb) s = nkb;
+  return s < 1 ? 1 : s;
+}
+
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
 // One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
@@ -234,19 +256,22 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
     p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
-    p.total_units = n_tiles * p.num_kb;
+    p.xh = p.n2 > 0 ? p.n1 : p.n1 / 2;
+    p.n_tiles = n_tiles;
+    p.cluster = (g_gemm_cluster > 1 && n_tiles >= 2) ? 2 : 1;
+    const int n_pairs = (n_tiles + p.cluster - 1) / p.cluster;     // work units are (tile pair, k-block) per cluster
+    const int max_cl = g_num_sms / p.cluster;
+    p.total_units = n_pairs * p.num_kb;
     int grid;
     if (p.split == SPLIT_K) {
-      int s = g_num_sms / n_tiles;
-      if (s > GEMM_MAX_SPLITS) s = GEMM_MAX_SPLITS;
-      if (s > p.num_kb) s = p.num_kb;
-      if (s < 1) s = 1;
-      p.splits = s; p.units_per_cta = 0;
-      grid = n_tiles * s;
+      p.splits = gemm_split_count(n_tiles, p.K);
+      p.units_per_cta = 0;
+      grid = n_pairs * p.splits * p.cluster;
     } else {
-      grid = p.total_units < g_num_sms ? p.total_units : g_num_sms;
-      p.units_per_cta = (p.total_units + grid - 1) / grid;
-      grid = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+      int n_cl = p.total_units < max_cl ? p.total_units : max_cl;
+      p.units_per_cta = (p.total_units + n_cl - 1) / n_cl;
+      n_cl = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+      grid = n_cl * p.cluster;
       p.splits = 1;
     }
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + n_pad * GEMM_BK * 2;
@@ -262,7 +287,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
       rc = get_map(w[i < n_w ? i : 0], p.part_rows, p.K, box_rows, &mw[i]);
       if (rc) return rc;
     }
-    rc = get_map(x, x_rows_cap, p.K, p.n1, &mx);
+    rc = get_map(x, x_rows_cap, p.K, p.xh, &mx);
     if (rc) return rc;
     CUtensorMap mo, mp;
     p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
@@ -276,7 +301,9 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_XCH_BYTES + 1024;
     {
       ProfScope ps(cat, st);
+      g_launch_cluster = p.cluster;
       cudaError_t e = launch_k(gemm_tcgen05_kernel, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
+      g_launch_cluster = 1;
       if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gemm_tcgen05_kernel failed: %s", cudaGetErrorString(e));
     }
     rc = check_launch("gemm_tcgen05_kernel");
@@ -539,12 +566,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   const long long split_stride = static_cast<long long>(ws.max_rows) * D;
   int prev_splits = 0;   // split-K slabs of the previous projection still to be added to the residual stream
-  auto split_count = [&](int n_tiles, int K) {
-    int s2 = g_num_sms / n_tiles, nkb = (K + GEMM_BK - 1) / GEMM_BK;
-    if (s2 > GEMM_MAX_SPLITS) s2 = GEMM_MAX_SPLITS;
-    if (s2 > nkb) s2 = nkb;
-    return s2 < 1 ? 1 : s2;
-  };
+  auto split_count = [&](int n_tiles, int K) { return gemm_split_count(n_tiles, K); };
   const int d_tiles = (D + GEMM_BM - 1) / GEMM_BM;
   for (int l = 0; l < c.n_layers; ++l) {
     const af_layer_weights& L = w->layers[l];

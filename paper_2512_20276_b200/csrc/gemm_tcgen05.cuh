@@ -55,6 +55,9 @@ struct GemmParams {
   int K, num_kb;       // reduction length, ceil(K / 64)
   int T, tok0;         // valid tokens of this launch, first token row
   int n1, n2;          // UMMA N of the two token halves (multiples of 16, n2 may be 0)
+  int xh;              // token rows per activation TMA box (two boxes per k-block): n1 if n2 > 0, else n1 / 2
+  int n_tiles;         // weight tiles in all
+  int cluster;         // CTAs per cluster: 1, or 2 (activation boxes multicast, work units = tile pairs)
   int split;           // GemmSplit
   int splits;          // SPLIT_K: pieces per tile
   int total_units, units_per_cta;  // SPLIT_STREAMK

@@ -22,6 +22,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const int cta = blockIdx.x;
+  // 2-CTA cluster: both CTAs sweep the same k-blocks of two neighbouring weight tiles and each loads one half of the
+  // activation k-block, multicast into both (halves the L2 -> SM traffic of the operand every CTA needs in full)
+  const int crank = p.cluster > 1 ? static_cast<int>(cluster_ctarank()) : 0;
+  const int cl = cta / p.cluster;   // work is split over clusters; a cluster's unit = (tile pair, k-block)
   long long* trace = p.trace ? p.trace + static_cast<size_t>(cta) * 32 : nullptr;
 #define AF_TRACE(slot) do { if (trace) trace[slot] = static_cast<long long>(globaltimer_ns()); } while (0)
   if (trace && threadIdx.x == 0) AF_TRACE(0);
@@ -36,7 +40,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     for (int s = 0; s < p.stages; ++s) {
       mbar_init(&full_bar[s], 1);
       mbar_init(&conv_bar[s], GEMM_EPI_WARPS);
-      mbar_init(&empty_bar[s], 1);
+      mbar_init(&empty_bar[s], p.cluster);
     }
     mbar_init(&tmem_full_bar, 1);
     mbar_init(&tmem_empty_bar, GEMM_EPI_WARPS);
@@ -46,17 +50,18 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   if (warp == GEMM_EPI_WARPS + 1) tmem_alloc(&tmem_base_smem, GEMM_TMEM_COLS);
   tc_fence_before();
   __syncthreads();
+  if (p.cluster > 1) cluster_sync();  // the peer's barriers exist before anything is multicast to them
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
   pdl_launch_dependents();  // dependents still wait (griddepcontrol.wait) for this whole grid before reading its output
 
   int u_begin, u_end;
   if (p.split == SPLIT_K) {
-    const int tile = cta / p.splits, s = cta - tile * p.splits;
+    const int tile = cl / p.splits, s = cl - tile * p.splits;
     u_begin = tile * p.num_kb + static_cast<int>(static_cast<long long>(s) * p.num_kb / p.splits);
     u_end = tile * p.num_kb + static_cast<int>(static_cast<long long>(s + 1) * p.num_kb / p.splits);
   } else {
-    u_begin = min(cta * p.units_per_cta, p.total_units);
+    u_begin = min(cl * p.units_per_cta, p.total_units);
     u_end = min(u_begin + p.units_per_cta, p.total_units);
   }
 
@@ -65,15 +70,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     if (lane == 0) {
       const uint64_t pol_w = policy_evict_first();  // weights are streamed once per step
       const uint64_t pol_x = policy_evict_last();   // the packed activations are re-read by every CTA
-      // SPLIT_K: CTAs of one split would sweep the same k-blocks in lockstep; rotate each tile's sweep instead
-      const int rot_lo = u_begin % p.num_kb, rot_len = u_end - u_begin;
-      const int rot = (p.split == SPLIT_K && (p.dbg & 16)) ? ((u_begin / p.num_kb) * 5) % rot_len : 0;
-      auto kb_of = [&](int u) {
-        const int kb = u % p.num_kb;
-        return rot ? rot_lo + (kb - rot_lo + rot) % rot_len : kb;
-      };
       auto load_w = [&](int u, int stage) {
-        const int tile = u / p.num_kb, kb = kb_of(u);
+        const int kb = u % p.num_kb;
+        const int tile = min((u / p.num_kb) * p.cluster + crank, p.n_tiles - 1);  // (an odd tile count: reload the last)
         uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
         if (p.a_pair) {  // every TMEM lane quadrant = 16 gate rows + the 16 up rows of the same features
 #pragma unroll
@@ -87,13 +86,17 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           tma_load_2d(sa, mw, &full_bar[stage], kb * GEMM_BK, tip * GEMM_BM, pol_w);
         }
       };
+      // the activation k-block = two boxes of p.xh token rows; in a cluster CTA r loads box r for both CTAs
       auto load_x = [&](int u, int stage) {
-        const int kb = kb_of(u);
+        const int kb = u % p.num_kb;
         uint8_t* sb = tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes;
-        tma_load_2d(sb, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0, pol_x);
-        if (p.n2 > 0)
-          tma_load_2d(sb + static_cast<size_t>(p.n1) * GEMM_BK * 2, &map_x, &full_bar[stage], kb * GEMM_BK,
-                      p.tok0 + p.n1, pol_x);
+        const size_t half = static_cast<size_t>(p.xh) * GEMM_BK * 2;
+        if (p.cluster > 1) {
+          tma_load_2d_mc(sb + crank * half, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0 + crank * p.xh, 0x3, pol_x);
+        } else {
+          tma_load_2d(sb, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0, pol_x);
+          tma_load_2d(sb + half, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0 + p.xh, pol_x);
+        }
       };
       // The weights do not depend on the previous kernel: start streaming them before the PDL dependency resolves.
       const int n_pre = min(p.stages, u_end - u_begin);
@@ -109,9 +112,20 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       uint32_t phase = n_pre == p.stages ? 1 : 0;
       for (int u = u_begin + n_pre; u < u_end; ++u) {
         mbar_wait(&empty_bar[stage], phase ^ 1);
+        const int ui = u - u_begin - 8;
+        if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[2 + 4 * ui] = clock64();
+        if (p.dbg & 1) {        // experiment: no activation loads after the first round (stale tiles are re-used)
+          mbar_arrive_expect_tx(&full_bar[stage], a_bytes);
+          load_w(u, stage);
+        } else if (p.dbg & 2) { // experiment: no weight loads after the first round
+          mbar_arrive_expect_tx(&full_bar[stage], stage_bytes - a_bytes);
+          load_x(u, stage);
+        } else {
         mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
         load_w(u, stage);
         load_x(u, stage);
+        }
+        if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[3 + 4 * ui] = clock64();
         if (++stage == p.stages) { stage = 0; phase ^= 1; }
       }
       AF_TRACE(26);
@@ -124,15 +138,21 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       int stage = 0;
       uint32_t phase = 0, acc_phase = 0;
       int u = u_begin;
+      long long t_wait = 0, t_issue = 0, t_acc = 0, t_prev = trace ? clock64() : 0;
+#define AF_MT(var) do { if (trace) { const long long t_ = clock64(); var += t_ - t_prev; t_prev = t_; } } while (0)
       while (u < u_end) {
         const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
         const int kb1 = min(p.num_kb, kb0 + (u_end - u));
         mbar_wait(&tmem_empty_bar, acc_phase ^ 1);  // epilogue has drained the accumulator
         tc_fence_after();
+        AF_MT(t_acc);
         for (int kb = kb0; kb < kb1; ++kb) {
           // the stage has landed (and, for bf16 weights, the epilogue warps have rewritten the W tile as fp16)
           mbar_wait(p.w_fp16 ? &full_bar[stage] : &conv_bar[stage], phase);
           tc_fence_after();
+          AF_MT(t_wait);
+          const int ui = u + (kb - kb0) - u_begin - 8;
+          if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[4 + 4 * ui] = clock64();
           const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
           const uint32_t sb = sa + a_bytes;
           const uint64_t da = umma_smem_desc_sw128(sa);
@@ -145,13 +165,18 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
             umma_bf16(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
             if (p.n2 > 0) umma_bf16(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
           }
-          umma_commit(&empty_bar[stage]);  // frees the smem slot when these MMAs have read it
+          // frees the smem slot when these MMAs have read it (in a cluster: in both CTAs, the peer multicasts into it)
+          if (p.cluster > 1) umma_commit_mc(&empty_bar[stage], 0x3); else umma_commit(&empty_bar[stage]);
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
+          AF_MT(t_issue);
+          if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[5 + 4 * ui] = clock64();
         }
         umma_commit(&tmem_full_bar);  // accumulator complete -> epilogue
         acc_phase ^= 1;
         u += kb1 - kb0;
       }
+      if (trace) { trace[28] = t_wait; trace[29] = t_issue; trace[30] = t_acc; trace[31] = u_end - u_begin; }
+#undef AF_MT
     }
   } else {
     // ================================ epilogue warps 0..7 ================================
@@ -164,6 +189,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     const int etid = threadIdx.x;  // 0..255
     uint8_t* stg_base = reinterpret_cast<uint8_t*>(xch) + warp * 8192;
     uint32_t n_st = 0;  // TMA stores issued by this warp; buffer = n_st & 1
+    bool store_ok = true;
 #define stg (stg_base + (n_st & 1) * 4096)
     long long tk[6] = {0, 0, 0, 0, 0, 0};
     long long tk0 = 0;
@@ -178,7 +204,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       fence_proxy_async();
       __syncwarp();
       AF_TICK(4);
-      if (lane == 0) {
+      if (lane == 0 && store_ok) {
         tma_store_3d(m, stg, c0_, c1_, c2_);
         bulk_commit();
       }
@@ -193,8 +219,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     int cstage = 0;
     int u = u_begin;
     while (u < u_end) {
-      const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
+      const int pair = u / p.num_kb, kb0 = u - pair * p.num_kb;
       const int kb1 = min(p.num_kb, kb0 + (u_end - u));
+      const int tile = pair * p.cluster + crank;
+      const bool tile_valid = tile < p.n_tiles;   // (an odd tile count leaves the last cluster's second CTA idle)
       const bool streamk = p.split == SPLIT_STREAMK;
       const bool contributor = streamk && kb0 > 0;
       const bool owner_partial = streamk && (kb0 == 0) && (kb1 < p.num_kb);
@@ -218,12 +246,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       int c_first = 0, n_contrib = 0;
       if (owner_partial) {
         // CTAs holding the rest of this tile: cta+1 .. while their range starts before the tile ends
-        c_first = cta + 1;
-        const int tile_end = (tile + 1) * p.num_kb;
-        const int c_last = min((tile_end - 1) / p.units_per_cta, static_cast<int>(gridDim.x) - 1);
+        c_first = cl + 1;   // cluster index; the contributing CTA of cluster c is c * cluster + crank
+        const int tile_end = (pair + 1) * p.num_kb;
+        const int c_last = min((tile_end - 1) / p.units_per_cta, static_cast<int>(gridDim.x) / p.cluster - 1);
         n_contrib = c_last - c_first + 1;
         if (etid < n_contrib) {
-          volatile int* f = p.flags + c_first + etid;
+          volatile int* f = p.flags + (c_first + etid) * p.cluster + crank;
           while (*f == 0) {
           }
           *f = 0;  // one consumer per flag: ready for the next launch (graph-replay safe)
@@ -231,10 +259,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
         AF_EPI_BAR();
       }
-      if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
+      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(2 + 4 * piece);
       mbar_wait(&tmem_full_bar, acc_phase);
       tc_fence_after();
-      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
+      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(3 + 4 * piece);
+      store_ok = tile_valid;
       // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
       int f0, mid;
       if (p.a_pair) {
@@ -242,7 +271,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       } else {
         const int part = tile / p.tiles_per_part;
         f0 = (tile - part * p.tiles_per_part) * GEMM_BM + quad * 32;
-        mid = p.split == SPLIT_K ? cta % p.splits : part;
+        mid = p.split == SPLIT_K ? cl % p.splits : part;
       }
       // column blocks: with contributors, their partial columns [b0, b1) are bulk-copied into the (now idle) stages,
       // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 64-column blocks
@@ -267,7 +296,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           mbar_arrive_expect_tx(&fix_bar, bytes * cnt);
           for (int c = 0; c < cnt; ++c)
             bulk_load_1d(tiles + static_cast<size_t>(c) * bytes,
-                         p.partial + (static_cast<size_t>(c_first + g0 + c) * GEMM_MAX_TOK + b0) * GEMM_BM, bytes,
+                         p.partial + (static_cast<size_t>((c_first + g0 + c) * p.cluster + crank) * GEMM_MAX_TOK + b0) * GEMM_BM,
+                         bytes,
                          &fix_bar);
         }
         mbar_wait(&fix_bar, fix_phase);
@@ -339,7 +369,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         if (n_groups <= 1) {
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
-            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
+            if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(4 + 4 * piece);
           }
           for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += 64) {
             const int cw = min(32, b1 - c0);
@@ -373,7 +403,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           atomicExch(p.flags + cta, 1);
         }
       }
-      if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
+      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(5 + 4 * piece);
       if (etid == 0 && trace) { for (int i = 0; i < 6; ++i) trace[18 + i] = tk[i]; }
       ++piece;
       acc_phase ^= 1;
@@ -386,6 +416,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
 
   tc_fence_before();
   __syncthreads();
+  if (p.cluster > 1) cluster_sync();  // no CTA leaves while its peer may still signal its barriers
   if (warp == GEMM_EPI_WARPS + 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, GEMM_TMEM_COLS);
