@@ -162,7 +162,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2512_20276_b200 import binding, inputs as I
+    from paper_2512_20276_b200 import binding, inputs as I, replicas
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -196,8 +196,7 @@ def main():
         tau[0] = t + 1
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize()
 
     for _ in range(K_STAGES - 1 + warmup):                       # pipeline fill + warm-up (untimed)
@@ -238,10 +237,7 @@ def main():
     binding.profile(False)
     clocks = sampler.stop()
 
-    t_dev = torch.tensor([ms_dev, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-    ms_dev, ms_e2e = float(t_dev[0]), float(t_dev[1])
+    ms_dev, ms_e2e = replicas.max_over_ranks([ms_dev, ms_e2e], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -249,8 +245,8 @@ def main():
 
     peaks = load_peaks()
     ms_step = ms_dev / args.steps
-    fps = world * args.steps / (ms_dev / 1e3)
-    fps_e2e = world * args.steps / (ms_e2e / 1e3)
+    fps = replicas.whole_job_throughput(args.steps, ms_dev)
+    fps_e2e = replicas.whole_job_throughput(args.steps, ms_e2e)
     gemm_classes = ["gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm"]
     gemm_ms = sum(prof[k][0] for k in gemm_classes) / n_prof
     gemm_n = sum(prof[k][1] for k in gemm_classes) / n_prof
