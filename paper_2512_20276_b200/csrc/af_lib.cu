@@ -136,14 +136,14 @@ static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
 
 // Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
 struct OutView { void* ptr; int elem_bytes; /* 4 = fp32, 2 = bf16, -2 = fp16 */ int features, n_mid, tokens; long long ld_mid, ld_tok; int box_feat; };
-static int get_out_map(const OutView& o, CUtensorMap* out) {
+static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
   const unsigned long long dims[3] = {static_cast<unsigned long long>(o.features), static_cast<unsigned long long>(o.n_mid),
                                       static_cast<unsigned long long>(o.tokens)};
   const int eb = o.elem_bytes < 0 ? -o.elem_bytes : o.elem_bytes;
   const unsigned long long strides[2] = {static_cast<unsigned long long>(o.ld_mid) * eb,
                                          static_cast<unsigned long long>(o.ld_tok) * eb};
   const int et = o.elem_bytes;
-  const unsigned box[3] = {static_cast<unsigned>(o.box_feat), 1u, 32u};
+  const unsigned box[3] = {static_cast<unsigned>(o.box_feat), 1u, (o.elem_bytes == 4 && stg_bytes < 4096) ? 16u : 32u};
   return get_map_nd(o.ptr, et, 3, dims, strides, box, false, out);
 }
 
@@ -152,6 +152,7 @@ static int get_out_map(const OutView& o, CUtensorMap* out) {
 // allocation, tensor-map prefetch, the first weight tiles) overlaps the previous kernel's tail, and each kernel
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
 static bool g_use_pdl = true;
+static int g_small_staging = 1;  // AF_SMALL_STAGING=0: always two 4 KB staging buffers per epilogue warp
 static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
 static int g_launch_cluster = 1;  // cluster size of the next launch_k call (set by launch_gemm, reset after the launch)
 template <typename... KArgs, typename... Args>
@@ -189,12 +190,13 @@ static int gemm_global_init() {
   if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
   g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
   if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
+  if (const char* e = getenv("AF_SMALL_STAGING")) g_small_staging = atoi(e) != 0;
   if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
   CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
-  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 128 * 2));
-  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * ATT_BQ * 64 * 2));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   return AF_OK;
 }
 
@@ -222,8 +224,9 @@ extern "C" int af_debug_trace_read(long long* out, int* meta) {
   return g_trace_n;
 }
 
-// threads of the one-block-per-row kernels: one 16-byte access per thread where the row allows it
-static int row_threads_for(int D) { int t = (D / 4 + 31) / 32 * 32; return t < 64 ? 64 : (t > 1024 ? 1024 : t); }
+// threads of the one-block-per-row kernels: two 16-byte accesses per thread and <= 512 threads, so that two blocks fit
+// an SM and the ~282 rows of a step run as one wave
+static int row_threads_for(int D) { int t = (D / 8 + 31) / 32 * 32; return t < 64 ? 64 : (t > 512 ? 512 : t); }
 
 // split-K pieces per tile of the O / down projections (also the number of slabs the next residual kernel adds)
 static int gemm_split_count(int n_tiles, int K) {
@@ -275,7 +278,15 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
       p.splits = 1;
     }
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + n_pad * GEMM_BK * 2;
-    int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_XCH_BYTES) / stage_bytes;
+    // epilogue staging: two 4 KB buffers per warp, or one 2 KB buffer when that buys a pipeline stage (the main loop
+    // is bound by TMA latency x stages in flight)
+    p.stg_bytes = 4096; p.stg_bufs = 2;
+    int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs) / stage_bytes;
+    if (g_small_staging && stages < 6) {
+      const int st2 = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * 2048) / stage_bytes;
+      if (st2 > stages) { stages = st2; p.stg_bytes = 2048; p.stg_bufs = 1; }
+    }
+    const int xch_bytes = GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs;
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
     if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
     p.stages = stages; p.flags = g_flags;
@@ -291,14 +302,14 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     if (rc) return rc;
     CUtensorMap mo, mp;
     p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
-    if ((rc = get_out_map(ov, &mo))) return rc;
+    if ((rc = get_out_map(ov, p.stg_bytes, &mo))) return rc;
     {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
       const unsigned long long strides[2] = {GEMM_BM * 4ull, GEMM_BM * 4ull * GEMM_MAX_TOK};
-      const unsigned box[3] = {32u, 32u, 1u};
+      const unsigned box[3] = {32u, p.stg_bytes < 4096 ? 16u : 32u, 1u};
       if ((rc = get_map_nd(p.partial, 4, 3, dims, strides, box, false, &mp))) return rc;
     }
-    const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_XCH_BYTES + 1024;
+    const size_t smem = static_cast<size_t>(stages) * stage_bytes + xch_bytes + 1024;
     {
       ProfScope ps(cat, st);
       g_launch_cluster = p.cluster;
@@ -591,11 +602,11 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a4: segment-masked causal attention over the ring
     if (hd == 128)
       AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(n_items, H), dim3(ATT_THREADS),
-                5 * ATT_BQ * 128 * 2, st, static_cast<const act_t*>(ws.q_rot),
+                att_smem_bytes(128), st, static_cast<const act_t*>(ws.q_rot),
                 static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     else
       AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(n_items, H), dim3(ATT_THREADS),
-                5 * ATT_BQ * 64 * 2, st, static_cast<const act_t*>(ws.q_rot),
+                att_smem_bytes(64), st, static_cast<const act_t*>(ws.q_rot),
                 static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     // a5: O projection, split-K slabs (added to the residual by the next kernel)
     {

@@ -10,7 +10,9 @@
 namespace af {
 
 constexpr int ATT_BQ = 64;
-constexpr int ATT_BKV = 64;
+constexpr int ATT_BKV = 32;
+constexpr int ATT_STAGES = 3;   // K/V tiles in flight (cp.async groups)
+constexpr int att_smem_bytes(int hd) { return (ATT_BQ + 2 * ATT_STAGES * ATT_BKV) * hd * 2; }
 constexpr int ATT_THREADS = 128;
 
 struct StepTables {      // device arrays written by rowmap_kernel (elementwise.cuh), one set per ring
@@ -60,7 +62,7 @@ __device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
 }
 
 template <int HD>
-__global__ void __launch_bounds__(ATT_THREADS)
+__global__ void __launch_bounds__(ATT_THREADS, 3)
 attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
                  const act_t* __restrict__ kv,    // ring, layer base: [2][R][H][C][HD]
                  act_t* __restrict__ out,         // [T, H*HD]
@@ -69,12 +71,12 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   constexpr int TILE_BYTES = ATT_BKV * HD * 2;
   extern __shared__ __align__(128) uint8_t att_smem[];
   uint8_t* sQ = att_smem;
-  uint8_t* sK = sQ + ATT_BQ * HD * 2;         // 2 stages
-  uint8_t* sV = sK + 2 * TILE_BYTES;          // 2 stages
+  uint8_t* sK = sQ + ATT_BQ * HD * 2;               // ATT_STAGES stages
+  uint8_t* sV = sK + ATT_STAGES * TILE_BYTES;       // ATT_STAGES stages
 
   pdl_wait();
   pdl_launch_dependents();
-  const int item = blockIdx.x, h = blockIdx.y;
+  const int item = static_cast<int>(gridDim.x) - 1 - blockIdx.x, h = blockIdx.y;  // late items see the longest ranges: first
   const int seg = tb.item_seg[item], q0 = tb.item_q0[item];
   const int req = tb.seg_req[seg], start = tb.seg_start[seg], len = tb.seg_len[seg];
   const int row0 = tb.seg_row0[seg], base = tb.seg_base[seg];
@@ -110,6 +112,8 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   };
   load_kv(0, 0);
   cp_async_commit();
+  if (n_tiles > 1) load_kv(1, 1);
+  cp_async_commit();
 
   float o_acc[HD / 8][4];
 #pragma unroll
@@ -122,10 +126,10 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   const int warp_pmax = start + q0 + warp * 16 + 15;
 
   for (int tile = 0; tile < n_tiles; ++tile) {
-    const int stage = tile & 1;
-    if (tile + 1 < n_tiles) load_kv(tile + 1, stage ^ 1);
+    const int stage = tile % ATT_STAGES;
+    if (tile + 2 < n_tiles) load_kv(tile + 2, (tile + 2) % ATT_STAGES);   // its stage was released at the end of tile - 1
     cp_async_commit();
-    cp_async_wait<1>();
+    cp_async_wait<2>();
     __syncthreads();
     if (tile == 0) {
 #pragma unroll

@@ -84,6 +84,7 @@ __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const f
   __shared__ float red[32];
   float* xr = x + static_cast<size_t>(src) * D;
   float ss = 0.f;
+#pragma unroll 2
   for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
     float4 v = *reinterpret_cast<const float4*>(xr + c);
     if (n_parts > 0) {
@@ -112,7 +113,7 @@ __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const f
   }
 }
 
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(512, 2)
 residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int n_parts, long long part_stride,
                      const __nv_bfloat16* __restrict__ g, act_t* __restrict__ y, int D, float eps) {
   pdl_wait();
@@ -123,7 +124,7 @@ residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int
 struct RowListArg { int rows[256]; };  // a10: the caller's row list, passed by value (no staging copy)
 
 // a10: y[i,:] = fp16( RMSNorm(hidden[rows[i],:]; g_final) ), the input of the LM-head GEMM
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(512, 2)
 gather_norm_kernel(const RowListArg rl, const float* __restrict__ x, const __nv_bfloat16* __restrict__ g,
                    act_t* __restrict__ y, int D, float eps) {
   pdl_wait();
@@ -134,7 +135,7 @@ gather_norm_kernel(const RowListArg rl, const float* __restrict__ x, const __nv_
 // a3 FusedRoPEAndWriteKV (Alg. 2 l.3): rotate q and k of every (row, head) at the row's logical
 // position in its own request (rotate-half pairing, table built in fp64), write q to the query buffer and
 // k (rotated), v straight to the row's ring slot.  One block per row, 8 elements (16 bytes) per thread-iteration.
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(512, 2)
 rope_append_kernel(const act_t* __restrict__ qkv,   // [T, 3*H*hd]  (q | k | v)
                    act_t* __restrict__ q_out,       // [T, H*hd]
                    act_t* __restrict__ kv_layer,    // [2][R][H][C][hd]

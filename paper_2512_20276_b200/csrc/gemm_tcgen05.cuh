@@ -38,7 +38,7 @@ constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
-constexpr int GEMM_XCH_BYTES = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB staging buffers for the TMA stores
+constexpr int GEMM_XCH_MAX = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB (or one 2 KB) staging buffers for TMA stores
 constexpr int GEMM_SMEM_BUDGET = 232448 - 1024;    // dynamic shared memory: 227 KB minus the static part
 
 enum GemmEpilogue : int { EPI_STORE = 0, EPI_SWIGLU = 1 };
@@ -62,6 +62,7 @@ struct GemmParams {
   int splits;          // SPLIT_K: pieces per tile
   int total_units, units_per_cta;  // SPLIT_STREAMK
   int stages;
+  int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile
   int out_bf16;        // EPI_STORE: 0 = fp32 output, 1 = bf16, 2 = fp16 (box 32 features x 32 tokens)

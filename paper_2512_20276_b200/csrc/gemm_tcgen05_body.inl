@@ -187,16 +187,18 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     const int quad = warp & 3, par = warp >> 2;
     const int row = quad * 32 + lane;
     const int etid = threadIdx.x;  // 0..255
-    uint8_t* stg_base = reinterpret_cast<uint8_t*>(xch) + warp * 8192;
+    uint8_t* stg_base = reinterpret_cast<uint8_t*>(xch) + warp * (p.stg_bytes * p.stg_bufs);
     uint32_t n_st = 0;  // TMA stores issued by this warp; buffer = n_st & 1
     bool store_ok = true;
-#define stg (stg_base + (n_st & 1) * 4096)
+#define stg (stg_base + (p.stg_bufs > 1 ? (n_st & 1) * p.stg_bytes : 0))
     long long tk[6] = {0, 0, 0, 0, 0, 0};
     long long tk0 = 0;
 #define AF_TICK(i) do { if (trace) { const long long t_ = clock64(); tk[i] += t_ - tk0; tk0 = t_; } } while (0)
     auto stage_free = [&]() {  // the TMA stores issued by this warp have finished reading the staging buffer
       AF_TICK(2);
-      if (lane == 0) bulk_wait_read<1>();  // all but the latest store (which reads the other buffer) are done reading
+      if (lane == 0) {  // all stores but the latest (which reads the other buffer, if there are two) are done reading
+        if (p.stg_bufs > 1) bulk_wait_read<1>(); else bulk_wait_read<0>();
+      }
       __syncwarp();
       AF_TICK(3);
     };
@@ -330,13 +332,28 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       };
       auto finish_chunk = [&](int c0, int cw, float* v) {
         if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
-          // fp32, one 32-token box: stream-K partial [cta][token][128 features] or the fp32 output
-          stage_free();
-          float* sb = reinterpret_cast<float*>(stg);
+          // fp32: stream-K partial [cta][token][128 features] or the fp32 output, one 32-token box per chunk (4 KB
+          // staging buffers) or two 16-token boxes (2 KB)
+          if (p.stg_bytes >= 4096) {
+            stage_free();
+            float* sb = reinterpret_cast<float*>(stg);
 #pragma unroll
-          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
-          if (contributor) stage_store(&map_part, quad * 32, c0, cta);
-          else stage_store(&map_out, f0, mid, p.tok0 + c0);
+            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
+            if (contributor) stage_store(&map_part, quad * 32, c0, cta);
+            else stage_store(&map_out, f0, mid, p.tok0 + c0);
+          } else {
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+              if (hh * 16 < cw) {
+                stage_free();
+                float* sb = reinterpret_cast<float*>(stg);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = v[hh * 16 + j];
+                if (contributor) stage_store(&map_part, quad * 32, c0 + hh * 16, cta);
+                else stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 16);
+              }
+            }
+          }
         } else if (p.epi == EPI_STORE) {  // bf16 or fp16, one 32-token box
           stage_free();
           uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
