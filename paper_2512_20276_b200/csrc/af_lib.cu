@@ -153,6 +153,7 @@ static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
 static bool g_use_pdl = true;
 static int g_small_staging = 1;  // AF_SMALL_STAGING=0: always two 4 KB staging buffers per epilogue warp
+static int g_gemm_mma2 = 1;      // AF_MMA2=0: keep cta_group::1 MMAs (with multicast) in the 2-CTA clusters
 static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
 static int g_launch_cluster = 1;  // cluster size of the next launch_k call (set by launch_gemm, reset after the launch)
 template <typename... KArgs, typename... Args>
@@ -191,10 +192,12 @@ static int gemm_global_init() {
   g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
   if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
   if (const char* e = getenv("AF_SMALL_STAGING")) g_small_staging = atoi(e) != 0;
+  if (const char* e = getenv("AF_MMA2")) g_gemm_mma2 = atoi(e) != 0;
   if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
   CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   return AF_OK;
@@ -277,7 +280,8 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
       grid = n_cl * p.cluster;
       p.splits = 1;
     }
-    const int stage_bytes = GEMM_BM * GEMM_BK * 2 + n_pad * GEMM_BK * 2;
+    p.mma2 = (g_gemm_mma2 && p.cluster == 2 && p.w_fp16) ? 1 : 0;
+    const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (p.mma2 ? n_pad / 2 : n_pad) * GEMM_BK * 2;
     // epilogue staging: two 4 KB buffers per warp, or one 2 KB buffer when that buys a pipeline stage (the main loop
     // is bound by TMA latency x stages in flight)
     p.stg_bytes = 4096; p.stg_bufs = 2;
@@ -298,7 +302,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
       rc = get_map(w[i < n_w ? i : 0], p.part_rows, p.K, box_rows, &mw[i]);
       if (rc) return rc;
     }
-    rc = get_map(x, x_rows_cap, p.K, p.xh, &mx);
+    rc = get_map(x, x_rows_cap, p.K, p.mma2 ? p.n1 / 2 : p.xh, &mx);
     if (rc) return rc;
     CUtensorMap mo, mp;
     p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
@@ -313,7 +317,8 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     {
       ProfScope ps(cat, st);
       g_launch_cluster = p.cluster;
-      cudaError_t e = launch_k(gemm_tcgen05_kernel, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
+      cudaError_t e = p.mma2 ? launch_k(gemm_tcgen05_kernel<true>, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p)
+                             : launch_k(gemm_tcgen05_kernel<false>, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
       g_launch_cluster = 1;
       if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gemm_tcgen05_kernel failed: %s", cudaGetErrorString(e));
     }

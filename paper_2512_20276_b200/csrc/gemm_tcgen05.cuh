@@ -57,7 +57,8 @@ struct GemmParams {
   int n1, n2;          // UMMA N of the two token halves (multiples of 16, n2 may be 0)
   int xh;              // token rows per activation TMA box (two boxes per k-block): n1 if n2 > 0, else n1 / 2
   int n_tiles;         // weight tiles in all
-  int cluster;         // CTAs per cluster: 1, or 2 (activation boxes multicast, work units = tile pairs)
+  int cluster;         // CTAs per cluster: 1, or 2 (work units = tile pairs; activation boxes multicast, or mma2)
+  int mma2;            // 1 (needs cluster == 2, w_fp16): tcgen05.mma.cta_group::2 over the pair, activation rows split
   int split;           // GemmSplit
   int splits;          // SPLIT_K: pieces per tile
   int total_units, units_per_cta;  // SPLIT_STREAMK

@@ -1,5 +1,6 @@
 // Body of gemm_tcgen05.cuh (kept in a second file only to keep each file short); see the header for the design.
 
+template <bool kMma2>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_constant__ CUtensorMap map_w1,
                     const __grid_constant__ CUtensorMap map_w2, const __grid_constant__ CUtensorMap map_x,
@@ -11,7 +12,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   uint8_t* tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   const int n_pad = p.n1 + p.n2;
   const uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
-  const uint32_t b_bytes = static_cast<uint32_t>(n_pad) * GEMM_BK * 2;
+  // mma2: one tcgen05.mma.cta_group::2 per CTA pair (M = 256 = the two CTAs' weight tiles); each CTA stages only HALF
+  // of the activation rows of every UMMA-N half, so a stage is 34 KB instead of 52 KB at T = 282
+  constexpr bool mma2 = kMma2;  // (a second instantiation: a kernel holding cta_group::2 instructions must be launched in clusters)
+  const uint32_t b_bytes = static_cast<uint32_t>(mma2 ? n_pad / 2 : n_pad) * GEMM_BK * 2;
   const uint32_t stage_bytes = a_bytes + b_bytes;
   float* xch = reinterpret_cast<float*>(tiles + static_cast<size_t>(p.stages) * stage_bytes);
 
@@ -40,14 +44,16 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     for (int s = 0; s < p.stages; ++s) {
       mbar_init(&full_bar[s], 1);
       mbar_init(&conv_bar[s], GEMM_EPI_WARPS);
-      mbar_init(&empty_bar[s], p.cluster);
+      mbar_init(&empty_bar[s], mma2 ? 1 : p.cluster);
     }
     mbar_init(&tmem_full_bar, 1);
-    mbar_init(&tmem_empty_bar, GEMM_EPI_WARPS);
+    mbar_init(&tmem_empty_bar, mma2 ? 2 * GEMM_EPI_WARPS : GEMM_EPI_WARPS);  // mma2: the leader waits for both drains
     mbar_init(&fix_bar, 1);
     fence_barrier_init();
   }
-  if (warp == GEMM_EPI_WARPS + 1) tmem_alloc(&tmem_base_smem, GEMM_TMEM_COLS);
+  if (warp == GEMM_EPI_WARPS + 1) {
+    if (mma2) tmem_alloc_cg2(&tmem_base_smem, GEMM_TMEM_COLS); else tmem_alloc(&tmem_base_smem, GEMM_TMEM_COLS);
+  }
   tc_fence_before();
   __syncthreads();
   if (p.cluster > 1) cluster_sync();  // the peer's barriers exist before anything is multicast to them
@@ -70,28 +76,54 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     if (lane == 0) {
       const uint64_t pol_w = policy_evict_first();  // weights are streamed once per step
       const uint64_t pol_x = policy_evict_last();   // the packed activations are re-read by every CTA
-      auto load_w = [&](int u, int stage) {
-        const int kb = u % p.num_kb;
-        const int tile = min((u / p.num_kb) * p.cluster + crank, p.n_tiles - 1);  // (an odd tile count: reload the last)
+      // (pair, kb) of the unit being loaded, advanced incrementally: no division in the steady-state loop
+      int l_pair = u_begin / p.num_kb, l_kb = u_begin - l_pair * p.num_kb;
+      const CUtensorMap* l_mw = &map_w0;
+      int l_row = 0;   // first weight row of this CTA's tile in its matrix
+      auto set_tile = [&]() {
+        const int tile = min(l_pair * p.cluster + crank, p.n_tiles - 1);  // (an odd tile count: reload the last)
+        if (p.a_pair) {
+          l_row = tile * 64;
+        } else {
+          const int part = tile / p.tiles_per_part;
+          l_mw = part == 0 ? &map_w0 : (part == 1 ? &map_w1 : &map_w2);
+          l_row = (tile - part * p.tiles_per_part) * GEMM_BM;
+        }
+      };
+      set_tile();
+      auto advance = [&]() {
+        if (++l_kb == p.num_kb) { l_kb = 0; ++l_pair; set_tile(); }
+      };
+      auto load_w = [&](int stage) {
         uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
+        const int kc = l_kb * GEMM_BK;
         if (p.a_pair) {  // every TMEM lane quadrant = 16 gate rows + the 16 up rows of the same features
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
-            tma_load_2d(sa + q * 4096, &map_w0, &full_bar[stage], kb * GEMM_BK, tile * 64 + q * 16, pol_w);
-            tma_load_2d(sa + q * 4096 + 2048, &map_w1, &full_bar[stage], kb * GEMM_BK, tile * 64 + q * 16, pol_w);
+            if (mma2) {
+              tma_load_2d_cg2(sa + q * 4096, &map_w0, &full_bar[stage], kc, l_row + q * 16, pol_w);
+              tma_load_2d_cg2(sa + q * 4096 + 2048, &map_w1, &full_bar[stage], kc, l_row + q * 16, pol_w);
+            } else {
+              tma_load_2d(sa + q * 4096, &map_w0, &full_bar[stage], kc, l_row + q * 16, pol_w);
+              tma_load_2d(sa + q * 4096 + 2048, &map_w1, &full_bar[stage], kc, l_row + q * 16, pol_w);
+            }
           }
         } else {
-          const int part = tile / p.tiles_per_part, tip = tile - part * p.tiles_per_part;
-          const CUtensorMap* mw = part == 0 ? &map_w0 : (part == 1 ? &map_w1 : &map_w2);
-          tma_load_2d(sa, mw, &full_bar[stage], kb * GEMM_BK, tip * GEMM_BM, pol_w);
+          if (mma2) tma_load_2d_cg2(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
+          else tma_load_2d(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
         }
       };
       // the activation k-block = two boxes of p.xh token rows; in a cluster CTA r loads box r for both CTAs
-      auto load_x = [&](int u, int stage) {
-        const int kb = u % p.num_kb;
+      auto load_x = [&](int kb, int stage) {
         uint8_t* sb = tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes;
         const size_t half = static_cast<size_t>(p.xh) * GEMM_BK * 2;
-        if (p.cluster > 1) {
+        if (mma2) {  // this CTA's half of the rows of each UMMA-N half (the map's box is n1 / 2 rows)
+          const int h1 = p.n1 / 2;
+          tma_load_2d_cg2(sb, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0 + crank * h1, pol_x);
+          if (p.n2 > 0)
+            tma_load_2d_cg2(sb + static_cast<size_t>(h1) * GEMM_BK * 2, &map_x, &full_bar[stage], kb * GEMM_BK,
+                            p.tok0 + p.n1 + crank * h1, pol_x);
+        } else if (p.cluster > 1) {
           tma_load_2d_mc(sb + crank * half, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0 + crank * p.xh, 0x3, pol_x);
         } else {
           tma_load_2d(sb, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0, pol_x);
@@ -100,31 +132,31 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       };
       // The weights do not depend on the previous kernel: start streaming them before the PDL dependency resolves.
       const int n_pre = min(p.stages, u_end - u_begin);
+      const int kb_first = l_kb;
       for (int i = 0; i < n_pre; ++i) {
-        mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
-        load_w(u_begin + i, i);
+        if (!mma2) mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
+        else if (crank == 0) mbar_arrive_expect_tx(&full_bar[i], 2 * stage_bytes);
+        load_w(i);
+        advance();
       }
       AF_TRACE(24);
       pdl_wait();
       AF_TRACE(25);
-      for (int i = 0; i < n_pre; ++i) load_x(u_begin + i, i);
+      for (int i = 0, kb = kb_first; i < n_pre; ++i) {
+        load_x(kb, i);
+        if (++kb == p.num_kb) kb = 0;
+      }
       int stage = n_pre == p.stages ? 0 : n_pre;
       uint32_t phase = n_pre == p.stages ? 1 : 0;
       for (int u = u_begin + n_pre; u < u_end; ++u) {
         mbar_wait(&empty_bar[stage], phase ^ 1);
         const int ui = u - u_begin - 8;
         if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[2 + 4 * ui] = clock64();
-        if (p.dbg & 1) {        // experiment: no activation loads after the first round (stale tiles are re-used)
-          mbar_arrive_expect_tx(&full_bar[stage], a_bytes);
-          load_w(u, stage);
-        } else if (p.dbg & 2) { // experiment: no weight loads after the first round
-          mbar_arrive_expect_tx(&full_bar[stage], stage_bytes - a_bytes);
-          load_x(u, stage);
-        } else {
-        mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
-        load_w(u, stage);
-        load_x(u, stage);
-        }
+        if (!mma2) mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
+        else if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
+        load_w(stage);
+        load_x(l_kb, stage);
+        advance();
         if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[3 + 4 * ui] = clock64();
         if (++stage == p.stages) { stage = 0; phase ^= 1; }
       }
@@ -132,9 +164,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     }
   } else if (warp == GEMM_EPI_WARPS + 1) {
     // ================================ MMA issuer (one thread) ================================
-    if (lane == 0) {
-      const uint32_t idesc1 = umma_idesc_bf16(GEMM_BM, p.n1);
-      const uint32_t idesc2 = umma_idesc_bf16(GEMM_BM, p.n2 > 0 ? p.n2 : 16);
+    if (lane == 0 && !(mma2 && crank != 0)) {   // mma2: only the pair's leader issues
+      const uint32_t idesc1 = umma_idesc_bf16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n1);
+      const uint32_t idesc2 = umma_idesc_bf16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n2 > 0 ? p.n2 : 16);
       int stage = 0;
       uint32_t phase = 0, acc_phase = 0;
       int u = u_begin;
@@ -157,21 +189,28 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           const uint32_t sb = sa + a_bytes;
           const uint64_t da = umma_smem_desc_sw128(sa);
           const uint64_t db1 = umma_smem_desc_sw128(sb);
-          const uint64_t db2 = umma_smem_desc_sw128(sb + p.n1 * GEMM_BK * 2);
+          const uint64_t db2 = umma_smem_desc_sw128(sb + (mma2 ? p.n1 / 2 : p.n1) * GEMM_BK * 2);
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k) {
             const uint32_t accum = (kb > kb0 || k > 0) ? 1u : 0u;
             // advancing 16 bf16 = 32 bytes along K inside the swizzle row: +2 in the (addr >> 4) field
+            if (mma2) {
+              umma_f16_cg2(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
+              if (p.n2 > 0) umma_f16_cg2(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
+            } else {
             umma_bf16(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
             if (p.n2 > 0) umma_bf16(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
+            }
           }
           // frees the smem slot when these MMAs have read it (in a cluster: in both CTAs, the peer multicasts into it)
-          if (p.cluster > 1) umma_commit_mc(&empty_bar[stage], 0x3); else umma_commit(&empty_bar[stage]);
+          if (mma2) umma_commit_cg2_mc(&empty_bar[stage], 0x3);
+          else if (p.cluster > 1) umma_commit_mc(&empty_bar[stage], 0x3);
+          else umma_commit(&empty_bar[stage]);
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
           AF_MT(t_issue);
           if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[5 + 4 * ui] = clock64();
         }
-        umma_commit(&tmem_full_bar);  // accumulator complete -> epilogue
+        if (mma2) umma_commit_cg2_mc(&tmem_full_bar, 0x3); else umma_commit(&tmem_full_bar);  // accumulator -> epilogue
         acc_phase ^= 1;
         u += kb1 - kb0;
       }
@@ -409,7 +448,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&tmem_empty_bar);
+      if (lane == 0) { if (mma2) mbar_arrive_leader(&tmem_empty_bar); else mbar_arrive(&tmem_empty_bar); }
       if (contributor) {
         if (lane == 0) { bulk_wait<0>(); fence_proxy_async_all(); }  // this warp's partial stores are complete
         __syncwarp();
@@ -436,6 +475,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   if (p.cluster > 1) cluster_sync();  // no CTA leaves while its peer may still signal its barriers
   if (warp == GEMM_EPI_WARPS + 1) {
     tc_fence_after();
-    tmem_dealloc(tmem_base, GEMM_TMEM_COLS);
+    if (mma2) tmem_dealloc_cg2(tmem_base, GEMM_TMEM_COLS); else tmem_dealloc(tmem_base, GEMM_TMEM_COLS);
   }
 }
