@@ -589,7 +589,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     act_t* kvl = g->kv + layer_elems * l;
     // a8(prev) + a1: x += down partials; xn = RMSNorm(x; g_attn)
     AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
-              static_cast<const float*>(ws.split), prev_splits, split_stride,
+              reinterpret_cast<const act_t*>(ws.split), prev_splits, split_stride,
               reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, D, c.rms_eps);
     // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
     {
@@ -617,14 +617,14 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     {
       GemmParams gp{};
       gp.w_fp16 = wfmt; gp.n_parts = 1; gp.part_rows = D; gp.K = D; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
-      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
+      const OutView ov{ws.split, -2, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wo[3] = {L.wo, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_O, st, gp, ov, ws.attn, ws.max_rows, wo, T))) return rc;
       prev_splits = split_count(d_tiles, D);
     }
     // a5 residual + a6: x += O partials; xn = RMSNorm(x; g_mlp)
     AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
-              static_cast<const float*>(ws.split), prev_splits, split_stride,
+              reinterpret_cast<const act_t*>(ws.split), prev_splits, split_stride,
               reinterpret_cast<const __nv_bfloat16*>(L.g_mlp), ws.xn, D, c.rms_eps);
     // a7: gate/up projection with the fused SiLU*mul epilogue
     {
@@ -639,7 +639,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     {
       GemmParams gp{};
       gp.w_fp16 = wfmt; gp.n_parts = 1; gp.part_rows = D; gp.K = F; gp.split = SPLIT_K; gp.epi = EPI_STORE; gp.partial = ws.partial;
-      const OutView ov{ws.split, 4, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
+      const OutView ov{ws.split, -2, D, GEMM_MAX_SPLITS, T, split_stride, D, 32};
       const void* wd[3] = {L.w_down, nullptr, nullptr};
       if ((rc = launch_gemm(PC_GEMM_DOWN, st, gp, ov, ws.h, ws.max_rows, wd, T))) return rc;
       prev_splits = split_count(d_tiles, F);
@@ -647,7 +647,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   }
   // a8 of the last layer: x += down partials (no norm: hidden_out is the pre-final-norm residual stream)
   AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
-            static_cast<const float*>(ws.split), prev_splits, split_stride, static_cast<const __nv_bfloat16*>(nullptr),
+            reinterpret_cast<const act_t*>(ws.split), prev_splits, split_stride, static_cast<const __nv_bfloat16*>(nullptr),
             static_cast<act_t*>(nullptr), D, c.rms_eps);
 #undef AF_LAUNCH
   // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----

@@ -76,9 +76,10 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 }
 
 // a5/a8 residual + a1/a6 RMSNorm in one pass (and a10's norm when rows != nullptr), one block per row:
-//   x[i,:] += sum_s parts[s][i,:]      the split-K partials of the preceding O / down projection, in split order
+//   x[i,:] += sum_s parts[s][i,:]      the split-K partials (fp16 slabs, summed in fp32) of the preceding O / down
+//                                      projection, in split order
 //   y[i,:]  = fp16( x[src,:] * g / sqrt(mean(x^2) + eps) )          (skipped when g == nullptr: reduce only)
-__device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const float* __restrict__ parts, int n_parts,
+__device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const act_t* __restrict__ parts, int n_parts,
                                                   long long part_stride, const __nv_bfloat16* __restrict__ g,
                                                   act_t* __restrict__ y, int i, int src, int D, float eps) {
   __shared__ float red[32];
@@ -88,10 +89,12 @@ __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const f
   for (int c = threadIdx.x * 4; c < D; c += blockDim.x * 4) {
     float4 v = *reinterpret_cast<const float4*>(xr + c);
     if (n_parts > 0) {
-      const float* pr = parts + static_cast<size_t>(src) * D + c;
+      const act_t* pr = parts + static_cast<size_t>(src) * D + c;
       for (int s = 0; s < n_parts; ++s) {
-        const float4 a = __ldcg(reinterpret_cast<const float4*>(pr + s * part_stride));
-        v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
+        const uint2 raw = __ldcg(reinterpret_cast<const uint2*>(pr + s * part_stride));
+        const float2 a0 = __half22float2(*reinterpret_cast<const __half2*>(&raw.x));
+        const float2 a1 = __half22float2(*reinterpret_cast<const __half2*>(&raw.y));
+        v.x += a0.x; v.y += a0.y; v.z += a1.x; v.w += a1.y;
       }
       *reinterpret_cast<float4*>(xr + c) = v;
     }
@@ -114,7 +117,7 @@ __device__ __forceinline__ void residual_norm_row(float* __restrict__ x, const f
 }
 
 __global__ void __launch_bounds__(512, 2)
-residual_norm_kernel(float* __restrict__ x, const float* __restrict__ parts, int n_parts, long long part_stride,
+residual_norm_kernel(float* __restrict__ x, const act_t* __restrict__ parts, int n_parts, long long part_stride,
                      const __nv_bfloat16* __restrict__ g, act_t* __restrict__ y, int D, float eps) {
   pdl_wait();
   pdl_launch_dependents();
