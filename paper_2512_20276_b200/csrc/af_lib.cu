@@ -309,9 +309,10 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     if ((rc = get_out_map(ov, p.stg_bytes, &mo))) return rc;
     {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
-      const unsigned long long strides[2] = {GEMM_BM * 4ull, GEMM_BM * 4ull * GEMM_MAX_TOK};
-      const unsigned box[3] = {32u, p.stg_bytes < 4096 ? 16u : 32u, 1u};
-      if ((rc = get_map_nd(p.partial, 4, 3, dims, strides, box, false, &mp))) return rc;
+      const unsigned long long pe = p.part_f16 ? 2 : 4;
+      const unsigned long long strides[2] = {GEMM_BM * pe, GEMM_BM * pe * GEMM_MAX_TOK};
+      const unsigned box[3] = {32u, (!p.part_f16 && p.stg_bytes < 4096) ? 16u : 32u, 1u};
+      if ((rc = get_map_nd(p.partial, p.part_f16 ? -2 : 4, 3, dims, strides, box, false, &mp))) return rc;
     }
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + xch_bytes + 1024;
     {
@@ -594,7 +595,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
     {
       GemmParams gp{};
-      gp.w_fp16 = wfmt; gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
+      gp.part_f16 = 1; gp.w_fp16 = wfmt; gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
       gp.partial = ws.partial;
       const OutView ov{ws.qkv, -2, D, 3, T, D, 3LL * D, 32};
       const void* wqkv[3] = {L.wq, L.wk, L.wv};
@@ -629,7 +630,7 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a7: gate/up projection with the fused SiLU*mul epilogue
     {
       GemmParams gp{};
-      gp.w_fp16 = wfmt; gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
+      gp.part_f16 = 1; gp.w_fp16 = wfmt; gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
       gp.partial = ws.partial;
       const OutView ov{ws.h, -2, F, 1, T, F, F, 16};
       const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
@@ -696,7 +697,7 @@ extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_
   if (ws_bytes < gemm_partial_bytes()) return fail(AF_ERR_WORKSPACE, "workspace < %zu bytes", gemm_partial_bytes());
   GemmParams gp{};
   gp.n_parts = 1; gp.part_rows = n_out; gp.K = k; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
-  gp.partial = reinterpret_cast<float*>(workspace);
+  gp.partial = workspace;
   if (n_out % 4) return fail(AF_ERR_ARG, "n_out must be a multiple of 4");
   const OutView ov{out, 4, n_out, 1, n_tok, n_out, n_out, 32};
   const void* wl[3] = {wmat, nullptr, nullptr};

@@ -67,7 +67,8 @@ struct GemmParams {
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile
   int out_bf16;        // EPI_STORE: 0 = fp32 output, 1 = bf16, 2 = fp16 (box 32 features x 32 tokens)
-  float* partial;      // [grid][288][128] fp32 stream-K partials (written through map_part)
+  void* partial;       // [grid][288][128] stream-K partials, fp32 or (part_f16) fp16, written through map_part
+  int part_f16;
   int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
   int dbg;
   long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr

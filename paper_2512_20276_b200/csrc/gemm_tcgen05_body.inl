@@ -318,26 +318,29 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 64-column blocks
       int blk_cols = n_pad, grp = n_contrib, n_groups = n_contrib > 0 ? 1 : 0;
       if (n_contrib > 0) {
-        const int grp_max = stage_area / (64 * GEMM_BM * 4);
+        const int pe = p.part_f16 ? 2 : 4;   // bytes per partial element
+        const int grp_max = stage_area / (64 * GEMM_BM * pe);
         if (n_contrib > grp_max) {
           grp = grp_max; blk_cols = 64; n_groups = (n_contrib + grp - 1) / grp;
         } else {
-          blk_cols = (stage_area / (n_contrib * GEMM_BM * 4)) / 64 * 64;
+          blk_cols = (stage_area / (n_contrib * GEMM_BM * pe)) / 64 * 64;
           if (blk_cols > n_pad) blk_cols = n_pad;
         }
       }
-      const float* fix = reinterpret_cast<const float*>(tiles);
+      const uint8_t* fix = tiles;
       bool fix_used = false;
       auto load_group = [&](int g0, int cnt, int b0, int b1) {
         if (fix_used) AF_EPI_BAR();  // everyone is done reading what the buffer held
         fix_used = true;
         if (etid == 0) {
-          const uint32_t bytes = static_cast<uint32_t>(b1 - b0) * GEMM_BM * 4;
+          const uint32_t pe = p.part_f16 ? 2 : 4;
+          const uint32_t bytes = static_cast<uint32_t>(b1 - b0) * GEMM_BM * pe;
           fence_proxy_async_all();
           mbar_arrive_expect_tx(&fix_bar, bytes * cnt);
           for (int c = 0; c < cnt; ++c)
             bulk_load_1d(tiles + static_cast<size_t>(c) * bytes,
-                         p.partial + (static_cast<size_t>((c_first + g0 + c) * p.cluster + crank) * GEMM_MAX_TOK + b0) * GEMM_BM,
+                         reinterpret_cast<const uint8_t*>(p.partial) +
+                             (static_cast<size_t>((c_first + g0 + c) * p.cluster + crank) * GEMM_MAX_TOK + b0) * GEMM_BM * pe,
                          bytes,
                          &fix_bar);
         }
@@ -358,19 +361,32 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       auto add_fix = [&](int cnt, int b0, int b1, int c0, float* v) {
         // (a 16-wide last chunk over-reads 16 columns of the staging area; those columns are never stored)
         for (int c = 0; c < cnt; ++c) {
-          const float* q = fix + (static_cast<size_t>(c) * (b1 - b0) + (c0 - b0)) * GEMM_BM + row;
+          const size_t e0 = (static_cast<size_t>(c) * (b1 - b0) + (c0 - b0)) * GEMM_BM + row;
 #pragma unroll
           for (int h2 = 0; h2 < 2; ++h2) {
             float t[16];
+            if (p.part_f16) {
+              const act_t* q = reinterpret_cast<const act_t*>(fix) + e0;
 #pragma unroll
-            for (int j = 0; j < 16; ++j) t[j] = q[(h2 * 16 + j) * GEMM_BM];
+              for (int j = 0; j < 16; ++j) t[j] = act2f(q[(h2 * 16 + j) * GEMM_BM]);
+            } else {
+              const float* q = reinterpret_cast<const float*>(fix) + e0;
+#pragma unroll
+              for (int j = 0; j < 16; ++j) t[j] = q[(h2 * 16 + j) * GEMM_BM];
+            }
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[h2 * 16 + j] += t[j];
           }
         }
       };
       auto finish_chunk = [&](int c0, int cw, float* v) {
-        if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
+        if (contributor && p.part_f16) {   // fp16 partial [cta][token][128 features], one 32-token box
+          stage_free();
+          uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __half_as_ushort(__float2half_rn(v[j]));
+          stage_store(&map_part, quad * 32, c0, cta);
+        } else if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
           // fp32: stream-K partial [cta][token][128 features] or the fp32 output, one 32-token box per chunk (4 KB
           // staging buffers) or two 16-token boxes (2 KB)
           if (p.stg_bytes >= 4096) {
