@@ -152,7 +152,8 @@ static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
 // allocation, tensor-map prefetch, the first weight tiles) overlaps the previous kernel's tail, and each kernel
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
 static bool g_use_pdl = true;
-static int g_small_staging = 1;  // AF_SMALL_STAGING=0: always two 4 KB staging buffers per epilogue warp
+static int g_staging_first = 0;   // AF_STAGING=0/1/2: first epilogue staging candidate tried (2x4 KB, 2x2 KB, 1x2 KB)
+static int g_min_stages = 5;      // AF_MIN_STAGES: shrink the staging until the ring has this many stages
 static int g_gemm_mma2 = 1;      // AF_MMA2=0: keep cta_group::1 MMAs (with multicast) in the 2-CTA clusters
 static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
 static int g_launch_cluster = 1;  // cluster size of the next launch_k call (set by launch_gemm, reset after the launch)
@@ -191,7 +192,8 @@ static int gemm_global_init() {
   if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
   g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
   if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
-  if (const char* e = getenv("AF_SMALL_STAGING")) g_small_staging = atoi(e) != 0;
+  if (const char* e = getenv("AF_STAGING")) g_staging_first = atoi(e) < 0 ? 0 : (atoi(e) > 2 ? 2 : atoi(e));
+  if (const char* e = getenv("AF_MIN_STAGES")) g_min_stages = atoi(e);
   if (const char* e = getenv("AF_MMA2")) g_gemm_mma2 = atoi(e) != 0;
   if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
@@ -258,7 +260,8 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     int n_pad = (Tc + 15) / 16 * 16;
     if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
     else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
-    const int box_rows = p.a_pair ? 16 : GEMM_BM;
+    { const char* d = getenv("AF_DBG"); p.dbg = d ? atoi(d) : 0; }
+    const int box_rows = (p.a_pair || (p.dbg & 32)) ? 16 : GEMM_BM;
     const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
     p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
@@ -284,11 +287,13 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (p.mma2 ? n_pad / 2 : n_pad) * GEMM_BK * 2;
     // epilogue staging: two 4 KB buffers per warp, or one 2 KB buffer when that buys a pipeline stage (the main loop
     // is bound by TMA latency x stages in flight)
-    p.stg_bytes = 4096; p.stg_bufs = 2;
-    int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs) / stage_bytes;
-    if (g_small_staging && stages < 6) {
-      const int st2 = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * 2048) / stage_bytes;
-      if (st2 > stages) { stages = st2; p.stg_bytes = 2048; p.stg_bufs = 1; }
+    // candidates, largest staging first; a smaller one is taken when it buys a pipeline stage (the main loop needs
+    // ~160 KB of loads in flight), down to one 2 KB buffer per warp
+    const int cand[3][2] = {{4096, 2}, {2048, 2}, {2048, 1}};
+    int stages = 0;
+    for (int i = g_staging_first; i < 3; ++i) {
+      const int st_i = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * cand[i][0] * cand[i][1]) / stage_bytes;
+      if (st_i > stages && (stages < g_min_stages || i == g_staging_first)) { stages = st_i; p.stg_bytes = cand[i][0]; p.stg_bufs = cand[i][1]; }
     }
     const int xch_bytes = GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs;
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;

@@ -109,6 +109,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
             }
           }
         } else {
+          if (mma2 && (p.dbg & 32)) {   // experiment: the same tile as 8 boxes of 16 rows (needs a 16-row map: a_pair GEMMs only)
+            for (int q = 0; q < 8; ++q) tma_load_2d_cg2(sa + q * 2048, l_mw, &full_bar[stage], kc, l_row + q * 16, pol_w);
+          } else
           if (mma2) tma_load_2d_cg2(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
           else tma_load_2d(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
         }
