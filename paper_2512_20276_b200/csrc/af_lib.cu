@@ -243,6 +243,44 @@ static int gemm_split_count(int n_tiles, int K) {
   return s < 1 ? 1 : s;
 }
 
+// Stream-K ranges: contiguous unit ranges of equal COST, where a range pays its k-blocks plus a charge for every tile
+// it touches (the accumulator drain stalls the MMA; a tile entered in its middle is a contributor piece, cheaper than
+// an owner / whole tile).  Charges are in k-block units (~0.43 us each at T = 282), from the kernel's timeline.
+// Returns the number of ranges used (<= n_max) and fills ub[0..n].
+static int streamk_partition(int total, int nkb, int n_max, int* ub) {
+  // Ranges shorter than a tile would create pieces in the middle of a tile, which finish last and stall their owner:
+  // there the plain uniform split (every tail piece is the first piece of its range) is the better one.
+  if (total / n_max < nkb) {
+    const int upc = (total + n_max - 1) / n_max, n = (total + upc - 1) / upc;
+    for (int i = 0; i <= n; ++i) ub[i] = i * upc < total ? i * upc : total;
+    return n;
+  }
+  const int kTail = 12, kHead = 20;
+  auto fill = [&](int cap, int* out) {   // greedy: every range takes as much as `cap` allows; returns ranges used
+    int u = 0, n = 0;
+    while (u < total) {
+      if (n == n_max) return n_max + 1;
+      if (out) out[n] = u;
+      int cost = 0, e = u;
+      while (e < total) {
+        const int tile_end = (e / nkb + 1) * nkb;
+        const int room = cap - cost - (e % nkb ? kTail : kHead);
+        int take = tile_end - e < room ? tile_end - e : room;
+        if (take <= 0) { if (e == u) take = 1; else break; }
+        cost += (e % nkb ? kTail : kHead) + take;
+        e += take;
+        if (e < tile_end) break;
+      }
+      u = e; ++n;
+    }
+    if (out) out[n] = total;
+    return n;
+  };
+  int lo = total / n_max, hi = total / n_max + 3 * kHead + nkb;   // smallest cap that fits n_max ranges
+  while (lo < hi) { const int mid = (lo + hi) / 2; if (fill(mid, nullptr) <= n_max) hi = mid; else lo = mid + 1; }
+  return fill(lo, ub);
+}
+
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
 // One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
@@ -260,8 +298,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     int n_pad = (Tc + 15) / 16 * 16;
     if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
     else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
-    { const char* d = getenv("AF_DBG"); p.dbg = d ? atoi(d) : 0; }
-    const int box_rows = (p.a_pair || (p.dbg & 32)) ? 16 : GEMM_BM;
+    const int box_rows = p.a_pair ? 16 : GEMM_BM;
     const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
     p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
@@ -274,12 +311,9 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     int grid;
     if (p.split == SPLIT_K) {
       p.splits = gemm_split_count(n_tiles, p.K);
-      p.units_per_cta = 0;
       grid = n_pairs * p.splits * p.cluster;
     } else {
-      int n_cl = p.total_units < max_cl ? p.total_units : max_cl;
-      p.units_per_cta = (p.total_units + n_cl - 1) / n_cl;
-      n_cl = (p.total_units + p.units_per_cta - 1) / p.units_per_cta;
+      const int n_cl = streamk_partition(p.total_units, p.num_kb, p.total_units < max_cl ? p.total_units : max_cl, p.ub);
       grid = n_cl * p.cluster;
       p.splits = 1;
     }
@@ -299,7 +333,6 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
     if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
     p.stages = stages; p.flags = g_flags;
-    { const char* d = getenv("AF_DBG"); p.dbg = d ? atoi(d) : 0; }
     if (g_trace) { p.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * 32; g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {cat, grid}; ++g_trace_n; }
     CUtensorMap mw[3], mx;
     for (int i = 0; i < 3; ++i) {

@@ -38,6 +38,7 @@ constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
+constexpr int GEMM_MAX_CLUSTERS = 160;  // stream-K ranges (clusters, or CTAs when the cluster size is 1)
 constexpr int GEMM_XCH_MAX = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB (or one 2 KB) staging buffers for TMA stores
 constexpr int GEMM_SMEM_BUDGET = 232448 - 1024;    // dynamic shared memory: 227 KB minus the static part
 
@@ -61,7 +62,8 @@ struct GemmParams {
   int mma2;            // 1 (needs cluster == 2, w_fp16): tcgen05.mma.cta_group::2 over the pair, activation rows split
   int split;           // GemmSplit
   int splits;          // SPLIT_K: pieces per tile
-  int total_units, units_per_cta;  // SPLIT_STREAMK
+  int total_units;     // SPLIT_STREAMK: (tile pair, k-block) units; cluster c owns units [ub[c], ub[c+1])
+  int ub[GEMM_MAX_CLUSTERS + 1];
   int stages;
   int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue
@@ -70,7 +72,6 @@ struct GemmParams {
   void* partial;       // [grid][288][128] stream-K partials, fp32 or (part_f16) fp16, written through map_part
   int part_f16;
   int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
-  int dbg;
   long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr
 };
 

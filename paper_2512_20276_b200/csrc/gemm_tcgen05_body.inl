@@ -67,8 +67,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     u_begin = tile * p.num_kb + static_cast<int>(static_cast<long long>(s) * p.num_kb / p.splits);
     u_end = tile * p.num_kb + static_cast<int>(static_cast<long long>(s + 1) * p.num_kb / p.splits);
   } else {
-    u_begin = min(cl * p.units_per_cta, p.total_units);
-    u_end = min(u_begin + p.units_per_cta, p.total_units);
+    u_begin = p.ub[cl];        // cost-balanced contiguous ranges (units + a charge per tile drain), computed on the host
+    u_end = p.ub[cl + 1];
   }
 
   if (warp == GEMM_EPI_WARPS) {
@@ -109,9 +109,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
             }
           }
         } else {
-          if (mma2 && (p.dbg & 32)) {   // experiment: the same tile as 8 boxes of 16 rows (needs a 16-row map: a_pair GEMMs only)
-            for (int q = 0; q < 8; ++q) tma_load_2d_cg2(sa + q * 2048, l_mw, &full_bar[stage], kc, l_row + q * 16, pol_w);
-          } else
           if (mma2) tma_load_2d_cg2(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
           else tma_load_2d(sa, l_mw, &full_bar[stage], kc, l_row, pol_w);
         }
@@ -153,14 +150,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       uint32_t phase = n_pre == p.stages ? 1 : 0;
       for (int u = u_begin + n_pre; u < u_end; ++u) {
         mbar_wait(&empty_bar[stage], phase ^ 1);
-        const int ui = u - u_begin - 8;
-        if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[2 + 4 * ui] = clock64();
         if (!mma2) mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
         else if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
         load_w(stage);
         load_x(l_kb, stage);
         advance();
-        if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[3 + 4 * ui] = clock64();
         if (++stage == p.stages) { stage = 0; phase ^= 1; }
       }
       AF_TRACE(26);
@@ -173,21 +167,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       int stage = 0;
       uint32_t phase = 0, acc_phase = 0;
       int u = u_begin;
-      long long t_wait = 0, t_issue = 0, t_acc = 0, t_prev = trace ? clock64() : 0;
-#define AF_MT(var) do { if (trace) { const long long t_ = clock64(); var += t_ - t_prev; t_prev = t_; } } while (0)
       while (u < u_end) {
         const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
         const int kb1 = min(p.num_kb, kb0 + (u_end - u));
         mbar_wait(&tmem_empty_bar, acc_phase ^ 1);  // epilogue has drained the accumulator
         tc_fence_after();
-        AF_MT(t_acc);
         for (int kb = kb0; kb < kb1; ++kb) {
           // the stage has landed (and, for bf16 weights, the epilogue warps have rewritten the W tile as fp16)
           mbar_wait(p.w_fp16 ? &full_bar[stage] : &conv_bar[stage], phase);
           tc_fence_after();
-          AF_MT(t_wait);
-          const int ui = u + (kb - kb0) - u_begin - 8;
-          if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[4 + 4 * ui] = clock64();
           const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
           const uint32_t sb = sa + a_bytes;
           const uint64_t da = umma_smem_desc_sw128(sa);
@@ -210,15 +198,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           else if (p.cluster > 1) umma_commit_mc(&empty_bar[stage], 0x3);
           else umma_commit(&empty_bar[stage]);
           if (++stage == p.stages) { stage = 0; phase ^= 1; }
-          AF_MT(t_issue);
-          if (trace && (p.dbg & 8) && ui >= 0 && ui < 4) trace[5 + 4 * ui] = clock64();
         }
         if (mma2) umma_commit_cg2_mc(&tmem_full_bar, 0x3); else umma_commit(&tmem_full_bar);  // accumulator -> epilogue
         acc_phase ^= 1;
         u += kb1 - kb0;
       }
-      if (trace) { trace[28] = t_wait; trace[29] = t_issue; trace[30] = t_acc; trace[31] = u_end - u_begin; }
-#undef AF_MT
     }
   } else {
     // ================================ epilogue warps 0..7 ================================
@@ -233,27 +217,20 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     uint32_t n_st = 0;  // TMA stores issued by this warp; buffer = n_st & 1
     bool store_ok = true;
 #define stg (stg_base + (p.stg_bufs > 1 ? (n_st & 1) * p.stg_bytes : 0))
-    long long tk[6] = {0, 0, 0, 0, 0, 0};
-    long long tk0 = 0;
-#define AF_TICK(i) do { if (trace) { const long long t_ = clock64(); tk[i] += t_ - tk0; tk0 = t_; } } while (0)
     auto stage_free = [&]() {  // the TMA stores issued by this warp have finished reading the staging buffer
-      AF_TICK(2);
       if (lane == 0) {  // all stores but the latest (which reads the other buffer, if there are two) are done reading
         if (p.stg_bufs > 1) bulk_wait_read<1>(); else bulk_wait_read<0>();
       }
       __syncwarp();
-      AF_TICK(3);
     };
     auto stage_store = [&](const CUtensorMap* m, int c0_, int c1_, int c2_) {
       fence_proxy_async();
       __syncwarp();
-      AF_TICK(4);
       if (lane == 0 && store_ok) {
         tma_store_3d(m, stg, c0_, c1_, c2_);
         bulk_commit();
       }
       ++n_st;
-      AF_TICK(5);
     };
     pdl_wait();
     if (etid == 0) AF_TRACE(1);
@@ -292,8 +269,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         // CTAs holding the rest of this tile: cta+1 .. while their range starts before the tile ends
         c_first = cl + 1;   // cluster index; the contributing CTA of cluster c is c * cluster + crank
         const int tile_end = (pair + 1) * p.num_kb;
-        const int c_last = min((tile_end - 1) / p.units_per_cta, static_cast<int>(gridDim.x) / p.cluster - 1);
-        n_contrib = c_last - c_first + 1;
+        const int n_cl = static_cast<int>(gridDim.x) / p.cluster;
+        while (c_first + n_contrib < n_cl && p.ub[c_first + n_contrib] < tile_end) ++n_contrib;
         if (etid < n_contrib) {
           volatile int* f = p.flags + (c_first + etid) * p.cluster + crank;
           while (*f == 0) {
@@ -303,10 +280,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
         AF_EPI_BAR();
       }
-      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(2 + 4 * piece);
+      if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
       mbar_wait(&tmem_full_bar, acc_phase);
       tc_fence_after();
-      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(3 + 4 * piece);
+      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
       store_ok = tile_valid;
       // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
       int f0, mid;
@@ -352,14 +329,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       };
       auto load_acc = [&](int c0, int cw, float* v) {
         uint32_t r[32];
-        if (trace) tk0 = clock64();
         const uint32_t ta = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0;
         tmem_ld16(ta, r);
         if (cw > 16) tmem_ld16(ta + 16, r + 16);
         tmem_ld_wait();
 #pragma unroll
         for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
-        AF_TICK(0);
       };
       auto add_fix = [&](int cnt, int b0, int b1, int c0, float* v) {
         // (a 16-wide last chunk over-reads 16 columns of the staging area; those columns are never stored)
@@ -444,7 +419,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         if (n_groups <= 1) {
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
-            if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(4 + 4 * piece);
+            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
           }
           for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += 64) {
             const int cw = min(32, b1 - c0);
@@ -478,8 +453,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           atomicExch(p.flags + cta, 1);
         }
       }
-      if (etid == 0 && piece < 4 && !(p.dbg & 8)) AF_TRACE(5 + 4 * piece);
-      if (etid == 0 && trace) { for (int i = 0; i < 6; ++i) trace[18 + i] = tk[i]; }
+      if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
       ++piece;
       acc_phase ^= 1;
       u += kb1 - kb0;
