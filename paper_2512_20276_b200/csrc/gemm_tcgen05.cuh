@@ -1,31 +1,38 @@
 // Packed-projection GEMM for sm_100a: out[token, feature] (op)= sum_k X[token, k] * W[feature, k]
-// (steps a2/a3/a5/a7/a8/a10 of SURVEY.md 8(a); Alg. 2 lines 2, 3 and 6).
+// (steps a2/a5/a7/a8/a10 of SURVEY.md 8(a); Alg. 2 lines 2 and 6).  DESIGN.md section 6.1.
 //
-// "Swap-AB" orientation: the WEIGHT tile (128 output features x 64 k) is the UMMA A operand and
-// the packed TOKEN tile (all T <= 288 tokens x 64 k) is the B operand, so the 282-row packed matrix of the paper's
-// schedule maps onto UMMA N = 2 x 144 with 2% padding instead of 3 x 128-row M tiles with 27% padding, and a
-// decode-only step (T <= 16) uses N = 16.  Both operands are K-major in global memory, are staged by TMA with the
-// 128-byte swizzle, and are consumed by tcgen05.mma (kind::f16, bf16 in, fp32 accumulate in TMEM).
+// "Swap-AB" orientation: the WEIGHT tile (128 output features x 64 k) is the UMMA A operand and the packed TOKEN tile
+// (all T <= 288 tokens x 64 k) is the B operand, so the 282-row packed matrix of the paper's schedule maps onto UMMA
+// N = 2 x 144 with 2% padding instead of 3 x 128-row M tiles with 27% padding, and a decode-only step (T <= 16) uses
+// N = 16.  Both operands are K-major in global memory, are staged by TMA with the 128-byte swizzle, and are consumed by
+// tcgen05.mma kind::f16 (fp16 activations x fp16 weights - prepared at load time, or bf16 weights rewritten as fp16 per
+// tile in shared memory - with the fp32 accumulator in TMEM).
+//
+// The grid is launched in 2-CTA clusters whose work unit is (pair of neighbouring weight tiles, k-block):
+//   kMma2 = true   the pair's leader issues tcgen05.mma.cta_group::2 (M = 256); each CTA stages its weight tile and
+//                  half of the activation rows (34 KB per stage at T = 282); the peer's loads complete on the leader's
+//                  mbarrier and the leader's commits are multicast to both CTAs.
+//   kMma2 = false  cta_group::1 MMAs per CTA; the activation boxes are TMA-multicast across the cluster.
 //
 // Work split over a persistent grid (<= 1 CTA per SM), two modes:
-//   SPLIT_STREAMK  the (tile, k-block) units are split evenly and contiguously over the grid.  A CTA that holds a
-//                  k-tail of a tile (always the FIRST piece of its range) writes its fp32 partial to the workspace
+//   SPLIT_STREAMK  contiguous ranges of units per cluster.  A CTA that holds a k-tail of a tile (always the FIRST
+//                  piece of its range) writes its partial (fp16 in the forward, fp32 in af_debug_gemm) to the workspace
 //                  and raises a flag; the CTA that holds the k-head (always the LAST piece of its range, so the
 //                  partials were written long before) pulls them into the freed pipeline stages with bulk copies,
-//                  adds them in CTA order (deterministic) and runs the fused epilogue.
-//   SPLIT_K        every tile is cut into `splits` equal k-ranges, one CTA each; every CTA stores its fp32 partial
-//                  [split][token][feature] and the NEXT kernel (residual + RMSNorm, elementwise.cuh) adds them in
+//                  adds them in CTA order (deterministic) and runs the epilogue.
+//   SPLIT_K        every tile is cut into `splits` equal k-ranges, one CTA each; every CTA stores its partial slab
+//                  [split][token][feature] and the NEXT kernel (residual + RMSNorm, elementwise.cuh) adds the slabs in
 //                  split order.  No CTA ever waits on another.
 //
 // Epilogues (features sit on TMEM lanes, tokens on columns): every warp stages its 32 features x 32 tokens in shared
-// memory and writes them with TMA tensor stores, bf16 or fp32.
+// memory and writes them with TMA tensor stores (fp16, bf16 or fp32).
 //   EPI_STORE      plain store (q|k|v, split-K slabs, logits).
 //   EPI_SWIGLU     tile = 64 gate rows + 64 up rows of the same features, loaded so that every lane quadrant holds
 //                  16 gate + 16 up rows of the same 16 features: the pairing is a warp shuffle, the output is
-//                  bf16(silu(gate) * up).
+//                  fp16(silu(gate) * up).
 //
 // Warp roles (320 threads): warps 0-7 epilogue (TMEM lane quadrant = warp % 4, two warps per quadrant alternate
-// 16-token chunks), warp 8 TMA producer, warp 9 MMA issuer.
+// 32-token chunks; with bf16 weights they also run the per-tile weight transform), warp 8 TMA producer, warp 9 MMA issuer.
 #pragma once
 #include "ptx.cuh"
 
@@ -33,7 +40,7 @@ namespace af {
 
 constexpr int GEMM_BM = 128;       // weight rows (output features) per tile = UMMA M
 constexpr int GEMM_BK = 64;        // bf16 elements per k-block = one 128-byte swizzle row
-constexpr int GEMM_EPI_WARPS = 8;  // two per TMEM lane quadrant (warp % 4), alternating 16-token chunks
+constexpr int GEMM_EPI_WARPS = 8;  // two per TMEM lane quadrant (warp % 4), alternating 32-token chunks
 constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
