@@ -26,7 +26,7 @@ L_P, K_STAGES, R_REGIONS, CAPACITY = 276, 7, 8, 512      # 256 patch + 20 prompt
 SEED = 2
 # DRAM bytes per gemm_tcgen05_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, averaged over the launches of
 # a steady step; cold caches): profiles/launches_r1.md.  Algorithmic weight bytes per launch: 102.8 MB.
-GEMM_TRAFFIC_BYTES_PER_LAUNCH = 109.7e6
+GEMM_TRAFFIC_BYTES_PER_LAUNCH = 107.2e6
 WORKLOAD = "cfg3: 32-layer Llama-2-7B shape, steady pipelined step = 276-row prefill + 6 decodes (ctx 277..282) + LM head on 7 rows"
 
 
