@@ -36,12 +36,25 @@
 #pragma once
 #include "ptx.cuh"
 
+// epilogue warps: 8, 12 or 16 (-DAF_EPI_WARPS=...); 12 and 16 were measured on B200 and are no faster than 8
+#ifndef AF_EPI_WARPS
+#define AF_EPI_WARPS 8
+#endif
+#if AF_EPI_WARPS == 8
+#define AF_EPI_THREADS 256
+#elif AF_EPI_WARPS == 12
+#define AF_EPI_THREADS 384
+#elif AF_EPI_WARPS == 16
+#define AF_EPI_THREADS 512
+#endif
+
 namespace af {
 
 constexpr int GEMM_BM = 128;       // weight rows (output features) per tile = UMMA M
 constexpr int GEMM_BK = 64;        // bf16 elements per k-block = one 128-byte swizzle row
-constexpr int GEMM_EPI_WARPS = 8;  // two per TMEM lane quadrant (warp % 4), alternating 32-token chunks
+constexpr int GEMM_EPI_WARPS = AF_EPI_WARPS;  // two per TMEM lane quadrant (warp % 4), alternating 32-token chunks
 constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
+constexpr int GEMM_BLK = 32 * (GEMM_EPI_WARPS / 4);  // columns one round of the epilogue warps covers
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
@@ -82,7 +95,9 @@ struct GemmParams {
   long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr
 };
 
-#define AF_EPI_BAR() asm volatile("bar.sync 1, 256;\n" ::: "memory")  /* the 8 epilogue warps only */
+#define AF_EPI_BAR_STR2(n) "bar.sync 1, " #n ";\n"
+#define AF_EPI_BAR_STR(n) AF_EPI_BAR_STR2(n)
+#define AF_EPI_BAR() asm volatile(AF_EPI_BAR_STR(AF_EPI_THREADS) ::: "memory")  /* the epilogue warps only */
 
 #include "gemm_tcgen05_body.inl"
 

@@ -253,11 +253,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         mbar_wait(&full_bar[cstage], cphase);
         uint4* wst = reinterpret_cast<uint4*>(tiles + static_cast<size_t>(cstage) * stage_bytes);
 #pragma unroll
-        for (int i = 0; i < static_cast<int>(a_bytes / 16) / (GEMM_EPI_WARPS * 32); ++i) {
-          uint4 raw = wst[etid + i * GEMM_EPI_WARPS * 32];
+        for (int i = etid; i < static_cast<int>(a_bytes / 16); i += GEMM_EPI_WARPS * 32) {
+          uint4 raw = wst[i];
           raw.x = bf16x2_to_f16x2(raw.x); raw.y = bf16x2_to_f16x2(raw.y);
           raw.z = bf16x2_to_f16x2(raw.z); raw.w = bf16x2_to_f16x2(raw.w);
-          wst[etid + i * GEMM_EPI_WARPS * 32] = raw;
+          wst[i] = raw;
         }
         fence_proxy_async();
         __syncwarp();
@@ -299,11 +299,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       int blk_cols = n_pad, grp = n_contrib, n_groups = n_contrib > 0 ? 1 : 0;
       if (n_contrib > 0) {
         const int pe = p.part_f16 ? 2 : 4;   // bytes per partial element
-        const int grp_max = stage_area / (64 * GEMM_BM * pe);
+        const int grp_max = stage_area / (GEMM_BLK * GEMM_BM * pe);
         if (n_contrib > grp_max) {
-          grp = grp_max; blk_cols = 64; n_groups = (n_contrib + grp - 1) / grp;
+          grp = grp_max; blk_cols = GEMM_BLK; n_groups = (n_contrib + grp - 1) / grp;
         } else {
-          blk_cols = (stage_area / (n_contrib * GEMM_BM * pe)) / 64 * 64;
+          blk_cols = (stage_area / (n_contrib * GEMM_BM * pe)) / GEMM_BLK * GEMM_BLK;
           if (blk_cols > n_pad) blk_cols = n_pad;
         }
       }
@@ -421,7 +421,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
             load_group(0, n_contrib, b0, b1);
             if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
           }
-          for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += 64) {
+          for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += GEMM_BLK) {
             const int cw = min(32, b1 - c0);
             load_acc(c0, cw, v);
             if (n_groups == 1) add_fix(n_contrib, b0, b1, c0, v);
