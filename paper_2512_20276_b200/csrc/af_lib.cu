@@ -281,6 +281,75 @@ static int streamk_partition(int total, int nkb, int n_max, int* ub) {
   return fill(lo, ub);
 }
 
+// ------------------------------------------------------------------------------------------------ GEMM schedules
+// Host-built piece lists (GemmPiece, gemm_tcgen05.cuh): which k-blocks of which tile pairs every cluster computes and
+// who reduces what.  Built once per (split mode, tile pairs, k-blocks, clusters) and kept on the device.
+//   SPLIT_K       one PK_PLAIN piece per cluster: slab `mid` of tile pair c / splits.
+//   stream-K      contiguous unit ranges; a range's k-tail piece is its first piece, its k-head piece its last.
+// (Two hand-made schedules for the QKV and gate/up shapes - owners with a single piece plus clusters made of
+//  contributor pieces only - were built on this table and measured no faster than the ranges; removed.)
+struct SchedKey {
+  int split, n_pairs, nkb, max_cl, splits;
+  bool operator<(const SchedKey& o) const { return memcmp(this, &o, sizeof(SchedKey)) < 0; }
+};
+struct Sched { GemmPiece* dev; int n_cl; };
+static std::map<SchedKey, Sched> g_scheds;
+
+static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  const SchedKey key{split, n_pairs, nkb, max_cl, splits};
+  auto it = g_scheds.find(key);
+  if (it != g_scheds.end()) { *out = it->second; return AF_OK; }
+  std::vector<std::vector<GemmPiece>> cl;    // pieces per cluster
+  auto piece = [](int pair, int kb0, int kb1, int kind, int slot, int n_contrib, int mid) {
+    return GemmPiece{pair, kb0, kb1, kind, slot, n_contrib, mid, 0};
+  };
+  if (split == SPLIT_K) {
+    cl.resize(static_cast<size_t>(n_pairs) * splits);
+    for (int c = 0; c < n_pairs * splits; ++c) {
+      const int t = c / splits, s = c % splits;
+      cl[c].push_back(piece(t, static_cast<int>(1LL * s * nkb / splits), static_cast<int>(1LL * (s + 1) * nkb / splits),
+                            PK_PLAIN, 0, 0, s));
+    }
+  } else {
+    // stream-K ranges (cost-balanced when a range is longer than a tile)
+    const int total = n_pairs * nkb;
+    std::vector<int> ub(max_cl + 2);
+    const int n = streamk_partition(total, nkb, total < max_cl ? total : max_cl, ub.data());
+    cl.resize(n);
+    for (int c = 0; c < n; ++c) {
+      int u = ub[c];
+      while (u < ub[c + 1]) {
+        const int t = u / nkb, kb0 = u - t * nkb;
+        const int kb1 = ub[c + 1] - t * nkb < nkb ? ub[c + 1] - t * nkb : nkb;
+        if (kb0 > 0) {
+          cl[c].push_back(piece(t, kb0, kb1, PK_CONTRIB, c, 0, 0));          // slot = its cluster (one tail per range)
+        } else if (kb1 < nkb) {
+          int nc = 0;
+          while (c + 1 + nc < n && ub[c + 1 + nc] < (t + 1) * nkb) ++nc;     // ranges that start inside this tile
+          cl[c].push_back(piece(t, 0, kb1, PK_OWNER, c + 1, nc, 0));
+        } else {
+          cl[c].push_back(piece(t, 0, nkb, PK_PLAIN, 0, 0, 0));
+        }
+        u = t * nkb + kb1;
+      }
+    }
+  }
+  const int n_cl = static_cast<int>(cl.size());
+  std::vector<GemmPiece> flat(static_cast<size_t>(n_cl) * GEMM_MAX_PIECES, GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
+  for (int c = 0; c < n_cl; ++c) {
+    if (static_cast<int>(cl[c].size()) > GEMM_MAX_PIECES - 1)
+      return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: %zu pieces in one cluster (max %d)", cl[c].size(), GEMM_MAX_PIECES - 1);
+    for (size_t i = 0; i < cl[c].size(); ++i) flat[static_cast<size_t>(c) * GEMM_MAX_PIECES + i] = cl[c][i];
+  }
+  Sched sc{nullptr, n_cl};
+  CUDA_TRY(cudaMalloc(&sc.dev, flat.size() * sizeof(GemmPiece)));
+  CUDA_TRY(cudaMemcpy(sc.dev, flat.data(), flat.size() * sizeof(GemmPiece), cudaMemcpyHostToDevice));
+  g_scheds[key] = sc;
+  *out = sc;
+  return AF_OK;
+}
+
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
 // One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
@@ -307,16 +376,11 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     p.cluster = (g_gemm_cluster > 1 && n_tiles >= 2) ? 2 : 1;
     const int n_pairs = (n_tiles + p.cluster - 1) / p.cluster;     // work units are (tile pair, k-block) per cluster
     const int max_cl = g_num_sms / p.cluster;
-    p.total_units = n_pairs * p.num_kb;
-    int grid;
-    if (p.split == SPLIT_K) {
-      p.splits = gemm_split_count(n_tiles, p.K);
-      grid = n_pairs * p.splits * p.cluster;
-    } else {
-      const int n_cl = streamk_partition(p.total_units, p.num_kb, p.total_units < max_cl ? p.total_units : max_cl, p.ub);
-      grid = n_cl * p.cluster;
-      p.splits = 1;
-    }
+    p.splits = p.split == SPLIT_K ? gemm_split_count(n_tiles, p.K) : 1;
+    Sched sc;
+    if ((rc = build_schedule(p.split, n_pairs, p.num_kb, max_cl, p.splits, &sc))) return rc;
+    p.sched = sc.dev;
+    const int grid = sc.n_cl * p.cluster;
     p.mma2 = (g_gemm_mma2 && p.cluster == 2 && p.w_fp16) ? 1 : 0;
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (p.mma2 ? n_pad / 2 : n_pad) * GEMM_BK * 2;
     // epilogue staging: two 4 KB buffers per warp, or one 2 KB buffer when that buys a pipeline stage (the main loop

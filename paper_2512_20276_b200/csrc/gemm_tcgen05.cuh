@@ -58,12 +58,21 @@ constexpr int GEMM_BLK = 32 * (GEMM_EPI_WARPS / 4);  // columns one round of the
 constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
-constexpr int GEMM_MAX_CLUSTERS = 160;  // stream-K ranges (clusters, or CTAs when the cluster size is 1)
 constexpr int GEMM_XCH_MAX = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB (or one 2 KB) staging buffers for TMA stores
 constexpr int GEMM_SMEM_BUDGET = 232448 - 1024;    // dynamic shared memory: 227 KB minus the static part
 
 enum GemmEpilogue : int { EPI_STORE = 0, EPI_SWIGLU = 1 };
 enum GemmSplit : int { SPLIT_STREAMK = 0, SPLIT_K = 1 };
+
+// One piece of a cluster's work: k-blocks [kb0, kb1) of tile pair `pair` (CTA r of the cluster computes tile
+// pair * cluster + r).  PK_PLAIN pieces cover a whole tile (or, in SPLIT_K mode, one slab `mid` of it) and are
+// drained straight to the output; a PK_CONTRIB piece writes its partial to slot `slot` and raises the slot's flag;
+// a PK_OWNER piece waits for the n_contrib partials in slots [slot, slot + n_contrib), adds them (in slot order) to
+// its own accumulator (nothing of its own when kb0 == kb1) and runs the epilogue.  The host builds the lists so that
+// contributor pieces come first in their cluster and owner pieces last (af_lib.cu, build_schedule).
+enum GemmPieceKind : int { PK_PLAIN = 0, PK_CONTRIB = 1, PK_OWNER = 2 };
+struct alignas(16) GemmPiece { int pair, kb0, kb1, kind, slot, n_contrib, mid, pad; };
+constexpr int GEMM_MAX_PIECES = 16;
 
 // The output is written with TMA tensor stores through map_out, a rank-3 view (feature, middle, token) of the
 // destination: middle = weight part (q|k|v stacked along the feature axis) or split-K slab; the map's extents clip
@@ -82,8 +91,7 @@ struct GemmParams {
   int mma2;            // 1 (needs cluster == 2, w_fp16): tcgen05.mma.cta_group::2 over the pair, activation rows split
   int split;           // GemmSplit
   int splits;          // SPLIT_K: pieces per tile
-  int total_units;     // SPLIT_STREAMK: (tile pair, k-block) units; cluster c owns units [ub[c], ub[c+1])
-  int ub[GEMM_MAX_CLUSTERS + 1];
+  const GemmPiece* sched;  // device: [clusters][GEMM_MAX_PIECES] pieces, ended by pair = -1
   int stages;
   int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue

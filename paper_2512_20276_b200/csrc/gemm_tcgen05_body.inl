@@ -61,15 +61,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   const uint32_t tmem_base = tmem_base_smem;
   pdl_launch_dependents();  // dependents still wait (griddepcontrol.wait) for this whole grid before reading its output
 
-  int u_begin, u_end;
-  if (p.split == SPLIT_K) {
-    const int tile = cl / p.splits, s = cl - tile * p.splits;
-    u_begin = tile * p.num_kb + static_cast<int>(static_cast<long long>(s) * p.num_kb / p.splits);
-    u_end = tile * p.num_kb + static_cast<int>(static_cast<long long>(s + 1) * p.num_kb / p.splits);
-  } else {
-    u_begin = p.ub[cl];        // cost-balanced contiguous ranges (units + a charge per tile drain), computed on the host
-    u_end = p.ub[cl + 1];
-  }
+  // this cluster's pieces (host-built schedule, see GemmPiece): every role walks the same list
+  const GemmPiece* my_pieces = p.sched + static_cast<size_t>(cl) * GEMM_MAX_PIECES;
+  auto get_piece = [&](int i) {
+    GemmPiece pc;
+    const int4* src = reinterpret_cast<const int4*>(my_pieces + i);
+    *reinterpret_cast<int4*>(&pc) = __ldg(src);
+    *(reinterpret_cast<int4*>(&pc) + 1) = __ldg(src + 1);
+    return pc;
+  };
 
   if (warp == GEMM_EPI_WARPS) {
     // ================================ TMA producer ================================
@@ -77,7 +77,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       const uint64_t pol_w = policy_evict_first();  // weights are streamed once per step
       const uint64_t pol_x = policy_evict_last();   // the packed activations are re-read by every CTA
       // (pair, kb) of the unit being loaded, advanced incrementally: no division in the steady-state loop
-      int l_pair = u_begin / p.num_kb, l_kb = u_begin - l_pair * p.num_kb;
+      int l_pi = -1, l_pair = 0, l_kb = 0, l_kb1 = 0;   // cursor over the (piece, k-block) units that need loads
+      bool l_more = true;
       const CUtensorMap* l_mw = &map_w0;
       int l_row = 0;   // first weight row of this CTA's tile in its matrix
       auto set_tile = [&]() {
@@ -90,9 +91,17 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           l_row = (tile - part * p.tiles_per_part) * GEMM_BM;
         }
       };
-      set_tile();
+      auto next_piece = [&]() {   // move the cursor to the next piece that has k-blocks
+        while (true) {
+          if (++l_pi >= GEMM_MAX_PIECES) { l_more = false; return; }
+          const GemmPiece pc = get_piece(l_pi);
+          if (pc.pair < 0) { l_more = false; return; }
+          if (pc.kb1 > pc.kb0) { l_pair = pc.pair; l_kb = pc.kb0; l_kb1 = pc.kb1; set_tile(); return; }
+        }
+      };
+      next_piece();
       auto advance = [&]() {
-        if (++l_kb == p.num_kb) { l_kb = 0; ++l_pair; set_tile(); }
+        if (++l_kb == l_kb1) next_piece();
       };
       auto load_w = [&](int stage) {
         uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
@@ -131,24 +140,23 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
       };
       // The weights do not depend on the previous kernel: start streaming them before the PDL dependency resolves.
-      const int n_pre = min(p.stages, u_end - u_begin);
-      const int kb_first = l_kb;
-      for (int i = 0; i < n_pre; ++i) {
-        if (!mma2) mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
-        else if (crank == 0) mbar_arrive_expect_tx(&full_bar[i], 2 * stage_bytes);
-        load_w(i);
+      int n_pre = 0;
+      int kb_pre[GEMM_MAX_STAGES];
+      while (n_pre < p.stages && l_more) {
+        if (!mma2) mbar_arrive_expect_tx(&full_bar[n_pre], stage_bytes);
+        else if (crank == 0) mbar_arrive_expect_tx(&full_bar[n_pre], 2 * stage_bytes);
+        load_w(n_pre);
+        kb_pre[n_pre] = l_kb;
         advance();
+        ++n_pre;
       }
       AF_TRACE(24);
       pdl_wait();
       AF_TRACE(25);
-      for (int i = 0, kb = kb_first; i < n_pre; ++i) {
-        load_x(kb, i);
-        if (++kb == p.num_kb) kb = 0;
-      }
+      for (int i = 0; i < n_pre; ++i) load_x(kb_pre[i], i);
       int stage = n_pre == p.stages ? 0 : n_pre;
       uint32_t phase = n_pre == p.stages ? 1 : 0;
-      for (int u = u_begin + n_pre; u < u_end; ++u) {
+      while (l_more) {
         mbar_wait(&empty_bar[stage], phase ^ 1);
         if (!mma2) mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
         else if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
@@ -166,10 +174,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       const uint32_t idesc2 = umma_idesc_bf16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n2 > 0 ? p.n2 : 16);
       int stage = 0;
       uint32_t phase = 0, acc_phase = 0;
-      int u = u_begin;
-      while (u < u_end) {
-        const int tile = u / p.num_kb, kb0 = u - tile * p.num_kb;
-        const int kb1 = min(p.num_kb, kb0 + (u_end - u));
+      for (int pi = 0; pi < GEMM_MAX_PIECES; ++pi) {
+        const GemmPiece pc = get_piece(pi);
+        if (pc.pair < 0) break;
+        const int kb0 = pc.kb0, kb1 = pc.kb1;
+        if (kb1 <= kb0) continue;                   // a reduce-only piece: nothing to multiply
         mbar_wait(&tmem_empty_bar, acc_phase ^ 1);  // epilogue has drained the accumulator
         tc_fence_after();
         for (int kb = kb0; kb < kb1; ++kb) {
@@ -201,7 +210,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
         if (mma2) umma_commit_cg2_mc(&tmem_full_bar, 0x3); else umma_commit(&tmem_full_bar);  // accumulator -> epilogue
         acc_phase ^= 1;
-        u += kb1 - kb0;
       }
     }
   } else {
@@ -238,15 +246,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     const int stage_area = p.stages * static_cast<int>(stage_bytes);
     uint32_t acc_phase = 0, fix_phase = 0, cphase = 0;
     int cstage = 0;
-    int u = u_begin;
-    while (u < u_end) {
-      const int pair = u / p.num_kb, kb0 = u - pair * p.num_kb;
-      const int kb1 = min(p.num_kb, kb0 + (u_end - u));
+    for (int pi = 0; pi < GEMM_MAX_PIECES; ++pi) {
+      const GemmPiece pc = get_piece(pi);
+      if (pc.pair < 0) break;
+      const int pair = pc.pair, kb0 = pc.kb0, kb1 = pc.kb1;
+      const bool has_mma = kb1 > kb0;             // false: a reduce-only owner piece (its whole tile was computed by others)
       const int tile = pair * p.cluster + crank;
       const bool tile_valid = tile < p.n_tiles;   // (an odd tile count leaves the last cluster's second CTA idle)
-      const bool streamk = p.split == SPLIT_STREAMK;
-      const bool contributor = streamk && kb0 > 0;
-      const bool owner_partial = streamk && (kb0 == 0) && (kb1 < p.num_kb);
+      const bool contributor = pc.kind == PK_CONTRIB;
+      const int my_slot = pc.slot * p.cluster + crank;   // contributor: where its partial and flag go
       // ---- weight transform: this piece's W stages bf16 -> fp16, in place, as they land (exact for every finite
       //      bf16 weight below 65504 in magnitude; values under 2^-14 keep 10 + e bits as fp16 subnormals) ----
       for (int kb = p.w_fp16 ? kb1 : kb0; kb < kb1; ++kb) {
@@ -265,12 +273,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         if (++cstage == p.stages) { cstage = 0; cphase ^= 1; }
       }
       int c_first = 0, n_contrib = 0;
-      if (owner_partial) {
-        // CTAs holding the rest of this tile: cta+1 .. while their range starts before the tile ends
-        c_first = cl + 1;   // cluster index; the contributing CTA of cluster c is c * cluster + crank
-        const int tile_end = (pair + 1) * p.num_kb;
-        const int n_cl = static_cast<int>(gridDim.x) / p.cluster;
-        while (c_first + n_contrib < n_cl && p.ub[c_first + n_contrib] < tile_end) ++n_contrib;
+      if (pc.kind == PK_OWNER) {
+        // the rest of this tile was (or is being) computed by the contributor pieces in slots [slot, slot + n_contrib)
+        c_first = pc.slot; n_contrib = pc.n_contrib;
         if (etid < n_contrib) {
           volatile int* f = p.flags + (c_first + etid) * p.cluster + crank;
           while (*f == 0) {
@@ -281,7 +286,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         AF_EPI_BAR();
       }
       if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
-      mbar_wait(&tmem_full_bar, acc_phase);
+      if (has_mma) mbar_wait(&tmem_full_bar, acc_phase);
       tc_fence_after();
       if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
       store_ok = tile_valid;
@@ -292,7 +297,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       } else {
         const int part = tile / p.tiles_per_part;
         f0 = (tile - part * p.tiles_per_part) * GEMM_BM + quad * 32;
-        mid = p.split == SPLIT_K ? cl % p.splits : part;
+        mid = p.split == SPLIT_K ? pc.mid : part;
       }
       // column blocks: with contributors, their partial columns [b0, b1) are bulk-copied into the (now idle) stages,
       // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 64-column blocks
@@ -328,6 +333,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         fix_phase ^= 1;
       };
       auto load_acc = [&](int c0, int cw, float* v) {
+        if (!has_mma) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = 0.f;
+          return;
+        }
         uint32_t r[32];
         const uint32_t ta = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0;
         tmem_ld16(ta, r);
@@ -363,7 +373,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
 #pragma unroll
           for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __half_as_ushort(__float2half_rn(v[j]));
-          stage_store(&map_part, quad * 32, c0, cta);
+          stage_store(&map_part, quad * 32, c0, my_slot);
         } else if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
           // fp32: stream-K partial [cta][token][128 features] or the fp32 output, one 32-token box per chunk (4 KB
           // staging buffers) or two 16-token boxes (2 KB)
@@ -372,7 +382,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
             float* sb = reinterpret_cast<float*>(stg);
 #pragma unroll
             for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
-            if (contributor) stage_store(&map_part, quad * 32, c0, cta);
+            if (contributor) stage_store(&map_part, quad * 32, c0, my_slot);
             else stage_store(&map_out, f0, mid, p.tok0 + c0);
           } else {
 #pragma unroll
@@ -382,7 +392,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
                 float* sb = reinterpret_cast<float*>(stg);
 #pragma unroll
                 for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = v[hh * 16 + j];
-                if (contributor) stage_store(&map_part, quad * 32, c0 + hh * 16, cta);
+                if (contributor) stage_store(&map_part, quad * 32, c0 + hh * 16, my_slot);
                 else stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 16);
               }
             }
@@ -442,7 +452,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) { if (mma2) mbar_arrive_leader(&tmem_empty_bar); else mbar_arrive(&tmem_empty_bar); }
+      if (lane == 0 && has_mma) { if (mma2) mbar_arrive_leader(&tmem_empty_bar); else mbar_arrive(&tmem_empty_bar); }
       if (contributor) {
         if (lane == 0) { bulk_wait<0>(); fence_proxy_async_all(); }  // this warp's partial stores are complete
         __syncwarp();
@@ -450,13 +460,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         AF_EPI_BAR();
         if (etid == 0) {
           __threadfence();
-          atomicExch(p.flags + cta, 1);
+          atomicExch(p.flags + my_slot, 1);
         }
       }
       if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
       ++piece;
-      acc_phase ^= 1;
-      u += kb1 - kb0;
+      if (has_mma) acc_phase ^= 1;
     }
     if (lane == 0) bulk_wait<0>();  // all output stores are complete before the CTA exits
   }
