@@ -149,6 +149,14 @@ int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32
 int af_debug_profile(int enable);
 int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
 
+/* The work lists of the GEMM kernel (pure host logic, needs no GPU): for `n_tile_pairs` pairs of 128-row weight tiles and
+ * `n_kblocks` 64-wide k-blocks on at most `max_clusters` 2-CTA clusters, either split-K (split_k != 0: `splits` slabs per
+ * tile pair) or stream-K ranges.  pieces = HOST int32 [max_clusters_out][16][8]; piece = {pair, kb0, kb1, kind (0 plain,
+ * 1 contributor, 2 owner), slot, n_contrib, slab, 0}, a cluster's list ends at pair = -1.  Returns the number of
+ * clusters used, or a negative AF_ERR_*. */
+int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters, int32_t splits,
+                           int32_t* pieces, int32_t max_clusters_out);
+
 /* Debug timeline of the GEMM kernel: while enabled every gemm_tcgen05_kernel launch records %globaltimer / clock stamps
  * per CTA (kernel start, PDL wait, per piece: accumulator ready / fix-up loaded / drained, producer and MMA-thread
  * counters) into a library-owned device buffer that keeps the last 16 launches.  af_debug_trace_read synchronises and

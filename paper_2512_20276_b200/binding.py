@@ -50,7 +50,7 @@ class af_weights(C.Structure):
 
 EXPORTS = ["af_convert_bf16_to_fp16", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
-           "af_debug_launch_count", "af_debug_gemm", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
+           "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
 PROFILE_CLASSES = ["gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm", "attention", "rope_append",
                    "rmsnorm", "silu_mul", "other"]

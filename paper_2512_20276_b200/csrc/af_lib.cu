@@ -276,7 +276,8 @@ static int streamk_partition(int total, int nkb, int n_max, int* ub) {
     if (out) out[n] = total;
     return n;
   };
-  int lo = total / n_max, hi = total / n_max + 3 * kHead + nkb;   // smallest cap that fits n_max ranges
+  // smallest cap that fits n_max ranges (one range can always take everything: hi is feasible)
+  int lo = total / n_max, hi = total + (total / nkb + 2) * kHead;
   while (lo < hi) { const int mid = (lo + hi) / 2; if (fill(mid, nullptr) <= n_max) hi = mid; else lo = mid + 1; }
   return fill(lo, ub);
 }
@@ -295,11 +296,9 @@ struct SchedKey {
 struct Sched { GemmPiece* dev; int n_cl; };
 static std::map<SchedKey, Sched> g_scheds;
 
-static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
-  std::lock_guard<std::mutex> lk(g_mu);
-  const SchedKey key{split, n_pairs, nkb, max_cl, splits};
-  auto it = g_scheds.find(key);
-  if (it != g_scheds.end()) { *out = it->second; return AF_OK; }
+// Pure host part: the flat [n_cl][GEMM_MAX_PIECES] table (also what af_debug_gemm_schedule returns, for CPU tests).
+static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, std::vector<GemmPiece>* flat_out, int* n_cl_out) {
+  if (n_pairs < 1 || nkb < 1 || max_cl < 1 || splits < 1) return fail(AF_ERR_ARG, "bad schedule shape");
   std::vector<std::vector<GemmPiece>> cl;    // pieces per cluster
   auto piece = [](int pair, int kb0, int kb1, int kind, int slot, int n_contrib, int mid) {
     return GemmPiece{pair, kb0, kb1, kind, slot, n_contrib, mid, 0};
@@ -336,12 +335,26 @@ static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int split
     }
   }
   const int n_cl = static_cast<int>(cl.size());
-  std::vector<GemmPiece> flat(static_cast<size_t>(n_cl) * GEMM_MAX_PIECES, GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
+  std::vector<GemmPiece>& flat = *flat_out;
+  flat.assign(static_cast<size_t>(n_cl) * GEMM_MAX_PIECES, GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
   for (int c = 0; c < n_cl; ++c) {
     if (static_cast<int>(cl[c].size()) > GEMM_MAX_PIECES - 1)
       return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: %zu pieces in one cluster (max %d)", cl[c].size(), GEMM_MAX_PIECES - 1);
     for (size_t i = 0; i < cl[c].size(); ++i) flat[static_cast<size_t>(c) * GEMM_MAX_PIECES + i] = cl[c][i];
   }
+  *n_cl_out = n_cl;
+  return AF_OK;
+}
+
+static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  const SchedKey key{split, n_pairs, nkb, max_cl, splits};
+  auto it = g_scheds.find(key);
+  if (it != g_scheds.end()) { *out = it->second; return AF_OK; }
+  std::vector<GemmPiece> flat;
+  int n_cl = 0;
+  const int rc = make_schedule(split, n_pairs, nkb, max_cl, splits, &flat, &n_cl);
+  if (rc) return rc;
   Sched sc{nullptr, n_cl};
   CUDA_TRY(cudaMalloc(&sc.dev, flat.size() * sizeof(GemmPiece)));
   CUDA_TRY(cudaMemcpy(sc.dev, flat.data(), flat.size() * sizeof(GemmPiece), cudaMemcpyHostToDevice));
@@ -590,6 +603,18 @@ extern "C" int af_convert_bf16_to_fp16(const void* src, void* dst, size_t n, voi
   convert_bf16_to_fp16_kernel<<<static_cast<unsigned>((n_vec + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(
       reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst), n_vec);
   return check_launch("convert_bf16_to_fp16_kernel");
+}
+
+extern "C" int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters,
+                                      int32_t splits, int32_t* pieces, int32_t max_clusters_out) {
+  if (!pieces) return fail(AF_ERR_ARG, "null output");
+  std::vector<GemmPiece> flat;
+  int n_cl = 0;
+  const int rc = make_schedule(split_k ? SPLIT_K : SPLIT_STREAMK, n_tile_pairs, n_kblocks, max_clusters, splits, &flat, &n_cl);
+  if (rc) return rc;
+  if (n_cl > max_clusters_out) return fail(AF_ERR_ARG, "%d clusters do not fit the output (%d)", n_cl, max_clusters_out);
+  memcpy(pieces, flat.data(), flat.size() * sizeof(GemmPiece));
+  return n_cl;
 }
 
 extern "C" int64_t af_debug_launch_count(void) { return g_launches.load(); }

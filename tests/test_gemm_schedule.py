@@ -1,0 +1,114 @@
+"""Host logic of the GEMM kernel's work split (af_debug_gemm_schedule; no GPU needed): every (tile pair, k-block) is
+computed exactly once, split tiles have exactly one owner whose contributor slots are exactly the pieces of the rest of
+the tile, contributor pieces come before owner pieces in every cluster (so no owner can wait on a piece that is queued
+behind another owner: deadlock freedom on a co-resident grid), and the ranges are balanced."""
+import ctypes as C
+
+import numpy as np
+import pytest
+from hypothesis import given, settings, strategies as st
+
+PLAIN, CONTRIB, OWNER = 0, 1, 2
+
+
+def schedule(split_k, n_pairs, nkb, max_cl, splits=1):
+    from paper_2512_20276_b200 import binding
+    L = binding.load_library()
+    L.af_debug_gemm_schedule.argtypes = [C.c_int32] * 5 + [C.c_void_p, C.c_int32]
+    L.af_debug_gemm_schedule.restype = C.c_int
+    cap = max(max_cl, n_pairs * splits)
+    buf = np.full((cap, 16, 8), -7, dtype=np.int32)
+    n = L.af_debug_gemm_schedule(int(split_k), n_pairs, nkb, max_cl, splits, buf.ctypes.data, cap)
+    assert n > 0, L.af_last_error().decode()
+    out = []
+    for c in range(n):
+        pieces = []
+        for i in range(16):
+            pair, kb0, kb1, kind, slot, n_contrib, mid, _ = (int(x) for x in buf[c, i])
+            if pair < 0:
+                break
+            pieces.append(dict(pair=pair, kb0=kb0, kb1=kb1, kind=kind, slot=slot, n_contrib=n_contrib, mid=mid))
+        out.append(pieces)
+    return out
+
+
+def check_streamk(n_pairs, nkb, max_cl):
+    cl = schedule(False, n_pairs, nkb, max_cl)
+    assert 1 <= len(cl) <= max_cl
+    cover = np.zeros((n_pairs, nkb), dtype=np.int32)
+    contrib_by_slot = {}
+    for c, pieces in enumerate(cl):
+        assert pieces, "a launched cluster has work"
+        seen_owner = False
+        for p in pieces:
+            assert 0 <= p["pair"] < n_pairs and 0 <= p["kb0"] <= p["kb1"] <= nkb
+            cover[p["pair"], p["kb0"]:p["kb1"]] += 1
+            if p["kind"] == CONTRIB:
+                assert not seen_owner, "a contributor piece queued behind an owner piece could deadlock"
+                assert p["slot"] not in contrib_by_slot, "one partial slot per contributor piece"
+                contrib_by_slot[p["slot"]] = p
+            elif p["kind"] == OWNER:
+                seen_owner = True
+                assert p is pieces[-1], "an owner piece is the last piece of its cluster (it reuses the pipeline stages)"
+            else:
+                assert p["kind"] == PLAIN and (p["kb0"], p["kb1"]) == (0, nkb)
+    assert (cover == 1).all(), "every (tile pair, k-block) exactly once"
+    owners = {}
+    for pieces in cl:
+        for p in pieces:
+            if p["kind"] == OWNER:
+                assert p["pair"] not in owners
+                owners[p["pair"]] = p
+                got = [(p["kb0"], p["kb1"])]
+                for s in range(p["slot"], p["slot"] + p["n_contrib"]):
+                    q = contrib_by_slot.pop(s)
+                    assert q["pair"] == p["pair"]
+                    got.append((q["kb0"], q["kb1"]))
+                got = sorted(g for g in got if g[1] > g[0])
+                assert got[0][0] == 0 and got[-1][1] == nkb and all(a[1] == b[0] for a, b in zip(got, got[1:]))
+    assert not contrib_by_slot, "every contributor piece belongs to exactly one owner"
+    units = [sum(p["kb1"] - p["kb0"] for p in pieces) for pieces in cl]
+    return cl, units
+
+
+@pytest.mark.parametrize("n_pairs,nkb,max_cl", [
+    (48, 64, 74),      # QKV at 7B
+    (86, 64, 74),      # gate/up at 7B
+    (125, 64, 74),     # LM head
+    (1, 1, 74), (1, 64, 74), (3, 4, 74), (6, 11, 74), (2, 172, 74), (500, 8, 74), (7, 3, 2), (74, 64, 74), (75, 64, 74),
+])
+def test_streamk_schedules_cover_and_order(n_pairs, nkb, max_cl):
+    cl, units = check_streamk(n_pairs, nkb, max_cl)
+    total = n_pairs * nkb
+    if total >= max_cl:
+        assert max(units) <= -(-total // len(cl)) + nkb              # ranges stay near the mean
+
+
+def test_7b_shapes_are_balanced_and_shallow():
+    for n_pairs in (48, 86):
+        cl, units = check_streamk(n_pairs, 64, 74)
+        assert len(cl) >= 72 and max(units) <= -(-n_pairs * 64 // 74) + 2 and sorted(units)[1] >= 40
+        assert max(len(p) for p in cl) <= 2 + (n_pairs == 48)       # no cluster drains more than 2 (3) accumulators
+
+
+@settings(max_examples=150, deadline=None)
+@given(st.integers(1, 300), st.integers(1, 200), st.integers(1, 80))
+def test_streamk_schedules_random_shapes(n_pairs, nkb, max_cl):
+    if -(-n_pairs * nkb // min(n_pairs * nkb, max_cl)) // nkb + 2 > 15:
+        return                                                          # more than 15 pieces per cluster is rejected
+    check_streamk(n_pairs, nkb, max_cl)
+
+
+@pytest.mark.parametrize("n_pairs,nkb,splits", [(16, 64, 4), (16, 172, 4), (1, 4, 4), (3, 11, 2), (5, 7, 1)])
+def test_splitk_schedules(n_pairs, nkb, splits):
+    cl = schedule(True, n_pairs, nkb, 74, splits)
+    assert len(cl) == n_pairs * splits
+    cover = np.zeros((n_pairs, nkb), dtype=np.int32)
+    slabs = set()
+    for pieces in cl:
+        assert len(pieces) == 1 and pieces[0]["kind"] == PLAIN and pieces[0]["kb1"] > pieces[0]["kb0"]
+        p = pieces[0]
+        cover[p["pair"], p["kb0"]:p["kb1"]] += 1
+        assert (p["pair"], p["mid"]) not in slabs
+        slabs.add((p["pair"], p["mid"]))
+    assert (cover == 1).all() and len(slabs) == n_pairs * splits
