@@ -147,6 +147,59 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------- cfg5 sweep
+def run_sweep(args):
+    """BASELINE.json configs[4]: concurrent decodes x prefill length at the 7B shape.  Prints one markdown table row per
+    grid point (step latency, packed tok/s, achieved HBM GB/s = algorithmic bytes / latency, tensor TFLOP/s, fraction
+    of the point's roofline at the measured peaks).  Not the bench line; a report for profiles/."""
+    import torch
+    from paper_2512_20276_b200 import binding, inputs as I
+    torch.cuda.set_device(0)
+    cfg = I.cfg_7b_layers(args.layers)
+    hw = I.make_weights(cfg, 4, threads=max(4, os.cpu_count() or 8))
+    W = binding.Weights(cfg, hw)
+    Rr, Cc = 17, 1024
+    ring = binding.Ring(cfg, Rr, Cc, max_rows=544)
+    H = I.make_embeds(cfg, 4, 1, 291).cuda()
+    E = I.make_embeds(cfg, 4, 0, 512).cuda()
+    for j in range(15):
+        ring.packed_forward(W, H[:276 + j].contiguous(), [(j + 1, 0, 0, 276 + j)])
+    peaks = load_peaks()
+    hidden = torch.empty(544, cfg.d_model, dtype=torch.float32, device="cuda")
+    print("| decodes | prefill | T | ms/step | packed tok/s | HBM GB/s (algorithmic) | TFLOP/s | roofline ms (measured peaks) | frac |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    for n_dec in (0, 1, 3, 6, 10, 15):
+        for p_len in (0, 128, 276, 512):
+            if n_dec == 0 and p_len == 0:
+                continue
+            segs, rows = [], []
+            if p_len:
+                segs.append((0, 0, 0, p_len)); rows.append(E[:p_len])
+            for j in range(n_dec):
+                segs.append((j + 1, 1, 276 + j, 1)); rows.append(H[276 + j:277 + j])
+            x = torch.cat(rows).contiguous()
+
+            def one():
+                ring.reset_slot(0, 0)
+                for j in range(15):
+                    ring.set_len(j + 1, 276 + j)
+                ring.packed_forward(W, x, segs, hidden_out=hidden[:x.shape[0]])
+            for _ in range(3):
+                one()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                one()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            wk = step_work(cfg, segs, 0)
+            roof = max(wk["bytes"] / (peaks["hbm_gbs"] * 1e9), wk["flops"] / (peaks["tf_sustained"] * 1e12)) * 1e3
+            print(f"| {n_dec} | {p_len} | {wk['T']} | {ms:.3f} | {wk['T'] / ms * 1e3:.0f} | {wk['bytes'] / ms / 1e6:.0f} | "
+                  f"{wk['flops'] / ms / 1e9:.0f} | {roof:.3f} | {roof / ms:.2f} |", flush=True)
+
+
 # ---------------------------------------------------------------------------------------------- our arm
 def main():
     ap = argparse.ArgumentParser()
@@ -156,9 +209,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=32, help="debug only: fewer layers (the line then says so)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import torch
     import torch.distributed as dist

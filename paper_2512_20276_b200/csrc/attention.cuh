@@ -11,7 +11,10 @@ namespace af {
 
 constexpr int ATT_BQ = 64;
 constexpr int ATT_BKV = 32;
-constexpr int ATT_STAGES = 3;   // K/V tiles in flight (cp.async groups)
+#ifndef AF_ATT_STAGES
+#define AF_ATT_STAGES 3
+#endif
+constexpr int ATT_STAGES = AF_ATT_STAGES;   // K/V tiles in flight (cp.async groups)
 constexpr int att_smem_bytes(int hd) { return (ATT_BQ + 2 * ATT_STAGES * ATT_BKV) * hd * 2; }
 constexpr int ATT_THREADS = 128;
 
@@ -110,10 +113,11 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
       cp_async16(sV + stage * TILE_BYTES + sw_off<HD>(r, c), vbase + off, ok);
     }
   };
-  load_kv(0, 0);
-  cp_async_commit();
-  if (n_tiles > 1) load_kv(1, 1);
-  cp_async_commit();
+#pragma unroll
+  for (int t = 0; t < ATT_STAGES - 1; ++t) {   // prologue: the first ATT_STAGES - 1 tiles (a group each, empty past the end)
+    if (t < n_tiles) load_kv(t, t);
+    cp_async_commit();
+  }
 
   float o_acc[HD / 8][4];
 #pragma unroll
@@ -127,9 +131,10 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
 
   for (int tile = 0; tile < n_tiles; ++tile) {
     const int stage = tile % ATT_STAGES;
-    if (tile + 2 < n_tiles) load_kv(tile + 2, (tile + 2) % ATT_STAGES);   // its stage was released at the end of tile - 1
+    // the stage of tile + STAGES - 1 was released at the end of tile - 1
+    if (tile + ATT_STAGES - 1 < n_tiles) load_kv(tile + ATT_STAGES - 1, (tile + ATT_STAGES - 1) % ATT_STAGES);
     cp_async_commit();
-    cp_async_wait<2>();
+    cp_async_wait<ATT_STAGES - 1>();
     __syncthreads();
     if (tile == 0) {
 #pragma unroll
