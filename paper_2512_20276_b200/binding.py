@@ -219,7 +219,7 @@ def debug_gemm(a: torch.Tensor, w: torch.Tensor) -> torch.Tensor:
     n_tok, k = a.shape
     n_out = w.shape[0]
     out = torch.empty(n_tok, n_out, dtype=torch.float32, device=a.device)
-    ws = torch.empty(160 * 288 * 128 * 4, dtype=torch.uint8, device=a.device)
+    ws = torch.empty(160 * 512 * 128 * 4, dtype=torch.uint8, device=a.device)
     _check(L.af_debug_gemm(a.data_ptr(), w.data_ptr(), out.data_ptr(), n_tok, n_out, k, ws.data_ptr(), ws.numel(),
                            _stream_ptr()))
     return out

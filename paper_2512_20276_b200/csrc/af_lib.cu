@@ -365,7 +365,7 @@ static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int split
 
 static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) * GEMM_MAX_TOK * GEMM_BM * sizeof(float); }
 
-// One projection over all T packed rows (token chunks of <= 288 rows per launch).  `proto` carries the weight
+// One projection over all T packed rows (token chunks of <= 512 rows per launch).  `proto` carries the weight
 // layout (n_parts / part_rows / a_pair), the split mode and the epilogue fields; the decomposition is filled here.
 static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView& ov, /* proto.w_fp16 set by the caller */ const void* x, int x_rows_cap,
                        const void* const* w, int T) {
@@ -422,7 +422,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     CUtensorMap mo, mp;
     p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
     if ((rc = get_out_map(ov, p.stg_bytes, &mo))) return rc;
-    {  // stream-K partials [grid][288 tokens][128 features] fp32, box = 32 features x 8 tokens of one CTA
+    {  // stream-K partials [slot][512 tokens][128 features], box = 32 features x 32 (or 16) tokens of one slot
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
       const unsigned long long pe = p.part_f16 ? 2 : 4;
       const unsigned long long strides[2] = {GEMM_BM * pe, GEMM_BM * pe * GEMM_MAX_TOK};

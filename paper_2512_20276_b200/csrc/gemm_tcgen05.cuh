@@ -2,7 +2,7 @@
 // (steps a2/a5/a7/a8/a10 of SURVEY.md 8(a); Alg. 2 lines 2 and 6).  DESIGN.md section 6.1.
 //
 // "Swap-AB" orientation: the WEIGHT tile (128 output features x 64 k) is the UMMA A operand and the packed TOKEN tile
-// (all T <= 288 tokens x 64 k) is the B operand, so the 282-row packed matrix of the paper's schedule maps onto UMMA
+// (all T <= 512 tokens x 64 k of a launch) is the B operand, so the 282-row packed matrix of the paper's schedule maps onto UMMA
 // N = 2 x 144 with 2% padding instead of 3 x 128-row M tiles with 27% padding, and a decode-only step (T <= 16) uses
 // N = 16.  Both operands are K-major in global memory, are staged by TMA with the 128-byte swizzle, and are consumed by
 // tcgen05.mma kind::f16 (fp16 activations x fp16 weights - prepared at load time, or bf16 weights rewritten as fp16 per
@@ -55,7 +55,7 @@ constexpr int GEMM_BK = 64;        // bf16 elements per k-block = one 128-byte s
 constexpr int GEMM_EPI_WARPS = AF_EPI_WARPS;  // two per TMEM lane quadrant (warp % 4), alternating 32-token chunks
 constexpr int GEMM_THREADS = (GEMM_EPI_WARPS + 2) * 32;
 constexpr int GEMM_BLK = 32 * (GEMM_EPI_WARPS / 4);  // columns one round of the epilogue warps covers
-constexpr int GEMM_MAX_TOK = 288;  // tokens per launch (two UMMA N halves of <= 144, or one of <= 256)
+constexpr int GEMM_MAX_TOK = 512;  // tokens per launch: one UMMA N <= 256, or two halves of <= 256 (all 512 TMEM columns)
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
 constexpr int GEMM_XCH_MAX = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB (or one 2 KB) staging buffers for TMA stores
@@ -97,7 +97,7 @@ struct GemmParams {
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile
   int out_bf16;        // EPI_STORE: 0 = fp32 output, 1 = bf16, 2 = fp16 (box 32 features x 32 tokens)
-  void* partial;       // [grid][288][128] stream-K partials, fp32 or (part_f16) fp16, written through map_part
+  void* partial;       // [slot][512][128] stream-K partials, fp32 or (part_f16) fp16, written through map_part
   int part_f16;
   int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
   long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr
