@@ -89,11 +89,11 @@ static std::map<MapKey, CUtensorMap> g_maps;
 
 // Cached cuTensorMapEncodeTiled.  dims / box innermost first; strides (bytes) of dims 1..rank-1.
 static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 2 = bf16, -2 = fp16, 4 = fp32 */ const unsigned long long* dims,
-                      const unsigned long long* strides, const unsigned* box, bool swizzle128, CUtensorMap* out) {
+                      const unsigned long long* strides, const unsigned* box, int swizzle /* 0 none, 128, 64 or 32 bytes */, CUtensorMap* out) {
   std::lock_guard<std::mutex> lk(g_mu);
   MapKey key;
   memset(&key, 0, sizeof key);
-  key.ptr = ptr; key.elem = elem_bytes; key.rank = rank; key.swz = swizzle128;
+  key.ptr = ptr; key.elem = elem_bytes; key.rank = rank; key.swz = swizzle;
   for (int i = 0; i < rank; ++i) { key.d[i] = dims[i]; key.b[i] = box[i]; }
   for (int i = 0; i + 1 < rank; ++i) key.st[i] = strides[i];
   auto it = g_maps.find(key);
@@ -116,7 +116,9 @@ static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 
   const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
                                  : (elem_bytes == -2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32);
   CUresult r = g_encode(&m, dt, rank, const_cast<void*>(ptr), d, st, bx, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                        swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                        : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                        : swizzle == 32 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE,
                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(AF_ERR_CUDA, "cuTensorMapEncodeTiled(%p, rank %d) -> %d", ptr, rank, (int)r);
   if (g_maps.size() > 8192) g_maps.clear();
@@ -131,7 +133,7 @@ static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
   const unsigned long long dims[2] = {static_cast<unsigned long long>(cols), static_cast<unsigned long long>(rows)};
   const unsigned long long strides[1] = {static_cast<unsigned long long>(cols) * 2};
   const unsigned box[2] = {static_cast<unsigned>(GEMM_BK), static_cast<unsigned>(box_rows)};
-  return get_map_nd(ptr, fp16 ? -2 : 2, 2, dims, strides, box, true, out);
+  return get_map_nd(ptr, fp16 ? -2 : 2, 2, dims, strides, box, 128, out);
 }
 
 // Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
@@ -144,7 +146,8 @@ static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
                                          static_cast<unsigned long long>(o.ld_tok) * eb};
   const int et = o.elem_bytes;
   const unsigned box[3] = {static_cast<unsigned>(o.box_feat), 1u, (o.elem_bytes == 4 && stg_bytes < 4096) ? 16u : 32u};
-  return get_map_nd(o.ptr, et, 3, dims, strides, box, false, out);
+  // fp16 boxes are staged by stmatrix in the swizzle of their row length (32 features = 64 bytes, 16 = 32 bytes)
+  return get_map_nd(o.ptr, et, 3, dims, strides, box, eb == 2 ? o.box_feat * 2 : 0, out);
 }
 
 // ------------------------------------------------------------------------------------------------ launches
@@ -198,8 +201,10 @@ static int gemm_global_init() {
   if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
   CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
-  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   return AF_OK;
@@ -401,10 +406,19 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     // candidates, largest staging first; a smaller one is taken when it buys a pipeline stage (the main loop needs
     // ~160 KB of loads in flight), down to one 2 KB buffer per warp
     const int cand[3][2] = {{4096, 2}, {2048, 2}, {2048, 1}};
+    if (ov.elem_bytes == 2) return fail(AF_ERR_UNSUPPORTED, "GEMM outputs are fp16 or fp32");
+    p.out_bf16 = ov.elem_bytes == -2 ? 2 : 0;
+    p.part_f16 = p.out_bf16 ? 1 : 0;   // fp16 outputs take fp16 partials (both in the fragment layout), fp32 take fp32
+    if (p.out_bf16) {
+      if (ov.features % 8 || ov.ld_tok % 8 || ov.ld_mid % 8 || (reinterpret_cast<uintptr_t>(ov.ptr) & 15))
+        return fail(AF_ERR_ARG, "fp16 GEMM output needs 16-byte aligned rows (features %d, ld %lld/%lld)", ov.features, ov.ld_tok, ov.ld_mid);
+      p.out = ov.ptr; p.out_ld_tok = ov.ld_tok; p.out_ld_mid = ov.ld_mid; p.out_features = ov.features;
+    }
     int stages = 0;
-    for (int i = g_staging_first; i < 3; ++i) {
+    // (fp16 outputs: one 2 KB image per warp, read back by the warp itself - nothing asynchronous to wait for)
+    for (int i = p.out_bf16 ? 2 : g_staging_first; i < 3; ++i) {
       const int st_i = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * cand[i][0] * cand[i][1]) / stage_bytes;
-      if (st_i > stages && (stages < g_min_stages || i == g_staging_first)) { stages = st_i; p.stg_bytes = cand[i][0]; p.stg_bufs = cand[i][1]; }
+      if (st_i > stages && (stages < g_min_stages || stages == 0)) { stages = st_i; p.stg_bytes = cand[i][0]; p.stg_bufs = cand[i][1]; }
     }
     const int xch_bytes = GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs;
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
@@ -420,21 +434,22 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     rc = get_map(x, x_rows_cap, p.K, p.mma2 ? p.n1 / 2 : p.xh, &mx);
     if (rc) return rc;
     CUtensorMap mo, mp;
-    p.out_bf16 = ov.elem_bytes == 2 ? 1 : (ov.elem_bytes == -2 ? 2 : 0);
     if ((rc = get_out_map(ov, p.stg_bytes, &mo))) return rc;
-    {  // stream-K partials [slot][512 tokens][128 features], box = 32 features x 32 (or 16) tokens of one slot
+    if (p.part_f16) {
+      mp = mo;   // fp16 partials are raw 2 KB staging images [slot][32-token chunk][quadrant], written by 1-D bulk copies
+    } else {     // fp32 stream-K partials [slot][512 tokens][128 features], box = 32 features x 32 (or 16) tokens of one slot
       const unsigned long long dims[3] = {GEMM_BM, GEMM_MAX_TOK, GEMM_MAX_GRID};
-      const unsigned long long pe = p.part_f16 ? 2 : 4;
-      const unsigned long long strides[2] = {GEMM_BM * pe, GEMM_BM * pe * GEMM_MAX_TOK};
-      const unsigned box[3] = {32u, (!p.part_f16 && p.stg_bytes < 4096) ? 16u : 32u, 1u};
-      if ((rc = get_map_nd(p.partial, p.part_f16 ? -2 : 4, 3, dims, strides, box, false, &mp))) return rc;
+      const unsigned long long strides[2] = {GEMM_BM * 4ull, GEMM_BM * 4ull * GEMM_MAX_TOK};
+      const unsigned box[3] = {32u, p.stg_bytes < 4096 ? 16u : 32u, 1u};
+      if ((rc = get_map_nd(p.partial, 4, 3, dims, strides, box, 0, &mp))) return rc;
     }
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + xch_bytes + 1024;
     {
       ProfScope ps(cat, st);
       g_launch_cluster = p.cluster;
-      cudaError_t e = p.mma2 ? launch_k(gemm_tcgen05_kernel<true>, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p)
-                             : launch_k(gemm_tcgen05_kernel<false>, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
+      auto kern = p.mma2 ? (p.out_bf16 ? gemm_tcgen05_kernel<true, true> : gemm_tcgen05_kernel<true, false>)
+                         : (p.out_bf16 ? gemm_tcgen05_kernel<false, true> : gemm_tcgen05_kernel<false, false>);
+      cudaError_t e = launch_k(kern, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
       g_launch_cluster = 1;
       if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gemm_tcgen05_kernel failed: %s", cudaGetErrorString(e));
     }

@@ -24,12 +24,21 @@
 //                  [split][token][feature] and the NEXT kernel (residual + RMSNorm, elementwise.cuh) adds the slabs in
 //                  split order.  No CTA ever waits on another.
 //
-// Epilogues (features sit on TMEM lanes, tokens on columns): every warp stages its 32 features x 32 tokens in shared
-// memory and writes them with TMA tensor stores (fp16, bf16 or fp32).
+// Epilogues (features sit on TMEM lanes, tokens on columns), per warp and 32-token chunk.  The drain is bound by the
+// TMEM read port (64 B/clk per SM: 128 lanes x 288 fp32 columns = 2300 clk), so everything else is kept off its path:
+//   fp16 outputs   (every GEMM of the forward; kernel variant kFrag) tcgen05.ld.16x256b delivers the accumulator in
+//                  the mma fragment layout (thread t: feature t/4 [+8], tokens 2(t%4), +1 of every 8), which four
+//                  stmatrix.trans write as a swizzled [token][feature] image in the warp's 2 KB staging buffer; the
+//                  warp reads the image back row-wise and stores 16 bytes per lane to global memory (64 contiguous
+//                  bytes per token).  The TMEM load of the next chunk is in flight meanwhile.  No TMA store, no
+//                  proxy fence, no bulk-group wait.  Stream-K partials are the same images written raw (2 KB each)
+//                  and are added by the owner with ldmatrix.trans in the same layout.
+//   fp32 outputs   (LM head, af_debug_gemm) tcgen05.ld.32x32b, one feature per lane, staged [token][feature] in
+//                  shared memory and written with TMA tensor stores; fp32 partials likewise through map_part.
 //   EPI_STORE      plain store (q|k|v, split-K slabs, logits).
 //   EPI_SWIGLU     tile = 64 gate rows + 64 up rows of the same features, loaded so that every lane quadrant holds
-//                  16 gate + 16 up rows of the same 16 features: the pairing is a warp shuffle, the output is
-//                  fp16(silu(gate) * up).
+//                  16 gate + 16 up rows of the same 16 features: in the fragment layout gate and up of one (feature,
+//                  token) sit in the same thread (registers j and 16 + j); the output is fp16(silu(gate) * up).
 //
 // Warp roles (320 threads): warps 0-7 epilogue (TMEM lane quadrant = warp % 4, two warps per quadrant alternate
 // 32-token chunks; with bf16 weights they also run the per-tile weight transform), warp 8 TMA producer, warp 9 MMA issuer.
@@ -96,9 +105,12 @@ struct GemmParams {
   int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile
-  int out_bf16;        // EPI_STORE: 0 = fp32 output, 1 = bf16, 2 = fp16 (box 32 features x 32 tokens)
-  void* partial;       // [slot][512][128] stream-K partials, fp32 or (part_f16) fp16, written through map_part
-  int part_f16;
+  int out_bf16;        // 0 = fp32 output (TMA stores through map_out), 2 = fp16 (16-byte global stores, fields below)
+  void* out;           // fp16 output: element (feature f, middle m, token t) at out + t * out_ld_tok + m * out_ld_mid + f
+  long long out_ld_tok, out_ld_mid;
+  int out_features;    // features per middle index (multiple of 8): clips a ragged last tile
+  void* partial;       // stream-K partials: fp32 [slot][512 tokens][128 features] written through map_part, or
+  int part_f16;        // (part_f16, with fp16 outputs) raw fp16 staging images [slot][32-token chunk][lane quadrant][2 KB]
   int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
   long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr
 };

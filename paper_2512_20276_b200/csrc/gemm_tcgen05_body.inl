@@ -1,6 +1,6 @@
 // Body of gemm_tcgen05.cuh (kept in a second file only to keep each file short); see the header for the design.
 
-template <bool kMma2>
+template <bool kMma2, bool kFrag>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_constant__ CUtensorMap map_w1,
                     const __grid_constant__ CUtensorMap map_w2, const __grid_constant__ CUtensorMap map_x,
@@ -215,13 +215,23 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   } else {
     // ================================ epilogue warps 0..7 ================================
     // Warp w reads TMEM lanes [32*(w%4), +32) = 32 output features; the two warps of a quadrant alternate 32-token
-    // chunks.  Per chunk: TMEM -> registers -> the warp's private 2 KB staging buffer -> global with TMA tensor stores
-    // ([tokens][features] boxes).  No epilogue warp waits for another (except for the stream-K fix-up loads) and the
-    // LSU is not involved.  EPI_SWIGLU pairs gate and up inside the warp (lanes l and l+16) with shuffles.
+    // chunks.  Per chunk: TMEM -> registers -> the warp's private staging buffer -> global ([tokens][features] rows;
+    // 16-byte global stores for fp16 outputs, TMA tensor stores for fp32, see gemm_tcgen05.cuh).  No epilogue warp
+    // waits for another (except for the stream-K fix-up loads).
     const int quad = warp & 3, par = warp >> 2;
     const int row = quad * 32 + lane;
     const int etid = threadIdx.x;  // 0..255
     uint8_t* stg_base = reinterpret_cast<uint8_t*>(xch) + warp * (p.stg_bytes * p.stg_bufs);
+    // 16-bit outputs (every GEMM of the forward) are drained in the mma fragment layout: tcgen05.ld.16x256b gives thread
+    // t (feature t/4 [+8], tokens 2(t%4), +1 of every 8), which is what stmatrix.trans writes as [token][feature] rows.
+    // Byte offset of this lane's row address inside a staging image (token group 0; the others are + 512 bytes):
+    constexpr bool frag = kFrag;   // == (p.out_bf16 != 0), a template parameter so that each variant holds one epilogue
+    const uint32_t frag_off64 = (lane & 7) * 64 + (((lane >> 3) ^ ((lane & 7) >> 1)) << 4);   // 64-byte rows, SWIZZLE_64B
+    const uint32_t frag_off32 = ((lane >> 4) * 8 + (lane & 7)) * 32 + ((((lane >> 3) & 1) ^ ((lane & 7) >> 2)) << 4);  // 32-byte rows, SWIZZLE_32B
+    // ... and of the 16-byte piece this lane reads back and stores: token lane/4 (+ 8 per group), features 8(lane%4).. for
+    // 64-byte rows; token lane/2 (+ 16 per half), features 8(lane%2).. for the 32-byte rows of the SwiGLU output
+    const uint32_t rb_off64 = (lane >> 2) * 64 + (((lane & 3) ^ ((lane >> 3) & 3)) << 4);
+    const uint32_t rb_off32 = (lane >> 1) * 32 + (((lane & 1) ^ ((lane >> 3) & 1)) << 4);
     uint32_t n_st = 0;  // TMA stores issued by this warp; buffer = n_st & 1
     bool store_ok = true;
 #define stg (stg_base + (p.stg_bufs > 1 ? (n_st & 1) * p.stg_bytes : 0))
@@ -299,6 +309,13 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         f0 = (tile - part * p.tiles_per_part) * GEMM_BM + quad * 32;
         mid = p.split == SPLIT_K ? pc.mid : part;
       }
+      // fp16 outputs: this lane's 16-byte piece of every row it stores (EPI_STORE: token lane/4 + 8g, features
+      // 8(lane%4)..; EPI_SWIGLU: token lane/2 + 16j, features 8(lane%2)..) - pointer and guards hoisted out of the chunks
+      const int st_sh = p.epi == EPI_SWIGLU ? 1 : 2;
+      const int st_feat = f0 + 8 * (lane & ((1 << st_sh) - 1)), st_tok = lane >> st_sh;
+      const bool st_ok = frag && store_ok && st_feat < p.out_features;
+      act_t* const st_ptr = reinterpret_cast<act_t*>(p.out) + static_cast<size_t>(mid) * p.out_ld_mid + st_feat +
+                            static_cast<size_t>(p.tok0 + st_tok) * p.out_ld_tok;
       // column blocks: with contributors, their partial columns [b0, b1) are bulk-copied into the (now idle) stages,
       // all contributors at once, or (a tile cut into very many pieces) `grp` at a time over 64-column blocks
       int blk_cols = n_pad, grp = n_contrib, n_groups = n_contrib > 0 ? 1 : 0;
@@ -319,7 +336,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         fix_used = true;
         if (etid == 0) {
           const uint32_t pe = p.part_f16 ? 2 : 4;
-          const uint32_t bytes = static_cast<uint32_t>(b1 - b0) * GEMM_BM * pe;
+          const uint32_t bytes = static_cast<uint32_t>(frag ? ((b1 - b0 + 31) & ~31) : b1 - b0) * GEMM_BM * pe;
           fence_proxy_async_all();
           mbar_arrive_expect_tx(&fix_bar, bytes * cnt);
           for (int c = 0; c < cnt; ++c)
@@ -340,6 +357,14 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
         uint32_t r[32];
         const uint32_t ta = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0;
+        if (frag) {   // fragment layout: r[0..15] = lanes [0, 16) of the quadrant, r[16..31] = lanes [16, 32)
+          tmem_ld_frag32(ta, r);
+          tmem_ld_frag32(ta + (16u << 16), r + 16);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+          return;
+        }
         tmem_ld16(ta, r);
         if (cw > 16) tmem_ld16(ta + 16, r + 16);
         tmem_ld_wait();
@@ -348,85 +373,146 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       };
       auto add_fix = [&](int cnt, int b0, int b1, int c0, float* v) {
         // (a 16-wide last chunk over-reads 16 columns of the staging area; those columns are never stored)
+        if (frag) {   // fp16 images [chunk][quadrant][2 KB], read back in the layout they were written from
+          const uint32_t img0 = smem_u32(fix) + static_cast<uint32_t>(((c0 - b0) >> 5) * 4 + quad) * 2048u + frag_off64;
+          const uint32_t img_stride = static_cast<uint32_t>((b1 - b0 + 31) & ~31) * GEMM_BM * 2;
+          for (int c = 0; c < cnt; ++c) {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+              uint32_t q[4];
+              ldmatrix_x4_trans(img0 + c * img_stride + g * 512, q[0], q[1], q[2], q[3]);
+#pragma unroll
+              for (int m = 0; m < 4; ++m) {
+                const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&q[m]));
+                v[(m >> 1) * 16 + 4 * g + (m & 1) * 2] += f.x;
+                v[(m >> 1) * 16 + 4 * g + (m & 1) * 2 + 1] += f.y;
+              }
+            }
+          }
+          return;
+        }
         for (int c = 0; c < cnt; ++c) {
           const size_t e0 = (static_cast<size_t>(c) * (b1 - b0) + (c0 - b0)) * GEMM_BM + row;
 #pragma unroll
           for (int h2 = 0; h2 < 2; ++h2) {
             float t[16];
-            if (p.part_f16) {
-              const act_t* q = reinterpret_cast<const act_t*>(fix) + e0;
+            const float* q = reinterpret_cast<const float*>(fix) + e0;
 #pragma unroll
-              for (int j = 0; j < 16; ++j) t[j] = act2f(q[(h2 * 16 + j) * GEMM_BM]);
-            } else {
-              const float* q = reinterpret_cast<const float*>(fix) + e0;
-#pragma unroll
-              for (int j = 0; j < 16; ++j) t[j] = q[(h2 * 16 + j) * GEMM_BM];
-            }
+            for (int j = 0; j < 16; ++j) t[j] = q[(h2 * 16 + j) * GEMM_BM];
 #pragma unroll
             for (int j = 0; j < 16; ++j) v[h2 * 16 + j] += t[j];
           }
         }
       };
       auto finish_chunk = [&](int c0, int cw, float* v) {
-        if (contributor && p.part_f16) {   // fp16 partial [cta][token][128 features], one 32-token box
-          stage_free();
-          uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
+        if (frag && (contributor || p.epi == EPI_STORE)) {
+          // 32 features x 32 tokens as fp16: four stmatrix.trans write the warp's 2 KB staging image [token][feature]
+          // (64-byte rows, chunk-XOR swizzle), which is read back row-wise and stored with 16-byte global stores:
+          // a partial goes out as the raw image, the output as 64 contiguous bytes per token.  No TMA store, so
+          // nothing to wait for before the buffer is reused but the warp's own read-back.
+          __syncwarp();
+          const uint32_t sa = smem_u32(stg_base);
 #pragma unroll
-          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __half_as_ushort(__float2half_rn(v[j]));
-          stage_store(&map_part, quad * 32, c0, my_slot);
-        } else if (contributor || (p.epi == EPI_STORE && !p.out_bf16)) {
-          // fp32: stream-K partial [cta][token][128 features] or the fp32 output, one 32-token box per chunk (4 KB
-          // staging buffers) or two 16-token boxes (2 KB)
-          if (p.stg_bytes >= 4096) {
-            stage_free();
-            float* sb = reinterpret_cast<float*>(stg);
+          for (int g = 0; g < 4; ++g)
+            stmatrix_x4_trans(sa + frag_off64 + g * 512, pack_act(v[4 * g], v[4 * g + 1]), pack_act(v[4 * g + 2], v[4 * g + 3]),
+                              pack_act(v[16 + 4 * g], v[16 + 4 * g + 1]), pack_act(v[16 + 4 * g + 2], v[16 + 4 * g + 3]));
+          __syncwarp();
+          if (contributor) {
+            uint8_t* dst = reinterpret_cast<uint8_t*>(p.partial) +
+                           (static_cast<size_t>(my_slot) * (GEMM_MAX_TOK / 32) * 4 + (c0 >> 5) * 4 + quad) * 2048 + lane * 16;
 #pragma unroll
-            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
-            if (contributor) stage_store(&map_part, quad * 32, c0, my_slot);
-            else stage_store(&map_out, f0, mid, p.tok0 + c0);
+            for (int g = 0; g < 4; ++g)
+              if (store_ok) *reinterpret_cast<uint4*>(dst + g * 512) = lds128(sa + lane * 16 + g * 512);
           } else {
+            act_t* dst = st_ptr + static_cast<size_t>(c0) * p.out_ld_tok;
+            const int n_ok = p.T - c0 - st_tok;   // rows 8g of this lane with 8g < n_ok exist
 #pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-              if (hh * 16 < cw) {
-                stage_free();
-                float* sb = reinterpret_cast<float*>(stg);
+            for (int g = 0; g < 4; ++g)
+              if (st_ok && 8 * g < n_ok)
+                *reinterpret_cast<uint4*>(dst + static_cast<size_t>(8 * g) * p.out_ld_tok) = lds128(sa + rb_off64 + g * 512);
+          }
+        } else if (frag) {
+          // EPI_SWIGLU: lanes [0,16) of the quadrant hold gate, lanes [16,32) up of the same 16 features, so v[j] and
+          // v[16 + j] are gate and up of one (feature, token).  16 features x 32 tokens, 32-byte rows.
+          uint32_t h[8];
 #pragma unroll
-                for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = v[hh * 16 + j];
-                if (contributor) stage_store(&map_part, quad * 32, c0 + hh * 16, my_slot);
-                else stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 16);
-              }
+          for (int j = 0; j < 16; j += 2) {
+            const float g0 = v[j], g1 = v[j + 1];
+            const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * v[16 + j], h1 = __fdividef(g1, 1.f + __expf(-g1)) * v[17 + j];
+            h[j >> 1] = pack_act(fminf(fmaxf(h0, -65504.f), 65504.f), fminf(fmaxf(h1, -65504.f), 65504.f));
+          }
+          __syncwarp();
+          const uint32_t sa = smem_u32(stg_base);
+          stmatrix_x4_trans(sa + frag_off32, h[0], h[1], h[2], h[3]);          // token groups 0, 1 (features 0-7 | 8-15 each)
+          stmatrix_x4_trans(sa + frag_off32 + 512, h[4], h[5], h[6], h[7]);    // token groups 2, 3
+          __syncwarp();
+          act_t* dst = st_ptr + static_cast<size_t>(c0) * p.out_ld_tok;
+          const int n_ok = p.T - c0 - st_tok;
+#pragma unroll
+          for (int j = 0; j < 2; ++j)
+            if (st_ok && 16 * j < n_ok)
+              *reinterpret_cast<uint4*>(dst + static_cast<size_t>(16 * j) * p.out_ld_tok) = lds128(sa + rb_off32 + j * 512);
+        } else if (p.stg_bytes >= 4096) {
+          // fp32 (stream-K partial [slot][token][128 features] or the fp32 output): one 32-token box per chunk (4 KB
+          // staging buffers) or two 16-token boxes (2 KB)
+          stage_free();
+          float* sb = reinterpret_cast<float*>(stg);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = v[j];
+          if (contributor) stage_store(&map_part, quad * 32, c0, my_slot);
+          else stage_store(&map_out, f0, mid, p.tok0 + c0);
+        } else {
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            if (hh * 16 < cw) {
+              stage_free();
+              float* sb = reinterpret_cast<float*>(stg);
+#pragma unroll
+              for (int j = 0; j < 16; ++j) sb[j * 32 + lane] = v[hh * 16 + j];
+              if (contributor) stage_store(&map_part, quad * 32, c0 + hh * 16, my_slot);
+              else stage_store(&map_out, f0, mid, p.tok0 + c0 + hh * 16);
             }
           }
-        } else if (p.epi == EPI_STORE) {  // bf16 or fp16, one 32-token box
-          stage_free();
-          uint16_t* sb = reinterpret_cast<uint16_t*>(stg);
-          if (p.out_bf16 == 2) {
-#pragma unroll
-            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __half_as_ushort(__float2half_rn(v[j]));
-          } else {
-#pragma unroll
-            for (int j = 0; j < 32; ++j) sb[j * 32 + lane] = __bfloat16_as_ushort(__float2bfloat16_rn(v[j]));
-          }
-          stage_store(&map_out, f0, mid, p.tok0 + c0);
-        } else {
-          // EPI_SWIGLU: lanes 0-15 hold gate, lanes 16-31 hold up of the same 16 features.  Lanes 0-15 finish tokens
-          // 0-15 of the chunk, lanes 16-31 tokens 16-31; each gets the other half's operand with one shuffle.
-          stage_free();
-          act_t* sb = reinterpret_cast<act_t*>(stg);
-          const bool lo = lane < 16;
-#pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const float other = __shfl_xor_sync(0xffffffffu, lo ? v[j + 16] : v[j], 16);
-            const float g = lo ? v[j] : other, up = lo ? other : v[j + 16];
-            sb[(lo ? j : j + 16) * 16 + (lane & 15)] = __float2half_rn(fminf(fmaxf(__fdividef(g, 1.f + __expf(-g)) * up, -65504.f), 65504.f));
-          }
-          stage_store(&map_out, f0, mid, p.tok0 + c0);
         }
       };
       for (int b0 = 0; b0 < n_pad && b0 < p.T; b0 += blk_cols) {
         const int b1 = min(b0 + blk_cols, n_pad);
         float v[32];
-        if (n_groups <= 1) {
+        if (frag && n_groups <= 1) {
+          // software pipeline over this warp's chunks: the TMEM load of chunk i + 1 is in flight while chunk i is
+          // converted and stored (two register sets, the loop is unrolled by two so that each keeps its registers)
+          float vb[32];
+          if (n_groups == 1) {
+            load_group(0, n_contrib, b0, b1);
+            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
+          }
+          auto issue = [&](int c0, float* w) {
+            if (has_mma) {
+              const uint32_t ta = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + c0;
+              tmem_ld_frag32f(ta, w);
+              tmem_ld_frag32f(ta + (16u << 16), w + 16);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) w[j] = 0.f;
+            }
+          };
+          auto step = [&](int c0, float* cur, float* nxt) {
+            tmem_ld_wait();
+            const int cn = c0 + GEMM_BLK;
+            if (cn < b1 && cn < p.T) issue(cn, nxt);
+            if (n_groups == 1) add_fix(n_contrib, b0, b1, c0, cur);
+            finish_chunk(c0, 32, cur);
+          };
+          int c0 = b0 + 32 * par;
+          if (c0 < b1 && c0 < p.T) issue(c0, v);
+          while (c0 < b1 && c0 < p.T) {
+            step(c0, v, vb);
+            c0 += GEMM_BLK;
+            if (!(c0 < b1 && c0 < p.T)) break;
+            step(c0, vb, v);
+            c0 += GEMM_BLK;
+          }
+        } else if (n_groups <= 1) {
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
             if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
