@@ -296,9 +296,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         AF_EPI_BAR();
       }
       if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
-      if (has_mma) mbar_wait(&tmem_full_bar, acc_phase);
-      tc_fence_after();
-      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
       store_ok = tile_valid;
       // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
       int f0, mid;
@@ -475,6 +472,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           }
         }
       };
+      // (everything above is address arithmetic: done while the MMAs of this piece are still running)
+      if (has_mma) mbar_wait(&tmem_full_bar, acc_phase);
+      tc_fence_after();
+      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
       for (int b0 = 0; b0 < n_pad && b0 < p.T; b0 += blk_cols) {
         const int b1 = min(b0 + blk_cols, n_pad);
         float v[32];
