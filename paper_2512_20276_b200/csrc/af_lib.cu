@@ -547,7 +547,7 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   g->base.assign(r->n_regions, 0); g->len.assign(r->n_regions, 0);
   const long long cap_rows = static_cast<long long>(r->n_regions) * r->capacity;
   g->max_rows = static_cast<int>(cap_rows > 65536 ? 65536 : cap_rows);
-  const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 2 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1;
+  const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 4 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1;
   cudaError_t e = cudaMalloc(&g->tables, n_int * sizeof(int));
   if (e == cudaSuccess) e = cudaMalloc(&g->rope_tab, static_cast<size_t>(r->capacity) * (c->head_dim / 2) * sizeof(float2));
   if (e != cudaSuccess) { cudaFree(g->tables); delete g; return fail(AF_ERR_CUDA, "cudaMalloc: %s", cudaGetErrorString(e)); }
@@ -556,7 +556,7 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   g->tb.seg_row0 = p; p += AF_MAX_SEGS; g->tb.seg_base = p; p += AF_MAX_SEGS;
   g->tb.row_req = p; p += g->max_rows; g->tb.row_pos = p; p += g->max_rows; g->tb.row_slot = p; p += g->max_rows;
   const int max_items = g->max_rows / ATT_BQ + AF_MAX_SEGS;
-  g->tb.item_seg = p; p += max_items; g->tb.item_q0 = p; p += max_items;
+  g->tb.item_seg = p; p += max_items; g->tb.item_q0 = p; p += max_items; g->tb.item_tmp = p; p += 2 * max_items;
   g->n_items_dev = p;
   const int n = r->capacity * (c->head_dim / 2);
   rope_table_kernel<<<(n + 255) / 256, 256>>>(g->rope_tab, r->capacity, c->head_dim, static_cast<double>(c->rope_theta));
@@ -749,11 +749,11 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
               H, hd, R, C);
     // a4: segment-masked causal attention over the ring
     if (hd == 128)
-      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(n_items, H), dim3(ATT_THREADS),
+      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(H, n_items), dim3(ATT_THREADS),
                 att_smem_bytes(128), st, static_cast<const act_t*>(ws.q_rot),
                 static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     else
-      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(n_items, H), dim3(ATT_THREADS),
+      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(H, n_items), dim3(ATT_THREADS),
                 att_smem_bytes(64), st, static_cast<const act_t*>(ws.q_rot),
                 static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
     // a5: O projection, split-K slabs (added to the residual by the next kernel)

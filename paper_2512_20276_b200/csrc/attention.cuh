@@ -27,8 +27,9 @@ struct StepTables {      // device arrays written by rowmap_kernel (elementwise.
   int* row_req;          // [T]
   int* row_pos;          // [T]
   int* row_slot;         // [T] global slot id req*C + (base+pos) mod C
-  int* item_seg;         // [n_items] attention work items
+  int* item_seg;         // [n_items] attention work items, heaviest first
   int* item_q0;          // [n_items]
+  int* item_tmp;         // [2 * n_items] scratch of rowmap_kernel (the unsorted list)
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid) {
@@ -79,7 +80,7 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
 
   pdl_wait();
   pdl_launch_dependents();
-  const int item = static_cast<int>(gridDim.x) - 1 - blockIdx.x, h = blockIdx.y;  // late items see the longest ranges: first
+  const int item = blockIdx.y, h = blockIdx.x;  // items are sorted heaviest first; all heads of an item are neighbours
   const int seg = tb.item_seg[item], q0 = tb.item_q0[item];
   const int req = tb.seg_req[seg], start = tb.seg_start[seg], len = tb.seg_len[seg];
   const int row0 = tb.seg_row0[seg], base = tb.seg_base[seg];

@@ -32,7 +32,25 @@ __global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_
     tb.seg_req[s] = st.req[s]; tb.seg_start[s] = st.start[s]; tb.seg_len[s] = st.len[s];
     tb.seg_row0[s] = row0[s]; tb.seg_base[s] = st.base[s];
     const int n_it = item0[s + 1] - item0[s];
-    for (int k = 0; k < n_it; ++k) { tb.item_seg[item0[s] + k] = s; tb.item_q0[item0[s] + k] = k * ATT_BQ; }
+    for (int k = 0; k < n_it; ++k) { tb.item_tmp[2 * (item0[s] + k)] = s; tb.item_tmp[2 * (item0[s] + k) + 1] = k * ATT_BQ; }
+  }
+  __syncthreads();
+  // attention work list, heaviest first (cost = query warps x visible KV tiles): the grid is (heads, items), so the
+  // block scheduler hands every SM one heavy item before the light ones - the kernel is one wave, placement is all
+  const int n_items = item0[st.n_segs];
+  auto cost = [&](int it) {
+    const int s = tb.item_tmp[2 * it], q0 = tb.item_tmp[2 * it + 1];
+    const int nq = min(ATT_BQ, st.len[s] - q0);
+    return ((nq + 15) / 16) * ((st.start[s] + q0 + nq + ATT_BKV - 1) / ATT_BKV);
+  };
+  for (int it = threadIdx.x; it < n_items; it += blockDim.x) {
+    const int c = cost(it);
+    int rank = 0;
+    for (int j = 0; j < n_items; ++j) {
+      const int cj = cost(j);
+      rank += (cj > c || (cj == c && j < it)) ? 1 : 0;
+    }
+    tb.item_seg[rank] = tb.item_tmp[2 * it]; tb.item_q0[rank] = tb.item_tmp[2 * it + 1];
   }
   const int T = row0[st.n_segs];
   for (int i = threadIdx.x; i < T; i += blockDim.x) {
