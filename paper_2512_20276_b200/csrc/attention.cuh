@@ -128,7 +128,7 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
 
   const bool warp_active = warp * 16 < nq;
   const int p_lo = start + q0 + warp * 16 + g;   // position of this thread's first row (second = +8)
-  const int warp_pmax = start + q0 + warp * 16 + 15;
+  const int warp_pmin = start + q0 + warp * 16, warp_pmax = warp_pmin + 15;
 
   for (int tile = 0; tile < n_tiles; ++tile) {
     const int stage = tile % ATT_STAGES;
@@ -166,15 +166,27 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
       }
       // ---- causal mask within the request + online softmax (base-2 exponent) ----
       float mx[2] = {-INFINITY, -INFINITY};
+      if (j0 + ATT_BKV - 1 > warp_pmin) {   // the tile crosses the diagonal of one of the warp's rows
 #pragma unroll
-      for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
+        for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int j = j0 + nb * 8 + 2 * t + (e & 1);
-          const int p = p_lo + (e >> 1) * 8;
-          const float v = (j <= p) ? s[nb][e] * scale_log2 : -INFINITY;
-          s[nb][e] = v;
-          mx[e >> 1] = fmaxf(mx[e >> 1], v);
+          for (int e = 0; e < 4; ++e) {
+            const int j = j0 + nb * 8 + 2 * t + (e & 1);
+            const int p = p_lo + (e >> 1) * 8;
+            const float v = (j <= p) ? s[nb][e] * scale_log2 : -INFINITY;
+            s[nb][e] = v;
+            mx[e >> 1] = fmaxf(mx[e >> 1], v);
+          }
+        }
+      } else {                              // every position of the tile is visible to every row of the warp
+#pragma unroll
+        for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float v = s[nb][e] * scale_log2;
+            s[nb][e] = v;
+            mx[e >> 1] = fmaxf(mx[e >> 1], v);
+          }
         }
       }
       float alpha[2];
@@ -199,10 +211,12 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
       }
 #pragma unroll
       for (int r = 0; r < 2; ++r) l_run[r] = l_run[r] * alpha[r] + rs[r];
+      if (__any_sync(0xffffffffu, alpha[0] != 1.f || alpha[1] != 1.f)) {   // some row's running maximum moved
 #pragma unroll
-      for (int i = 0; i < HD / 8; ++i) {
-        o_acc[i][0] *= alpha[0]; o_acc[i][1] *= alpha[0];
-        o_acc[i][2] *= alpha[1]; o_acc[i][3] *= alpha[1];
+        for (int i = 0; i < HD / 8; ++i) {
+          o_acc[i][0] *= alpha[0]; o_acc[i][1] *= alpha[0];
+          o_acc[i][2] *= alpha[1]; o_acc[i][3] *= alpha[1];
+        }
       }
       // ---- O += P V ----
 #pragma unroll
