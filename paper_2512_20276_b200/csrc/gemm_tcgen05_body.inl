@@ -34,6 +34,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
 #define AF_TRACE(slot) do { if (trace) trace[slot] = static_cast<long long>(globaltimer_ns()); } while (0)
   if (trace && threadIdx.x == 0) AF_TRACE(0);
 
+  // the first use of this cluster's piece list (a dependent global load in front of the first TMA request) would cost
+  // ~0.8 us after the cluster barrier: pull its line into L1 now
+  if (lane == 0) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(p.sched + static_cast<size_t>(cl) * GEMM_MAX_PIECES));
   if (warp == GEMM_EPI_WARPS && lane == 0) {
     tma_prefetch_desc(&map_w0);
     if (p.n_parts > 1 || p.a_pair) tma_prefetch_desc(&map_w1);
