@@ -82,19 +82,31 @@ typedef struct {                 /* all device bf16 */
 
 #define AF_WEIGHTS_BF16 0         /* projection matrices are bf16; every weight tile is converted to fp16 in shared memory */
 #define AF_WEIGHTS_FP16 1         /* projection matrices were prepared once with af_convert_bf16_to_fp16 (same values) */
+#define AF_WEIGHTS_FP16_GU 2      /* as AF_WEIGHTS_FP16, and w_gate of every layer holds gate AND up, interleaved by
+                                   * af_prepare_gate_up (w_up is ignored): one TMA box per weight tile instead of eight */
 
 typedef struct {
   af_model_cfg cfg;
   const af_layer_weights* layers; /* HOST array [n_layers] of device pointers */
   const void* g_final;            /* device bf16 [d_model] */
   const void* w_lm;               /* device bf16 (or prepared fp16) [vocab, d_model] */
-  int32_t weight_format;          /* AF_WEIGHTS_BF16 or AF_WEIGHTS_FP16: format of wq..w_down and w_lm (gains stay bf16) */
+  int32_t weight_format;          /* AF_WEIGHTS_BF16, AF_WEIGHTS_FP16 or AF_WEIGHTS_FP16_GU: format of wq..w_down and w_lm (gains stay bf16) */
 } af_weights;
 
 /* Load-time weight preparation: dst[i] = fp16(src[i]) for n_elems bf16 values (n_elems % 8 == 0,
  * both device, 16-byte aligned, may not overlap).  Exact for every finite bf16 value with 2^-14 <= |w| <= 65504; smaller
  * values round to fp16 subnormals (absolute error <= 2^-25).  Enqueued on cuda_stream. */
 int af_convert_bf16_to_fp16(const void* src_bf16, void* dst_fp16, size_t n_elems, void* cuda_stream);
+
+/* Load-time preparation of the MLP input projections for AF_WEIGHTS_FP16_GU: converts gate and up ([ffn, d_model]
+ * bf16, device) to fp16 like af_convert_bf16_to_fp16 and writes them as ONE matrix dst_fp16 of
+ * af_gate_up_rows(ffn) x d_model in the row order the SwiGLU epilogue wants (h = silu(gate) * up): for
+ * every tile t of 64 features and every quarter q of it, 16 gate rows (features 64t + 16q ..) followed by the 16 up
+ * rows of the same features; rows of features >= ffn are zero.  dst_fp16 is caller-owned (device, 16-byte aligned,
+ * d_model % 8 == 0).  Enqueued on cuda_stream. */
+size_t af_gate_up_rows(int32_t ffn);
+int af_prepare_gate_up(const void* gate_bf16, const void* up_bf16, void* dst_fp16, int32_t ffn, int32_t d_model,
+                       void* cuda_stream);
 
 /* Bytes of kv_mem needed for (cfg, ring): 2 * n_layers * R * n_heads * C * head_dim * 2. */
 size_t af_ring_bytes(const af_model_cfg* cfg, const af_ring_cfg* ring);

@@ -48,7 +48,7 @@ class af_weights(C.Structure):
                 ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
 
 
-EXPORTS = ["af_convert_bf16_to_fp16", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+EXPORTS = ["af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
@@ -74,6 +74,10 @@ def load_library():
     L.af_workspace_bytes.argtypes = [C.POINTER(af_model_cfg), i32, i32]
     L.af_convert_bf16_to_fp16.argtypes = [vp, vp, sz, vp]
     L.af_convert_bf16_to_fp16.restype = C.c_int
+    L.af_gate_up_rows.argtypes = [C.c_int32]
+    L.af_gate_up_rows.restype = C.c_size_t
+    L.af_prepare_gate_up.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp]
+    L.af_prepare_gate_up.restype = C.c_int
     L.af_ring_create.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg), vp, sz, C.POINTER(vp)]
     L.af_ring_reset_slot.argtypes = [vp, i32, i32]
     L.af_packed_forward.argtypes = [C.POINTER(af_weights), vp, C.POINTER(af_segment), i32, vp, vp, vp, sz, vp]
@@ -115,8 +119,10 @@ def _stream_ptr(stream=None):
 
 class Weights:
     """Device copies of the bf16 weights + the af_weights struct pointing at them.  With prepared=True (default) the
-    projection matrices are rewritten once, on the device, as fp16 by af_convert_bf16_to_fp16 (AF_WEIGHTS_FP16: the
-    same values, no per-tile conversion in the GEMM); prepared=False keeps them bf16 (AF_WEIGHTS_BF16)."""
+    projection matrices are rewritten once, on the device, as fp16 by af_convert_bf16_to_fp16 and gate | up are
+    interleaved by af_prepare_gate_up (AF_WEIGHTS_FP16_GU: the same values, no per-tile conversion in the GEMM, one
+    TMA box per gate/up tile); prepared="fp16" converts only (AF_WEIGHTS_FP16); prepared=False keeps them bf16
+    (AF_WEIGHTS_BF16)."""
 
     def __init__(self, cfg, host_weights: dict, device="cuda", prepared=True):
         self.cfg = cfg
@@ -125,14 +131,26 @@ class Weights:
         self._layers = (af_layer_weights * cfg.n_layers)()
         for l, L in enumerate(host_weights["layers"]):
             for name, _ in af_layer_weights._fields_:
+                if prepared is True and name in ("w_gate", "w_up"):
+                    continue
                 t = self._prep(L[name].to(torch.bfloat16).contiguous().to(device), name.startswith("w"))
                 self.tensors.append(t)
                 setattr(self._layers[l], name, t.data_ptr())
+            if prepared is True:
+                gate = L["w_gate"].to(torch.bfloat16).contiguous().to(device)
+                up = L["w_up"].to(torch.bfloat16).contiguous().to(device)
+                lib = load_library()
+                gu = torch.empty(lib.af_gate_up_rows(cfg.ffn), cfg.d_model, dtype=torch.float16, device=device)
+                _check(lib.af_prepare_gate_up(gate.data_ptr(), up.data_ptr(), gu.data_ptr(), cfg.ffn, cfg.d_model, _stream_ptr()))
+                torch.cuda.synchronize()
+                self.tensors.append(gu)
+                self._layers[l].w_gate = gu.data_ptr()
+                self._layers[l].w_up = gu.data_ptr()
         self.g_final = host_weights["g_final"].to(torch.bfloat16).contiguous().to(device)
         self.w_lm = self._prep(host_weights["w_lm"].to(torch.bfloat16).contiguous().to(device), True)
         torch.cuda.synchronize()
         self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr(),
-                                 1 if prepared else 0)
+                                 2 if prepared is True else (1 if prepared else 0))
 
     def _prep(self, t: torch.Tensor, is_matrix: bool) -> torch.Tensor:
         if not (self.prepared and is_matrix):

@@ -385,7 +385,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     int n_pad = (Tc + 15) / 16 * 16;
     if (n_pad <= 256) { p.n1 = n_pad; p.n2 = 0; }
     else { p.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; p.n2 = p.n1; n_pad = 2 * p.n1; }
-    const int box_rows = p.a_pair ? 16 : GEMM_BM;
+    const int box_rows = p.a_pair == 1 ? 16 : GEMM_BM;
     const int n_tiles = p.a_pair ? (p.part_rows + 63) / 64 : p.n_parts * ((p.part_rows + GEMM_BM - 1) / GEMM_BM);
     p.tiles_per_part = (p.part_rows + GEMM_BM - 1) / GEMM_BM;
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
@@ -427,8 +427,8 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     if (g_trace) { p.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * 32; g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {cat, grid}; ++g_trace_n; }
     CUtensorMap mw[3], mx;
     for (int i = 0; i < 3; ++i) {
-      const int n_w = p.a_pair ? 2 : p.n_parts;
-      rc = get_map(w[i < n_w ? i : 0], p.part_rows, p.K, box_rows, &mw[i]);
+      const int n_w = p.a_pair == 1 ? 2 : (p.a_pair == 2 ? 1 : p.n_parts);
+      rc = get_map(w[i < n_w ? i : 0], p.a_pair == 2 ? n_tiles * GEMM_BM : p.part_rows, p.K, box_rows, &mw[i]);
       if (rc) return rc;
     }
     rc = get_map(x, x_rows_cap, p.K, p.mma2 ? p.n1 / 2 : p.xh, &mx);
@@ -620,6 +620,19 @@ extern "C" int af_convert_bf16_to_fp16(const void* src, void* dst, size_t n, voi
   return check_launch("convert_bf16_to_fp16_kernel");
 }
 
+extern "C" size_t af_gate_up_rows(int32_t ffn) { return ffn > 0 ? static_cast<size_t>((ffn + 63) / 64) * GEMM_BM : 0; }
+
+extern "C" int af_prepare_gate_up(const void* gate, const void* up, void* dst, int32_t ffn, int32_t d_model, void* cuda_stream) {
+  if (!gate || !up || !dst || ffn <= 0 || d_model <= 0 || (d_model % 8)) return fail(AF_ERR_ARG, "null pointer, or d_model not a multiple of 8");
+  if ((reinterpret_cast<uintptr_t>(gate) | reinterpret_cast<uintptr_t>(up) | reinterpret_cast<uintptr_t>(dst)) & 15)
+    return fail(AF_ERR_ARG, "pointers must be 16-byte aligned");
+  const int vec_per_row = d_model / 8;
+  const size_t n_vec = af_gate_up_rows(ffn) * vec_per_row;
+  interleave_gate_up_kernel<<<static_cast<unsigned>((n_vec + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(
+      reinterpret_cast<const uint4*>(gate), reinterpret_cast<const uint4*>(up), reinterpret_cast<uint4*>(dst), ffn, vec_per_row, n_vec);
+  return check_launch("interleave_gate_up_kernel");
+}
+
 extern "C" int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters,
                                       int32_t splits, int32_t* pieces, int32_t max_clusters_out) {
   if (!pieces) return fail(AF_ERR_ARG, "null output");
@@ -646,8 +659,8 @@ static int check_weights(const af_weights* w, bool need_lm) {
       return fail(AF_ERR_ARG, "null weight pointer in layer %d", l);
   }
   if (need_lm && (!w->g_final || !w->w_lm)) return fail(AF_ERR_ARG, "null g_final / w_lm");
-  if (w->weight_format != AF_WEIGHTS_BF16 && w->weight_format != AF_WEIGHTS_FP16)
-    return fail(AF_ERR_ARG, "weight_format %d is neither AF_WEIGHTS_BF16 nor AF_WEIGHTS_FP16", w->weight_format);
+  if (w->weight_format != AF_WEIGHTS_BF16 && w->weight_format != AF_WEIGHTS_FP16 && w->weight_format != AF_WEIGHTS_FP16_GU)
+    return fail(AF_ERR_ARG, "weight_format %d is not AF_WEIGHTS_BF16, AF_WEIGHTS_FP16 or AF_WEIGHTS_FP16_GU", w->weight_format);
   return AF_OK;
 }
 
@@ -720,7 +733,8 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
               reinterpret_cast<const __nv_bfloat16*>(packed_embeds), hidden_out, n);
   }
   const int row_threads = row_threads_for(D);
-  const int wfmt = w->weight_format == AF_WEIGHTS_FP16;
+  const int wfmt = w->weight_format == AF_WEIGHTS_FP16 || w->weight_format == AF_WEIGHTS_FP16_GU;
+  const bool gu_packed = w->weight_format == AF_WEIGHTS_FP16_GU;
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   const long long split_stride = static_cast<long long>(ws.max_rows) * D;
@@ -772,10 +786,10 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     // a7: gate/up projection with the fused SiLU*mul epilogue
     {
       GemmParams gp{};
-      gp.part_f16 = 1; gp.w_fp16 = wfmt; gp.n_parts = 2; gp.part_rows = F; gp.a_pair = 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
+      gp.part_f16 = 1; gp.w_fp16 = wfmt; gp.n_parts = 2; gp.part_rows = F; gp.a_pair = gu_packed ? 2 : 1; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_SWIGLU;
       gp.partial = ws.partial;
       const OutView ov{ws.h, -2, F, 1, T, F, F, 16};
-      const void* wgu[3] = {L.w_gate, L.w_up, nullptr};
+      const void* wgu[3] = {L.w_gate, gu_packed ? L.w_gate : L.w_up, nullptr};
       if ((rc = launch_gemm(PC_GEMM_GATEUP, st, gp, ov, ws.xn, ws.max_rows, wgu, T))) return rc;
     }
     // a8: down projection, split-K slabs
@@ -823,7 +837,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   }
   if ((rc = check_launch("gather_norm_kernel"))) return rc;
   GemmParams gp{};
-  gp.w_fp16 = w->weight_format == AF_WEIGHTS_FP16;
+  gp.w_fp16 = w->weight_format != AF_WEIGHTS_BF16;
   gp.n_parts = 1; gp.part_rows = c.vocab; gp.K = c.d_model; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
   gp.partial = ws.partial;
   if (c.vocab % 4) return fail(AF_ERR_UNSUPPORTED, "vocab must be a multiple of 4 (16-byte logits rows)");

@@ -215,6 +215,22 @@ __global__ void convert_bf16_to_fp16_kernel(const uint4* __restrict__ src, uint4
   dst[i] = v;
 }
 
+// Load-time preparation of gate | up (af_prepare_gate_up): dst row t*128 + q*32 + half*16 + i = fp16 of row
+// 64t + 16q + i of gate (half 0) or up (half 1); zero rows past F.  8 elements per thread.
+__global__ void interleave_gate_up_kernel(const uint4* __restrict__ gate, const uint4* __restrict__ up, uint4* __restrict__ dst,
+                                          int F, int vec_per_row, size_t n_vec) {
+  const size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n_vec) return;
+  const int row = static_cast<int>(i / vec_per_row), c = static_cast<int>(i - static_cast<size_t>(row) * vec_per_row);
+  const int t = row >> 7, q = (row >> 5) & 3, half = (row >> 4) & 1, f = t * 64 + q * 16 + (row & 15);
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (f < F) {
+    v = (half ? up : gate)[static_cast<size_t>(f) * vec_per_row + c];
+    v.x = bf16x2_to_f16x2(v.x); v.y = bf16x2_to_f16x2(v.y); v.z = bf16x2_to_f16x2(v.z); v.w = bf16x2_to_f16x2(v.w);
+  }
+  dst[i] = v;
+}
+
 // RoPE table in fp64: tab[pos][c] = (cos, sin)(pos * theta^(-2c/hd))
 __global__ void rope_table_kernel(float2* tab, int C, int hd, double theta) {
   const int half = hd / 2;

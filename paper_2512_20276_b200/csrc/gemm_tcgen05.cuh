@@ -90,7 +90,8 @@ struct GemmParams {
   int n_parts;         // weight matrices stacked along the feature axis (q|k|v): 1..3 (when a_pair == 0)
   int part_rows;       // output features per part (a_pair: rows of gate = rows of up)
   int tiles_per_part;  // ceil(part_rows / 128)
-  int a_pair;          // 1: tile t = rows [64t, 64t+64) of map_w0 (gate) and of map_w1 (up), interleaved 16 + 16 per lane quadrant
+  int a_pair;          // 2: map_w0 holds gate | up interleaved at load time (af_prepare_gate_up), tile t = its rows [128t, +128);
+                       // 1: tile t = rows [64t, 64t+64) of map_w0 (gate) and of map_w1 (up), interleaved 16 + 16 per lane quadrant
   int K, num_kb;       // reduction length, ceil(K / 64)
   int T, tok0;         // valid tokens of this launch, first token row
   int n1, n2;          // UMMA N of the two token halves (multiples of 16, n2 may be 0)

@@ -39,7 +39,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   if (lane == 0) asm volatile("prefetch.global.L1 [%0];\n" ::"l"(p.sched + static_cast<size_t>(cl) * GEMM_MAX_PIECES));
   if (warp == GEMM_EPI_WARPS && lane == 0) {
     tma_prefetch_desc(&map_w0);
-    if (p.n_parts > 1 || p.a_pair) tma_prefetch_desc(&map_w1);
+    if (p.n_parts > 1 || p.a_pair == 1) tma_prefetch_desc(&map_w1);
     if (p.n_parts > 2) tma_prefetch_desc(&map_w2);
     tma_prefetch_desc(&map_x);
     tma_prefetch_desc(&map_out);
@@ -87,7 +87,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       auto set_tile = [&]() {
         const int tile = min(l_pair * p.cluster + crank, p.n_tiles - 1);  // (an odd tile count: reload the last)
         if (p.a_pair) {
-          l_row = tile * 64;
+          l_row = tile * (p.a_pair == 2 ? GEMM_BM : 64);   // (2: gate | up interleaved at load time, 128 rows per tile)
         } else {
           const int part = tile / p.tiles_per_part;
           l_mw = part == 0 ? &map_w0 : (part == 1 ? &map_w1 : &map_w2);
@@ -109,7 +109,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       auto load_w = [&](int stage) {
         uint8_t* sa = tiles + static_cast<size_t>(stage) * stage_bytes;
         const int kc = l_kb * GEMM_BK;
-        if (p.a_pair) {  // every TMEM lane quadrant = 16 gate rows + the 16 up rows of the same features
+        if (p.a_pair == 1) {  // every TMEM lane quadrant = 16 gate rows + the 16 up rows of the same features
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             if (mma2) {

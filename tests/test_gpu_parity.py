@@ -180,18 +180,20 @@ def test_cfg2_single_7b_layer(binding):
 
 
 def test_bf16_weight_path_equals_prepared_fp16_path(binding):
-    """AF_WEIGHTS_BF16 (every weight tile converted bf16 -> fp16 in shared memory by the GEMM) and AF_WEIGHTS_FP16
-    (matrices prepared once by af_convert_bf16_to_fp16) hold the same values, so the two paths agree bit for bit."""
+    """AF_WEIGHTS_BF16 (every weight tile converted bf16 -> fp16 in shared memory by the GEMM), AF_WEIGHTS_FP16
+    (matrices prepared once by af_convert_bf16_to_fp16) and AF_WEIGHTS_FP16_GU (gate | up also interleaved once by
+    af_prepare_gate_up; ffn = 688 leaves a ragged last tile) hold the same values, so the paths agree bit for bit."""
     cfg = I.CFG_TINY
     hw = I.make_weights(cfg, seed=0)
     e = I.make_embeds(cfg, 0, 7, 100).cuda()
     outs = []
-    for prepared in (True, False):
+    for prepared in (True, "fp16", False):
         W = binding.Weights(cfg, hw, prepared=prepared)
         ring = binding.Ring(cfg, 4, 128, max_rows=128)
         hid = ring.packed_forward(W, e, [(0, 0, 0, 60), (3, 0, 0, 40)])
         outs.append((hid.clone(), ring.logits_rows(W, hid, [59, 99]).clone()))
-    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    for o in outs[1:]:
+        assert torch.equal(outs[0][0], o[0]) and torch.equal(outs[0][1], o[1])
     w = (0.02 * torch.randn(256, 512)).to(torch.bfloat16).cuda()
     w16 = torch.empty(256, 512, dtype=torch.float16, device="cuda")
     L = binding.load_library()
