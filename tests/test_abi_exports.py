@@ -50,3 +50,4 @@ def test_host_helpers_need_no_gpu():
     r = binding.af_ring_cfg(8, 512)
     assert L.af_ring_bytes(ctypes.byref(c), ctypes.byref(r)) == 2 * 32 * 8 * 32 * 512 * 128 * 2
     assert L.af_workspace_bytes(ctypes.byref(c), 288, 8) > 288 * (4096 * 6 + 3 * 11008) * 2
+    assert L.af_gate_up_rows(11008) == 172 * 128 and L.af_gate_up_rows(688) == 11 * 128 and L.af_gate_up_rows(0) == 0

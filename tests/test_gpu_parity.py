@@ -202,3 +202,26 @@ def test_bf16_weight_path_equals_prepared_fp16_path(binding):
     big = w.float().abs() >= 2.0 ** -14
     assert torch.equal(w16.float()[big], w.float()[big])                   # exact in the fp16 normal range
     assert float((w16.float() - w.float()).abs().max()) <= 2.0 ** -25        # fp16 subnormals below it
+
+
+def test_prepare_gate_up_layout(binding):
+    """af_prepare_gate_up: row t*128 + q*32 + half*16 + i of the packed matrix = row 64t + 16q + i of gate (half 0) or
+    up (half 1), converted to fp16; rows of features >= ffn are zero (ffn = 688 leaves a 48-feature last tile).
+    Bit-exact (index work)."""
+    F, D = 688, 256
+    g = torch.Generator().manual_seed(11)
+    gate = (0.05 * torch.randn(F, D, generator=g)).to(torch.bfloat16)
+    up = (0.05 * torch.randn(F, D, generator=g)).to(torch.bfloat16)
+    L = binding.load_library()
+    rows = L.af_gate_up_rows(F)
+    assert rows == 128 * ((F + 63) // 64)
+    out = torch.full((rows, D), 7.0, dtype=torch.float16, device="cuda")
+    assert L.af_prepare_gate_up(gate.cuda().data_ptr(), up.cuda().data_ptr(), out.data_ptr(), F, D, None) == 0
+    torch.cuda.synchronize()
+    ref = torch.zeros(rows, D, dtype=torch.float16)
+    for r in range(rows):
+        t, q, half, i = r >> 7, (r >> 5) & 3, (r >> 4) & 1, r & 15
+        f = 64 * t + 16 * q + i
+        if f < F:
+            ref[r] = (up if half else gate)[f].to(torch.float16)
+    assert torch.equal(out.cpu(), ref)
