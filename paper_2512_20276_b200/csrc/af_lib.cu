@@ -156,6 +156,8 @@ static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
 static bool g_use_pdl = true;
 static int g_staging_first = 0;   // AF_STAGING=0/1/2: first epilogue staging candidate tried (2x4 KB, 2x2 KB, 1x2 KB)
+static int g_w_pre = 3;           // AF_WPRE: weight stages requested before griddepcontrol.wait (measured: 3 beats all 6 by 0.6 % -
+                                  // a resident CTA's prefetch competes for HBM with the tail of the kernel it is waiting for)
 static int g_min_stages = 5;      // AF_MIN_STAGES: shrink the staging until the ring has this many stages
 static int g_gemm_mma2 = 1;      // AF_MMA2=0: keep cta_group::1 MMAs (with multicast) in the 2-CTA clusters
 static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
@@ -197,6 +199,7 @@ static int gemm_global_init() {
   if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
   if (const char* e = getenv("AF_STAGING")) g_staging_first = atoi(e) < 0 ? 0 : (atoi(e) > 2 ? 2 : atoi(e));
   if (const char* e = getenv("AF_MIN_STAGES")) g_min_stages = atoi(e);
+  if (const char* e = getenv("AF_WPRE")) g_w_pre = atoi(e);
   if (const char* e = getenv("AF_MMA2")) g_gemm_mma2 = atoi(e) != 0;
   if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
   CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
@@ -424,6 +427,7 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
     if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
     p.stages = stages; p.flags = g_flags;
+    p.w_pre = g_w_pre < stages ? g_w_pre : stages;
     if (g_trace) { p.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * 32; g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {cat, grid}; ++g_trace_n; }
     CUtensorMap mw[3], mx;
     for (int i = 0; i < 3; ++i) {

@@ -103,6 +103,7 @@ struct GemmParams {
   int splits;          // SPLIT_K: pieces per tile
   const GemmPiece* sched;  // device: [clusters][GEMM_MAX_PIECES] pieces, ended by pair = -1
   int stages;
+  int w_pre;           // weight tiles (pipeline stages) requested before griddepcontrol.wait
   int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile

@@ -142,10 +142,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           tma_load_2d(sb + half, &map_x, &full_bar[stage], kb * GEMM_BK, p.tok0 + p.xh, pol_x);
         }
       };
-      // The weights do not depend on the previous kernel: start streaming them before the PDL dependency resolves.
+      // The weights do not depend on the previous kernel: start streaming the first p.w_pre stages before the PDL
+      // dependency resolves (not all of them: the previous kernel's last CTAs still need the memory system).
       int n_pre = 0;
       int kb_pre[GEMM_MAX_STAGES];
-      while (n_pre < p.stages && l_more) {
+      while (n_pre < p.w_pre && l_more) {
         if (!mma2) mbar_arrive_expect_tx(&full_bar[n_pre], stage_bytes);
         else if (crank == 0) mbar_arrive_expect_tx(&full_bar[n_pre], 2 * stage_bytes);
         load_w(n_pre);
