@@ -225,3 +225,20 @@ def test_prepare_gate_up_layout(binding):
         if f < F:
             ref[r] = (up if half else gate)[f].to(torch.float16)
     assert torch.equal(out.cpu(), ref)
+
+
+@pytest.mark.parametrize("n_prefill", [257, 300, 513])
+def test_wide_packed_steps_tiny(binding, n_prefill):
+    """Packed steps wider than one UMMA N (two accumulator halves: 257, 300 rows) and wider than one GEMM launch (513
+    rows: two token chunks) on the tiny model, whose ffn = 688 leaves a ragged SwiGLU tile: a long prefill that wraps
+    its region, packed with decode rows of three other requests."""
+    cfg = I.CFG_TINY
+    hw = I.make_weights(cfg, seed=5)
+    R, C = 4, 640
+    P = Pair(cfg, hw, R=R, C=C, max_rows=640, bases=[600, 0, 17, 639])
+    for r in (1, 2, 3):
+        P.step([(r, 0, 0, 20 + r)], I.make_embeds(cfg, 5, r, 20 + r))
+    segs = [(0, 0, 0, n_prefill)] + [(r, 1, 20 + r, 1) for r in (1, 2, 3)]
+    hid, ref = P.step(segs, I.make_embeds(cfg, 5, 9, n_prefill + 3))
+    P.check_ring([0, 1, 2, 3])
+    P.check_logits(hid, ref, I.prediction_rows(segs))
