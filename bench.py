@@ -158,18 +158,23 @@ def run_sweep(args):
     cfg = I.cfg_7b_layers(args.layers)
     hw = I.make_weights(cfg, 4, threads=max(4, os.cpu_count() or 8))
     W = binding.Weights(cfg, hw)
-    Rr, Cc = 17, 1024
+    # --chunks: SURVEY.md 8(f) row f2, the paper's longer action chunks (section 4.3, Fig. 5): K - 1 decode segments
+    # ride on one 276-row prefill, K in {7, 16, 24, 32}; decode j's history is the first 276 + j rows of H as in cfg5
+    max_dec = 31 if args.chunks else 15
+    Rr, Cc = max_dec + 2, 1024 if not args.chunks else 512
     ring = binding.Ring(cfg, Rr, Cc, max_rows=544)
-    H = I.make_embeds(cfg, 4, 1, 291).cuda()
+    H = I.make_embeds(cfg, 4, 1, 276 + max_dec).cuda()
     E = I.make_embeds(cfg, 4, 0, 512).cuda()
-    for j in range(15):
+    for j in range(max_dec):
         ring.packed_forward(W, H[:276 + j].contiguous(), [(j + 1, 0, 0, 276 + j)])
     peaks = load_peaks()
     hidden = torch.empty(544, cfg.d_model, dtype=torch.float32, device="cuda")
     print("| decodes | prefill | T | ms/step | packed tok/s | HBM GB/s (algorithmic) | TFLOP/s | roofline ms (measured peaks) | frac |")
     print("|---|---|---|---|---|---|---|---|---|")
-    for n_dec in (0, 1, 3, 6, 10, 15):
-        for p_len in (0, 128, 276, 512):
+    grid = [(n, 276) for n in (6, 15, 23, 31)] if args.chunks else \
+           [(n, p) for n in (0, 1, 3, 6, 10, 15) for p in (0, 128, 276, 512)]
+    for n_dec, p_len in grid:
+        if True:
             if n_dec == 0 and p_len == 0:
                 continue
             segs, rows = [], []
@@ -181,7 +186,7 @@ def run_sweep(args):
 
             def one():
                 ring.reset_slot(0, 0)
-                for j in range(15):
+                for j in range(max_dec):
                     ring.set_len(j + 1, 276 + j)
                 ring.packed_forward(W, x, segs, hidden_out=hidden[:x.shape[0]])
             for _ in range(3):
@@ -210,10 +215,11 @@ def main():
     ap.add_argument("--layers", type=int, default=32, help="debug only: fewer layers (the line then says so)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
+    ap.add_argument("--chunks", action="store_true", help="with --sweep: the longer-action-chunk points K = 7, 16, 24, 32 (276-row prefill + K - 1 decodes)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    if args.sweep:
+    if args.sweep or args.chunks:
         return run_sweep(args)
 
     import torch

@@ -103,6 +103,34 @@ def test_cfg5_scheduling_shape_sweep(binding, w7b):
     print(f"cfg5: worst hidden {worst:.3e} over {len(points) - 1} grid points")
 
 
+def test_f2_longer_action_chunks(binding, w7b):
+    """SURVEY.md 8(f) f2 (the paper's section 4.3 / Fig. 5 workload): K - 1 = 15, 23, 31 decode segments of K - 1
+    different in-flight requests (contexts 277 .. 276 + K - 1) packed with one 276-row prefill, R = 33 regions.  Same
+    oracle trick as cfg5: decode j's history is the first 276 + j rows of one stream H, so one 307-row oracle forward of
+    H and one 276-row forward of E give every expected row."""
+    cfg, hw, W = w7b
+    max_dec = 31
+    E = I.make_embeds(cfg, 6, 0, 276)
+    H = I.make_embeds(cfg, 6, 1, 276 + max_dec)
+    orc = O.Oracle(cfg, hw, torch.float32)
+    ref_E = orc.step([(0, 0, 0, 276)], E)
+    ref_H = orc.step([(1, 0, 0, 276 + max_dec)], H)
+    ring = binding.Ring(cfg, max_dec + 2, 512, max_rows=320)
+    for j in range(max_dec):
+        ring.packed_forward(W, H[:276 + j].cuda().contiguous(), [(j + 1, 0, 0, 276 + j)])
+    for n_dec in (15, 23, 31):
+        ring.reset_slot(0, 0)
+        for j in range(max_dec):
+            ring.set_len(j + 1, 276 + j)
+        segs = [(0, 0, 0, 276)] + [(j + 1, 1, 276 + j, 1) for j in range(n_dec)]
+        x = torch.cat([E] + [H[276 + j:277 + j] for j in range(n_dec)])
+        hid = ring.packed_forward(W, x.cuda().contiguous(), segs)
+        ref = torch.cat([ref_E] + [ref_H[276 + j:277 + j] for j in range(n_dec)])
+        err = relmax(hid, ref)
+        print(f"f2: K = {n_dec + 1}: hidden {err:.3e}")
+        assert err <= TOL, f"K={n_dec + 1}: {err:.3e}"
+
+
 def _cfg4_schedule(rng, Cc, n_req):
     """Deterministic scheduler of BASELINE.json configs[3]: chunked prefills (U{128..512}, <= 4 chunks per step) until
     len = 1015, then one decode token per step up to len = 1023."""
