@@ -290,6 +290,25 @@ def main():
     ev3.record(stream)
     barrier()
     ms_e2e = ev2.elapsed_time(ev3)
+    # ---- timed region 3: the same loop closed on the device - the decode rows of step t + 1 are
+    #      af_embed_rows(af_argmax_rows(logits of step t)); only the prefill rows come from the host and only the 7
+    #      tokens go back.  The embedding table is synthetic (seeded), like every other input. ----
+    table = (0.5 * torch.randn(cfg.vocab, cfg.d_model, generator=torch.Generator().manual_seed(SEED + 7))).to(torch.bfloat16).cuda()
+    tokens = torch.zeros(K_STAGES, dtype=torch.int32, device="cuda")
+    tokens_host = torch.empty(K_STAGES, dtype=torch.int32).pin_memory()
+    for timed in (False, True):
+        barrier()
+        ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev4.record(stream)
+        for _ in range(args.steps if timed else 3):
+            e_stage[:L_P].copy_(e_host[tau[0] % n_buf][:L_P], non_blocking=True)   # H2D: the new frame's prefill rows
+            binding.embed_rows(table, tokens[:K_STAGES - 1], out=e_stage[L_P:T])   # decode rows: last tokens, on device
+            step(e_stage)
+            tokens.copy_(binding.argmax_rows(logits))
+            tokens_host.copy_(tokens, non_blocking=True)                           # D2H: 7 action tokens
+        ev5.record(stream)
+        barrier()
+    ms_loop = ev4.elapsed_time(ev5)
     # ---- per-kernel-class events (separate pass; same steps) ----
     n_prof = min(20, args.steps)
     binding.profile(True)
@@ -299,7 +318,7 @@ def main():
     binding.profile(False)
     clocks = sampler.stop()
 
-    ms_dev, ms_e2e = replicas.max_over_ranks([ms_dev, ms_e2e], device="cuda")
+    ms_dev, ms_e2e, ms_loop = replicas.max_over_ranks([ms_dev, ms_e2e, ms_loop], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -342,6 +361,9 @@ def main():
         "kernel_ms_per_step": {k: v[0] / n_prof for k, v in prof.items()},
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": T * cfg.d_model * 2,
                 "d2h_bytes_per_step": K_STAGES * cfg.vocab * 4},
+        "e2e_device_loop": {"value": replicas.whole_job_throughput(args.steps, ms_loop), "unit": "frames/s",
+                            "what": "f1: decode rows = af_embed_rows(af_argmax_rows(previous logits)) on the device",
+                            "h2d_bytes_per_step": L_P * cfg.d_model * 2, "d2h_bytes_per_step": K_STAGES * 4},
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline:

@@ -138,6 +138,21 @@ int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_s
 int af_logits_rows(const af_weights* w, const float* hidden, const int32_t* rows, int32_t n_rows,
                    float* logits_out, void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* ---- the device half of Alg. 1's loop around the forward ----
+ * tokens_out[i] = ArgMax_v logits[i, v]  (Alg. 1 l.5 / l.8 "ArgMax(LMHead(Norm(H[s])))").  Ties go to the LOWEST index;
+ * NaN entries are never selected (a row of only NaNs gives 0).  An integer decided by floating point: it is taken on
+ * the fp32 logits exactly as stored, so any implementation given the same logits returns the same tokens.
+ *   logits : device fp32 [n_rows, vocab] (row pitch = vocab);  tokens_out : device int32 [n_rows].  Enqueued. */
+int af_argmax_rows(const float* logits, int32_t n_rows, int32_t vocab, int32_t* tokens_out, void* cuda_stream);
+
+/* embeds_out[i, :] = table[tokens[i], :]  (the token half of Alg. 1 l.2 "Embed(.., GetLastTokenEach(A_sequences))",
+ * P:134): the rows a step's decode segments take as input.  A copy, bit-exact.
+ *   table : device bf16 [vocab, d_model] (d_model % 8 == 0, 16-byte aligned);  tokens : device int32 [n_rows], each in
+ *   [0, vocab) (a token outside the range writes a row of zeros);  embeds_out : device bf16 [n_rows, d_model],
+ *   typically rows of the next step's packed_embeds.  Enqueued. */
+int af_embed_rows(const void* table, int32_t vocab, int32_t d_model, const int32_t* tokens, int32_t n_rows,
+                  void* embeds_out, void* cuda_stream);
+
 int af_ring_destroy(af_ring* ring); /* frees the handle and its own metadata; never frees caller memory */
 
 /* ---- introspection for bit-exact bookkeeping parity; these synchronise, they are not hot path ---- */

@@ -241,3 +241,27 @@ def ring_reset_model(C: int, base: int, length: int, new_base: int):
     if new_base >= 0:
         return new_base % C, 0
     return (base + length) % C, 0
+
+
+def argmax_rows(logits) -> list:
+    """Alg. 1 l.5 / l.8 "ArgMax(LMHead(Norm(H[s])))" as the plain definition, one scalar loop per row:
+    the LOWEST index whose value is the row maximum; NaN entries are never selected (a row of only NaNs gives 0).
+    The decision is taken on the logits exactly as given (fp32), which is the precision the library decides in."""
+    out = []
+    for row in logits.tolist():
+        best, best_i = float("-inf"), -1
+        for i, v in enumerate(row):
+            if v > best or (v == best and best_i < 0):
+                best, best_i = v, i
+        out.append(max(best_i, 0))
+    return out
+
+
+def embed_rows(table: torch.Tensor, tokens) -> torch.Tensor:
+    """The token half of Alg. 1 l.2 "Embed(.., GetLastTokenEach(A_sequences))": row i = table[tokens[i]]
+    (a token outside the table gives a row of zeros, as the library documents)."""
+    out = torch.zeros(len(tokens), table.shape[1], dtype=table.dtype)
+    for i, t in enumerate(tokens):
+        if 0 <= int(t) < table.shape[0]:
+            out[i] = table[int(t)]
+    return out

@@ -48,7 +48,7 @@ class af_weights(C.Structure):
                 ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
 
 
-EXPORTS = ["af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+EXPORTS = ["af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
@@ -74,6 +74,10 @@ def load_library():
     L.af_workspace_bytes.argtypes = [C.POINTER(af_model_cfg), i32, i32]
     L.af_convert_bf16_to_fp16.argtypes = [vp, vp, sz, vp]
     L.af_convert_bf16_to_fp16.restype = C.c_int
+    L.af_argmax_rows.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
+    L.af_argmax_rows.restype = C.c_int
+    L.af_embed_rows.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int32, vp, vp]
+    L.af_embed_rows.restype = C.c_int
     L.af_gate_up_rows.argtypes = [C.c_int32]
     L.af_gate_up_rows.restype = C.c_size_t
     L.af_prepare_gate_up.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp]
@@ -257,3 +261,21 @@ def profile_read() -> dict:
     ms, cnt = (C.c_double * n)(), (C.c_int64 * n)()
     _check(load_library().af_debug_profile_read(ms, cnt, n))
     return {k: (ms[i], cnt[i]) for i, k in enumerate(PROFILE_CLASSES)}
+
+
+def argmax_rows(logits: torch.Tensor) -> torch.Tensor:
+    """af_argmax_rows: int32 [n] = lowest index of the maximum of every row of fp32 logits [n, V] (device)."""
+    assert logits.is_cuda and logits.dtype == torch.float32 and logits.dim() == 2 and logits.is_contiguous()
+    out = torch.empty(logits.shape[0], dtype=torch.int32, device=logits.device)
+    _check(load_library().af_argmax_rows(logits.data_ptr(), logits.shape[0], logits.shape[1], out.data_ptr(), _stream_ptr()))
+    return out
+
+
+def embed_rows(table: torch.Tensor, tokens: torch.Tensor, out: torch.Tensor = None) -> torch.Tensor:
+    """af_embed_rows: out[i] = table[tokens[i]] for a bf16 table [V, D] and int32 tokens [n] (all device)."""
+    assert table.is_cuda and table.dtype == torch.bfloat16 and table.is_contiguous() and tokens.dtype == torch.int32
+    if out is None:
+        out = torch.empty(tokens.shape[0], table.shape[1], dtype=torch.bfloat16, device=table.device)
+    _check(load_library().af_embed_rows(table.data_ptr(), table.shape[0], table.shape[1], tokens.data_ptr(),
+                                        tokens.shape[0], out.data_ptr(), _stream_ptr()))
+    return out

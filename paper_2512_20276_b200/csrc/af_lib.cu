@@ -624,6 +624,24 @@ extern "C" int af_convert_bf16_to_fp16(const void* src, void* dst, size_t n, voi
   return check_launch("convert_bf16_to_fp16_kernel");
 }
 
+extern "C" int af_argmax_rows(const float* logits, int32_t n_rows, int32_t vocab, int32_t* tokens_out, void* cuda_stream) {
+  if (n_rows < 0 || vocab <= 0 || (n_rows > 0 && (!logits || !tokens_out))) return fail(AF_ERR_ARG, "af_argmax_rows: bad argument");
+  if (n_rows == 0) return AF_OK;
+  argmax_rows_kernel<<<n_rows, 256, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(logits, vocab, tokens_out);
+  return check_launch("argmax_rows_kernel");
+}
+
+extern "C" int af_embed_rows(const void* table, int32_t vocab, int32_t d_model, const int32_t* tokens, int32_t n_rows,
+                             void* embeds_out, void* cuda_stream) {
+  if (n_rows < 0 || vocab <= 0 || d_model <= 0 || (d_model % 8) || (n_rows > 0 && (!table || !tokens || !embeds_out)))
+    return fail(AF_ERR_ARG, "af_embed_rows: bad argument (d_model must be a multiple of 8)");
+  if ((reinterpret_cast<uintptr_t>(table) | reinterpret_cast<uintptr_t>(embeds_out)) & 15) return fail(AF_ERR_ARG, "af_embed_rows: pointers must be 16-byte aligned");
+  if (n_rows == 0) return AF_OK;
+  embed_rows_kernel<<<n_rows, 128, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(
+      reinterpret_cast<const uint4*>(table), vocab, d_model / 8, tokens, reinterpret_cast<uint4*>(embeds_out));
+  return check_launch("embed_rows_kernel");
+}
+
 extern "C" size_t af_gate_up_rows(int32_t ffn) { return ffn > 0 ? static_cast<size_t>((ffn + 63) / 64) * GEMM_BM : 0; }
 
 extern "C" int af_prepare_gate_up(const void* gate, const void* up, void* dst, int32_t ffn, int32_t d_model, void* cuda_stream) {

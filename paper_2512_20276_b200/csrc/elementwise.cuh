@@ -231,6 +231,46 @@ __global__ void interleave_gate_up_kernel(const uint4* __restrict__ gate, const 
   dst[i] = v;
 }
 
+// f1: ArgMax over one logits row per block (Alg. 1 l.5/l.8).  (value, index) pairs are reduced with "greater value, or
+// equal value and lower index, wins", which is associative and commutative, so the result does not depend on the
+// reduction order: the lowest index of the maximum.  NaNs lose every comparison.
+__global__ void __launch_bounds__(256)
+argmax_rows_kernel(const float* __restrict__ logits, int vocab, int* __restrict__ tokens_out) {
+  __shared__ float s_v[8];
+  __shared__ int s_i[8];
+  const float* row = logits + static_cast<size_t>(blockIdx.x) * vocab;
+  float best = -INFINITY;
+  int best_i = 0x7fffffff;
+  for (int v = threadIdx.x; v < vocab; v += blockDim.x) {
+    const float x = row[v];
+    if (x > best || (x == best && v < best_i)) { best = x; best_i = v; }
+  }
+  auto better = [](float a, int ai, float b, int bi) { return a > b || (a == b && ai < bi); };
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, best_i, o);
+    if (better(ov, oi, best, best_i)) { best = ov; best_i = oi; }
+  }
+  if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = best; s_i[threadIdx.x >> 5] = best_i; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < static_cast<int>(blockDim.x >> 5); ++w)
+      if (better(s_v[w], s_i[w], best, best_i)) { best = s_v[w]; best_i = s_i[w]; }
+    tokens_out[blockIdx.x] = best_i == 0x7fffffff ? 0 : best_i;
+  }
+}
+
+// f1: embeds_out[i, :] = table[tokens[i], :] (16 bytes per thread-iteration); a token outside [0, vocab) gives zeros
+__global__ void embed_rows_kernel(const uint4* __restrict__ table, int vocab, int vec_per_row,
+                                  const int* __restrict__ tokens, uint4* __restrict__ out) {
+  const int tok = tokens[blockIdx.x];
+  const bool ok = tok >= 0 && tok < vocab;
+  for (int c = threadIdx.x; c < vec_per_row; c += blockDim.x)
+    out[static_cast<size_t>(blockIdx.x) * vec_per_row + c] =
+        ok ? table[static_cast<size_t>(tok) * vec_per_row + c] : make_uint4(0u, 0u, 0u, 0u);
+}
+
 // RoPE table in fp64: tab[pos][c] = (cos, sin)(pos * theta^(-2c/hd))
 __global__ void rope_table_kernel(float2* tab, int C, int hd, double theta) {
   const int half = hd / 2;

@@ -242,3 +242,47 @@ def test_wide_packed_steps_tiny(binding, n_prefill):
     hid, ref = P.step(segs, I.make_embeds(cfg, 5, 9, n_prefill + 3))
     P.check_ring([0, 1, 2, 3])
     P.check_logits(hid, ref, I.prediction_rows(segs))
+
+
+def test_argmax_rows_bit_exact(binding):
+    """f1: af_argmax_rows against the oracle's scalar definition on the SAME fp32 logits (an integer decided by floating
+    point: both sides decide on the stored fp32 values): random rows at vocab 32000 and 1001, planted ties (the lowest
+    index must win, wherever the tie sits in the block's reduction tree), NaNs, constant rows."""
+    g = torch.Generator().manual_seed(21)
+    for n, V in ((7, 32000), (5, 1001), (3, 17)):
+        lg = torch.randn(n, V, generator=g)
+        lg[0, V // 3] = lg[0, V - 1] = lg[0].max() + 1.0             # a tie far apart
+        if n > 1:
+            lg[1, 5] = float("nan"); lg[1, 6] = lg[1, 300 % V] = 9.0   # NaN next to a tie
+        if n > 2:
+            lg[2] = -2.5                                              # constant row -> 0
+        got = binding.argmax_rows(lg.cuda()).cpu().tolist()
+        assert got == O.argmax_rows(lg), (n, V)
+    allnan = torch.full((2, 64), float("nan"))
+    assert binding.argmax_rows(allnan.cuda()).cpu().tolist() == O.argmax_rows(allnan) == [0, 0]
+
+
+def test_embed_rows_bit_exact(binding):
+    g = torch.Generator().manual_seed(22)
+    table = torch.randn(512, 256, generator=g).to(torch.bfloat16)
+    toks = [0, 511, 17, 17, 512, -3, 255]
+    got = binding.embed_rows(table.cuda(), torch.tensor(toks, dtype=torch.int32).cuda()).cpu()
+    assert torch.equal(got, O.embed_rows(table, toks))
+
+
+def test_closed_loop_tokens_on_device(binding):
+    """f1 wiring on the tiny model: logits rows of a packed step -> af_argmax_rows -> af_embed_rows gives the next
+    step's decode rows without the logits leaving the device; tokens equal the oracle's argmax of the same logits."""
+    cfg = I.CFG_TINY
+    hw = I.make_weights(cfg, seed=0)
+    W = binding.Weights(cfg, hw)
+    ring = binding.Ring(cfg, 4, 128, max_rows=128)
+    hid = ring.packed_forward(W, I.make_embeds(cfg, 0, 0, 40).cuda(), [(0, 0, 0, 30), (1, 0, 0, 10)])
+    lg = ring.logits_rows(W, hid, [29, 39])
+    tok = binding.argmax_rows(lg)
+    assert tok.cpu().tolist() == O.argmax_rows(lg.cpu())
+    table = hw["w_lm"].to(torch.bfloat16).cuda().contiguous()         # any [V, D] bf16 table serves as the embedding
+    nxt = binding.embed_rows(table, tok)
+    assert torch.equal(nxt.cpu(), O.embed_rows(table.cpu(), tok.cpu().tolist()))
+    hid2 = ring.packed_forward(W, nxt, [(0, 1, 30, 1), (1, 1, 10, 1)])
+    assert hid2.shape[0] == 2 and torch.isfinite(hid2).all()

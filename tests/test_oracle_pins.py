@@ -237,3 +237,24 @@ def test_p11_silu_values():
     assert abs(float(s[1]) - 0.7310585786) < 1e-9
     assert abs(float(s[2]) + 0.2689414214) < 1e-9
     assert float(s[3]) == 100.0 and abs(float(s[4])) < 1e-40 and torch.isfinite(s).all()
+
+
+def test_argmax_rows_ties_nans_and_library_routine():
+    """oracle.argmax_rows against what fixes it: hand-made rows (ties -> lowest index, NaNs skipped, all -inf / all
+    NaN -> 0) and, on random rows without ties, numpy's argmax."""
+    import numpy as np
+    nan, inf = float("nan"), float("inf")
+    rows = torch.tensor([[1.0, 3.0, 3.0, 2.0], [nan, -1.0, nan, -1.0], [-inf, -inf, -inf, -inf], [nan, nan, nan, nan],
+                         [0.0, -0.0, 0.0, -0.0], [5.0, 1.0, inf, inf]])
+    assert O.argmax_rows(rows) == [1, 1, 0, 0, 0, 2]
+    g = torch.Generator().manual_seed(3)
+    r = torch.randn(9, 1000, generator=g)
+    assert O.argmax_rows(r) == [int(i) for i in np.argmax(r.numpy(), axis=1)]
+
+
+def test_embed_rows_is_a_row_gather():
+    g = torch.Generator().manual_seed(4)
+    table = torch.randn(50, 16, generator=g).to(torch.bfloat16)
+    toks = [3, 49, 0, 3, 50, -1]
+    out = O.embed_rows(table, toks)
+    assert torch.equal(out[:4], table[torch.tensor(toks[:4])]) and not out[4:].any()
