@@ -17,7 +17,8 @@ Pins (tests/test_oracle_pins.py): brute-force full-sequence recomputation (brute
 cache and an explicit mask), RMSNorm / RoPE / SiLU closed forms and worked values, attention special cases
 (one key, zero Wq -> running mean, torch SDPA), identity layer, HF transformers LlamaModel as a black box,
 prefill-then-decode == prefill of the concatenation, chunked prefill, request independence, ring-index brute
-force.  Parity unpinned: the paper prints no numeric worked example of any forward quantity; eps, theta and
+force; greedy_frame (Alg. 1's token loop) by brute-force recomputation of every stage and by "the K-stage pipeline
+gives every frame the tokens of that frame run alone".  Parity unpinned: the paper prints no numeric worked example of any forward quantity; eps, theta and
 the rotate-half RoPE pairing come from BASELINE.json configs[0] and the HF-Llama convention (A2, A5).
 """
 from __future__ import annotations
@@ -265,3 +266,24 @@ def embed_rows(table: torch.Tensor, tokens) -> torch.Tensor:
         if 0 <= int(t) < table.shape[0]:
             out[i] = table[int(t)]
     return out
+
+
+def greedy_frame(oracle: "Oracle", req: int, prefill_embeds: torch.Tensor, table: torch.Tensor, K: int, forced=None):
+    """Algorithm 1 for ONE frame run alone - the paper's sequential "Baseline" schedule, which the
+    pipelined loop must reproduce ("functionally lossless"): prefill the frame's L_P rows,
+    a_0 = ArgMax(LMHead(Norm(H[last]))) (l.5); then for s = 1..K-1 decode Embed(a_{s-1}) (l.2) at 0-indexed position
+    L_P + s - 1 (A4) and take a_s the same way (l.8).  `forced`: optional K tokens fed back INSTEAD of the
+    oracle's own argmax (teacher forcing, used when the caller compares logits along another implementation's token
+    path).  Returns (tokens [K] the oracle's own argmax at every stage, logits [K, V])."""
+    oracle.reset(req)
+    L_P = prefill_embeds.shape[0]
+    hid = oracle.step([(req, 0, 0, L_P)], prefill_embeds)
+    lg = [oracle.logits(hid, [L_P - 1])[0]]
+    toks = [argmax_rows(lg[0][None].to(torch.float32))[0]]
+    for s in range(1, K):
+        fed = toks[s - 1] if forced is None else int(forced[s - 1])
+        x = embed_rows(table, [fed])
+        hid = oracle.step([(req, 1, L_P + s - 1, 1)], x)
+        lg.append(oracle.logits(hid, [0])[0])
+        toks.append(argmax_rows(lg[s][None].to(torch.float32))[0])
+    return toks, torch.stack(lg)

@@ -258,3 +258,72 @@ def test_embed_rows_is_a_row_gather():
     toks = [3, 49, 0, 3, 50, -1]
     out = O.embed_rows(table, toks)
     assert torch.equal(out[:4], table[torch.tensor(toks[:4])]) and not out[4:].any()
+
+
+# ---------------------------------------------------------------- f1: Algorithm 1's token loop
+def _frame_inputs(cfg, n_frames, L_P):
+    g = torch.Generator().manual_seed(31)
+    table = (torch.randn(cfg.vocab, cfg.d_model, generator=g)).to(torch.bfloat16)
+    return table, [I.make_embeds(cfg, 31, f, L_P) for f in range(n_frames)]
+
+
+def test_greedy_frame_equals_bruteforce_recomputation():
+    """greedy_frame pinned by brute force: at every stage s the logits equal LMHead(Norm(.)) of the last row of a
+    cache-free full-sequence forward over [prefill rows ; Embed(a_0) .. Embed(a_{s-1})] and the token is numpy's argmax."""
+    import numpy as np
+    cfg, L_P, K = SMALL, 11, 5
+    w = I.make_weights(cfg, seed=7)
+    table, frames = _frame_inputs(cfg, 1, L_P)
+    o = O.Oracle(cfg, w, F64)
+    toks, lg = O.greedy_frame(o, 2, frames[0], table, K)
+    seq = frames[0].to(F64)
+    for s in range(K):
+        hid = O.brute_forward(cfg, w, seq)
+        hn = O.rmsnorm(hid[-1:], w["g_final"].to(F64), cfg.rms_eps)
+        ref = (hn @ w["w_lm"].to(F64).T)[0]
+        assert relerr(lg[s], ref) < 1e-9
+        assert toks[s] == int(np.argmax(ref.to(torch.float32).numpy()))
+        seq = torch.cat([seq, table[toks[s]][None].to(F64)])
+    # teacher forcing feeds the given tokens, and reports the oracle's own argmax at each stage
+    forced = [(t + 1) % cfg.vocab for t in toks]
+    toks_f, lg_f = O.greedy_frame(o, 2, frames[0], table, K, forced=forced)
+    assert toks_f[0] == toks[0] and relerr(lg_f[0], lg[0]) < 1e-12
+    seq = torch.cat([frames[0].to(F64), table[forced[0]][None].to(F64)])
+    hn = O.rmsnorm(O.brute_forward(cfg, w, seq)[-1:], w["g_final"].to(F64), cfg.rms_eps)
+    assert relerr(lg_f[1], (hn @ w["w_lm"].to(F64).T)[0]) < 1e-9
+
+
+def test_pipelined_loop_equals_sequential_frames():
+    """The paper's claim the loop rests on ("functionally lossless"): running Alg. 1 as the K-stage pipeline
+    (steady_schedule, tokens of step t feeding the decode rows of step t+1, regions recycled) gives every frame the
+    tokens and logits of that frame run alone by greedy_frame."""
+    cfg, L_P, K, R, n_frames = SMALL, 9, 4, 5, 9
+    w = I.make_weights(cfg, seed=8)
+    table, frames = _frame_inputs(cfg, n_frames, L_P)
+    alone = O.Oracle(cfg, w, F64)
+    want = [O.greedy_frame(alone, 0, frames[f], table, K) for f in range(n_frames)]
+    o = O.Oracle(cfg, w, F64)
+    got_tok = [[None] * K for _ in range(n_frames)]
+    prev = []                                             # tokens of the previous step, by stage
+    for t in range(n_frames + K - 1):
+        segs = [s for s in I.steady_schedule(t, L_P, K, R) if (t - (s[2] - L_P + 1 if s[1] else 0)) < n_frames]
+        dec = [s for s in segs if s[1] == 1]
+        pre = [s for s in segs if s[1] == 0]
+        rows, stages = [], []
+        if pre:
+            o.reset(pre[0][0])
+            rows.append(frames[t]); stages.append(0)
+        for s in dec:
+            st = s[2] - L_P + 1
+            rows.append(O.embed_rows(table, [prev[st - 1]])); stages.append(st)
+        hid = o.step(segs, torch.cat(rows))
+        lg = o.logits(hid, I.prediction_rows(segs))
+        toks = O.argmax_rows(lg.to(torch.float32))
+        cur = [None] * K
+        for i, st in enumerate(stages):
+            f = t - st
+            got_tok[f][st] = toks[i]
+            cur[st] = toks[i]
+            assert relerr(lg[i], want[f][1][st]) < 1e-9, (t, st)
+        prev = cur
+    assert got_tok == [w_[0] for w_ in want]
