@@ -309,6 +309,27 @@ def main():
         ev5.record(stream)
         barrier()
     ms_loop = ev4.elapsed_time(ev5)
+    # ---- timed region 4 (f1, second half): af_loop_* - segment table, ring bookkeeping and A_sequences advanced on the
+    #      device, the steady step replayed as ONE CUDA graph; the host copies the new frame's prefill rows in and the
+    #      completed frame's 7 tokens out, and never synchronises inside the region ----
+    ring2 = binding.Ring(cfg, R_REGIONS, CAPACITY, max_rows=288)
+    loop = binding.Loop(W, ring2, table, L_P, K_STAGES)
+    gs = torch.cuda.Stream()
+    frame_host = torch.empty(1 + K_STAGES, dtype=torch.int32).pin_memory()
+    with torch.cuda.stream(gs):
+        for timed in (False, True):
+            barrier()
+            ev6, ev7 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            launches_g0 = binding.launch_count()
+            ev6.record(gs)
+            for i in range(args.steps if timed else K_STAGES - 1 + max(3, warmup)):
+                loop.prefill_embeds.copy_(e_host[i % n_buf][:L_P], non_blocking=True)
+                loop.step(use_graph=True, stream=gs)
+                frame_host.copy_(loop.frame, non_blocking=True)
+            ev7.record(gs)
+            barrier()
+    ms_graph = ev6.elapsed_time(ev7)
+    launches_graph = binding.launch_count() - launches_g0
     # ---- per-kernel-class events (separate pass; same steps) ----
     n_prof = min(20, args.steps)
     binding.profile(True)
@@ -318,7 +339,7 @@ def main():
     binding.profile(False)
     clocks = sampler.stop()
 
-    ms_dev, ms_e2e, ms_loop = replicas.max_over_ranks([ms_dev, ms_e2e, ms_loop], device="cuda")
+    ms_dev, ms_e2e, ms_loop, ms_graph = replicas.max_over_ranks([ms_dev, ms_e2e, ms_loop, ms_graph], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -364,6 +385,11 @@ def main():
         "e2e_device_loop": {"value": replicas.whole_job_throughput(args.steps, ms_loop), "unit": "frames/s",
                             "what": "f1: decode rows = af_embed_rows(af_argmax_rows(previous logits)) on the device",
                             "h2d_bytes_per_step": L_P * cfg.d_model * 2, "d2h_bytes_per_step": K_STAGES * 4},
+        "e2e_graph_loop": {"value": replicas.whole_job_throughput(args.steps, ms_graph), "unit": "frames/s",
+                           "what": "f1: af_loop_step - device-side segment table / ring bookkeeping / A_sequences, the steady "
+                                   "step replayed as one CUDA graph; prefill rows in, the completed frame's tokens out",
+                           "h2d_bytes_per_step": L_P * cfg.d_model * 2, "d2h_bytes_per_step": (1 + K_STAGES) * 4,
+                           "kernel_nodes_per_step": launches_graph / args.steps},
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline:

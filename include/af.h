@@ -153,6 +153,36 @@ int af_argmax_rows(const float* logits, int32_t n_rows, int32_t vocab, int32_t* 
 int af_embed_rows(const void* table, int32_t vocab, int32_t d_model, const int32_t* tokens, int32_t n_rows,
                   void* embeds_out, void* cuda_stream);
 
+/* ---- f1, second half: Algorithm 1's pipeline loop with its state on the device ----
+ * An af_loop drives the paper's K-stage pipeline over one ring: step t packs the prefill of frame t (prefill_len rows,
+ * region t mod R, recycled first exactly as af_ring_reset_slot(ring, t mod R, -1)) with decode stage s = 1..min(t, K-1)
+ * of frame t-s (region (t-s) mod R, position prefill_len + s - 1; Alg. 1 l.2-10).  The segment table,
+ * the per-region (base, len) bookkeeping and A_sequences live in device memory and are advanced by kernels; the decode
+ * rows are Embed(ArgMax(logits of the previous step)) (af_embed_rows / af_argmax_rows' kernels, lowest index wins).
+ * The host keeps an integer mirror (the ring's own) for validation and launch geometry only.  Once the pipeline is
+ * full every step has the same shape: the first full step is issued as plain launches, the second is captured into
+ * ONE CUDA graph, later steps replay it (use_graph != 0 and a non-default stream; otherwise plain launches).  No call
+ * synchronises.
+ *   af_loop_create : w (needs g_final, w_lm; the struct is copied, w->layers must outlive the loop), ring (all regions
+ *     are emptied at their current rotation; the loop owns the ring's bookkeeping until af_loop_destroy), embed_table =
+ *     device bf16 [vocab, d_model], 16-byte aligned, caller-owned; workspace as for af_packed_forward with
+ *     max_rows >= prefill_len + chunk_k - 1, caller-owned, must outlive the loop.  Needs chunk_k <= n_regions
+ *     (AF_ERR_SEGMENT) and prefill_len + chunk_k - 1 <= capacity (AF_ERR_CAPACITY).  The loop's own buffers (a few MB)
+ *     are library-owned device memory.
+ *   af_loop_buffers : device pointers, each may be NULL: prefill_embeds = bf16 [prefill_len, d_model], the caller writes
+ *     frame t's projected embeddings here on `cuda_stream` before af_loop_step; hidden = fp32 [T, d_model] and
+ *     logits = fp32 [1 + n_dec, vocab] of the last step (prediction rows in stage order); tokens = int32 [1 + n_dec]
+ *     tokens of the last step by stage; frame = int32 [1 + chunk_k]: {frame id, its chunk_k tokens} of the last
+ *     COMPLETED frame (id -1 while the pipeline fills).
+ *   af_loop_step : enqueues step t on cuda_stream and advances the host mirror. */
+typedef struct af_loop af_loop;
+int af_loop_create(const af_weights* w, af_ring* ring, const void* embed_table, int32_t prefill_len, int32_t chunk_k,
+                   void* workspace, size_t ws_bytes, af_loop** out);
+int af_loop_buffers(af_loop* loop, void** prefill_embeds, float** hidden, float** logits, int32_t** tokens, int32_t** frame);
+int af_loop_step(af_loop* loop, int32_t use_graph, void* cuda_stream);
+int32_t af_loop_steps_done(const af_loop* loop);
+int af_loop_destroy(af_loop* loop);
+
 int af_ring_destroy(af_ring* ring); /* frees the handle and its own metadata; never frees caller memory */
 
 /* ---- introspection for bit-exact bookkeeping parity; these synchronise, they are not hot path ---- */

@@ -48,7 +48,8 @@ class af_weights(C.Structure):
                 ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
 
 
-EXPORTS = ["af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+EXPORTS = ["af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
+           "af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
@@ -97,6 +98,13 @@ def load_library():
     L.af_debug_profile.restype = C.c_int
     L.af_debug_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), i32]
     L.af_debug_profile_read.restype = C.c_int
+    L.af_loop_create.argtypes = [C.POINTER(af_weights), vp, vp, i32, i32, vp, sz, C.POINTER(vp)]
+    L.af_loop_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    L.af_loop_step.argtypes = [vp, i32, vp]
+    L.af_loop_steps_done.argtypes = [vp]
+    L.af_loop_destroy.argtypes = [vp]
+    for n in ("af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy"):
+        getattr(L, n).restype = C.c_int
     L.af_last_error.restype = C.c_char_p
     L.af_last_error.argtypes = []
     for n in ("af_ring_create", "af_ring_reset_slot", "af_packed_forward", "af_logits_rows", "af_ring_destroy",
@@ -279,3 +287,54 @@ def embed_rows(table: torch.Tensor, tokens: torch.Tensor, out: torch.Tensor = No
     _check(load_library().af_embed_rows(table.data_ptr(), table.shape[0], table.shape[1], tokens.data_ptr(),
                                         tokens.shape[0], out.data_ptr(), _stream_ptr()))
     return out
+
+
+def _wrap_device(ptr: int, dtype, shape, device):
+    """A torch view of library-owned device memory (no copy, no ownership)."""
+    iface = {"shape": tuple(shape), "typestr": {torch.float32: "<f4", torch.int32: "<i4", torch.int16: "<i2"}[dtype],
+             "data": (ptr, False), "version": 2}
+    holder = type("_DevMem", (), {"__cuda_array_interface__": iface})()
+    return torch.as_tensor(holder, device=device)
+
+
+class Loop:
+    """af_loop_create / af_loop_buffers / af_loop_step / af_loop_destroy: Algorithm 1's pipeline with device-side state."""
+
+    def __init__(self, weights: "Weights", ring: "Ring", embed_table: torch.Tensor, prefill_len: int, chunk_k: int):
+        L = load_library()
+        assert embed_table.dtype == torch.bfloat16 and embed_table.is_contiguous()
+        self.weights, self.ring, self.table = weights, ring, embed_table        # keep the caller-owned memory alive
+        self.L_P, self.K = prefill_len, chunk_k
+        h = C.c_void_p()
+        _check(L.af_loop_create(C.byref(weights.struct), ring.handle, embed_table.data_ptr(), prefill_len, chunk_k,
+                                ring.workspace.data_ptr(), ring.ws_bytes, C.byref(h)))
+        self.handle = h
+        p = [C.c_void_p() for _ in range(5)]
+        _check(L.af_loop_buffers(h, *[C.byref(x) for x in p]))
+        cfg, dev = ring.cfg, embed_table.device
+        T = prefill_len + chunk_k - 1
+        # bf16 has no __cuda_array_interface__ typestr: view the embeddings as int16 and reinterpret
+        self.prefill_embeds = _wrap_device(p[0].value, torch.int16,
+                                           (prefill_len, cfg.d_model), dev).view(torch.bfloat16)
+        self.hidden = _wrap_device(p[1].value, torch.float32, (T, cfg.d_model), dev)
+        self.logits = _wrap_device(p[2].value, torch.float32, (chunk_k, cfg.vocab), dev)
+        self.tokens = _wrap_device(p[3].value, torch.int32, (chunk_k,), dev)
+        self.frame = _wrap_device(p[4].value, torch.int32, (1 + chunk_k,), dev)
+
+    def step(self, use_graph: bool = True, stream=None):
+        _check(load_library().af_loop_step(self.handle, 1 if use_graph else 0, _stream_ptr(stream)))
+
+    @property
+    def steps_done(self) -> int:
+        return load_library().af_loop_steps_done(self.handle)
+
+    def destroy(self):
+        if self.handle is not None:
+            load_library().af_loop_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -686,8 +686,11 @@ static int check_weights(const af_weights* w, bool need_lm) {
   return AF_OK;
 }
 
-extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
-                                 af_ring* g, float* hidden_out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+// sta_dev != nullptr: the kernels ingest the segment table from that device struct (written by loop_advance_kernel, f1)
+// instead of the by-value copy of `segs`; `segs` still drives validation, the host mirror and the launch geometry.
+static int packed_forward_impl(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
+                               af_ring* g, float* hidden_out, void* workspace, size_t ws_bytes, void* cuda_stream,
+                               const SegTableArg* sta_dev) {
   if (!g) return fail(AF_ERR_ARG, "null ring");
   if (n_segs < 0) return fail(AF_ERR_ARG, "n_segs < 0");
   if (n_segs == 0) { g->last_T = 0; return AF_OK; }  // legal no-op
@@ -745,7 +748,8 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
     if ((rc = check_launch(name))) return rc;                                                                  \
   } while (0)
   { ProfScope ps_(PC_OTHER, st);
-  rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
+  if (sta_dev) rowmap_dev_kernel<<<1, 256, 0, st>>>(sta_dev, g->tb, g->n_items_dev);
+  else rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
   }
   if ((rc = check_launch("rowmap_kernel"))) return rc;
   {
@@ -835,6 +839,11 @@ extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds,
   return AF_OK;
 }
 
+extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
+                                 af_ring* g, float* hidden_out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  return packed_forward_impl(w, packed_embeds, segs, n_segs, g, hidden_out, workspace, ws_bytes, cuda_stream, nullptr);
+}
+
 extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const int32_t* rows, int32_t n_rows,
                               float* logits_out, void* workspace, size_t ws_bytes, void* cuda_stream) {
   int rc = check_weights(w, true);
@@ -881,3 +890,157 @@ extern "C" int af_debug_gemm(const void* a, const void* wmat, float* out, int32_
   const void* wl[3] = {wmat, nullptr, nullptr};
   return launch_gemm(PC_OTHER, reinterpret_cast<cudaStream_t>(cuda_stream), gp, ov, a, n_tok, wl, n_tok);
 }
+
+// ------------------------------------------------------------------------------------------------ f1: Alg. 1 on the device
+// The pipeline loop of Algorithm 1 with its state on the device: segment table and ring bookkeeping
+// advanced by loop_advance_kernel, ArgMax -> Embed feedback through af_argmax_rows / af_embed_rows' kernels,
+// A_sequences kept by loop_commit_kernel.  The host only mirrors the integer schedule (validation, launch geometry)
+// and, once the pipeline is full, replays ONE captured CUDA graph per step: no host synchronisation anywhere.
+struct af_loop {
+  af_weights w;
+  af_ring* g;
+  const void* table;
+  int L_P, K, t;
+  void* ws; size_t ws_bytes;
+  uint8_t* mem;
+  LoopState* ls; SegTableArg* sta;
+  __nv_bfloat16* packed; float* hidden; float* logits; int* tok;
+  int steady_direct;            // steady-shape steps issued as plain launches (the first one warms every host cache)
+  cudaGraphExec_t graph; int64_t graph_nodes;
+};
+
+extern "C" int af_loop_create(const af_weights* w, af_ring* g, const void* embed_table, int32_t prefill_len, int32_t chunk_k,
+                              void* workspace, size_t ws_bytes, af_loop** out) {
+  if (!g || !out || !embed_table) return fail(AF_ERR_ARG, "null argument");
+  int rc = check_weights(w, true);
+  if (rc) return rc;
+  if (memcmp(&w->cfg, &g->cfg, sizeof w->cfg) != 0) return fail(AF_ERR_ARG, "weights cfg differs from the ring's cfg");
+  if (reinterpret_cast<uintptr_t>(embed_table) & 15) return fail(AF_ERR_ARG, "embed_table must be 16-byte aligned");
+  const int R = g->rc.n_regions, C = g->rc.capacity, K = chunk_k, L_P = prefill_len;
+  if (K < 1 || K > AF_MAX_SEGS || L_P < 1) return fail(AF_ERR_ARG, "need 1 <= chunk_k <= %d and prefill_len >= 1", AF_MAX_SEGS);
+  if (R < K || R > AF_MAX_SEGS) return fail(AF_ERR_SEGMENT, "the pipeline needs chunk_k <= n_regions <= %d (K = %d, R = %d)", AF_MAX_SEGS, K, R);
+  if (L_P + K - 1 > C) return fail(AF_ERR_CAPACITY, "prefill_len %d + chunk_k %d - 1 > capacity %d", L_P, K, C);
+  const int T = L_P + K - 1;
+  if (T > g->max_rows) return fail(AF_ERR_CAPACITY, "%d packed rows > ring rows %d", T, g->max_rows);
+  Workspace wsp;
+  if ((rc = carve(&w->cfg, workspace, ws_bytes, T, &wsp))) return rc;
+  const size_t D = w->cfg.d_model, V = w->cfg.vocab;
+  size_t off = 0;
+  auto take = [&](size_t n) { const size_t o = off; off += align_up(n, 256); return o; };
+  const size_t o_ls = take(sizeof(LoopState)), o_sta = take(sizeof(SegTableArg)), o_pk = take(T * D * 2),
+               o_hid = take(T * D * 4), o_lg = take(K * V * 4), o_tok = take(AF_MAX_SEGS * sizeof(int));
+  af_loop* lp = new af_loop();
+  cudaError_t e = cudaMalloc(&lp->mem, off);
+  if (e != cudaSuccess) { delete lp; return fail(AF_ERR_CUDA, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  lp->w = *w; lp->g = g; lp->table = embed_table; lp->L_P = L_P; lp->K = K; lp->t = 0;
+  lp->ws = workspace; lp->ws_bytes = ws_bytes;
+  lp->ls = reinterpret_cast<LoopState*>(lp->mem + o_ls); lp->sta = reinterpret_cast<SegTableArg*>(lp->mem + o_sta);
+  lp->packed = reinterpret_cast<__nv_bfloat16*>(lp->mem + o_pk); lp->hidden = reinterpret_cast<float*>(lp->mem + o_hid);
+  lp->logits = reinterpret_cast<float*>(lp->mem + o_lg); lp->tok = reinterpret_cast<int*>(lp->mem + o_tok);
+  lp->steady_direct = 0; lp->graph = nullptr; lp->graph_nodes = 0;
+  // every region starts empty at its current rotation; the device state starts as a copy of the host mirror
+  LoopState* h = new LoopState();
+  memset(h, 0, sizeof *h);
+  h->L_P = L_P; h->K = K; h->R = R; h->C = C; h->frame_id = -1;
+  for (int r = 0; r < R; ++r) { g->len[r] = 0; h->base[r] = g->base[r]; }
+  for (int s = 0; s < AF_MAX_SEGS; ++s) h->frame_tok[s] = -1;
+  e = cudaMemset(lp->mem, 0, off);
+  if (e == cudaSuccess) e = cudaMemcpy(lp->ls, h, sizeof *h, cudaMemcpyHostToDevice);
+  delete h;
+  if (e != cudaSuccess) { cudaFree(lp->mem); delete lp; return fail(AF_ERR_CUDA, "loop state upload: %s", cudaGetErrorString(e)); }
+  *out = lp;
+  return AF_OK;
+}
+
+extern "C" int af_loop_destroy(af_loop* lp) {
+  if (!lp) return AF_OK;
+  if (lp->graph) cudaGraphExecDestroy(lp->graph);
+  cudaFree(lp->mem);
+  delete lp;
+  return AF_OK;
+}
+
+extern "C" int af_loop_buffers(af_loop* lp, void** prefill_embeds, float** hidden, float** logits, int32_t** tokens,
+                               int32_t** frame) {
+  if (!lp) return fail(AF_ERR_ARG, "null loop");
+  if (prefill_embeds) *prefill_embeds = lp->packed;
+  if (hidden) *hidden = lp->hidden;
+  if (logits) *logits = lp->logits;
+  if (tokens) *tokens = lp->tok;
+  if (frame) *frame = &lp->ls->frame_id;
+  return AF_OK;
+}
+
+// the launches of one pipeline step, in stream order (also what the graph captures)
+static int loop_enqueue(af_loop* lp, const af_segment* segs, int n_dec, cudaStream_t st) {
+  const af_model_cfg& c = lp->w.cfg;
+  int rc;
+  loop_advance_kernel<<<1, 32, 0, st>>>(lp->ls, lp->sta);
+  if ((rc = check_launch("loop_advance_kernel"))) return rc;
+  if (n_dec > 0) {   // Alg. 1 l.2: decode row of stage s = Embed(token stage s-1 produced in the previous step)
+    embed_rows_kernel<<<n_dec, 128, 0, st>>>(reinterpret_cast<const uint4*>(lp->table), c.vocab, c.d_model / 8, lp->tok,
+                                             reinterpret_cast<uint4*>(lp->packed + static_cast<size_t>(lp->L_P) * c.d_model));
+    if ((rc = check_launch("embed_rows_kernel"))) return rc;
+  }
+  if ((rc = packed_forward_impl(&lp->w, lp->packed, segs, 1 + n_dec, lp->g, lp->hidden, lp->ws, lp->ws_bytes, st, lp->sta))) return rc;
+  int32_t rows[AF_MAX_SEGS];
+  for (int s = 0; s <= n_dec; ++s) rows[s] = lp->L_P - 1 + s;   // prediction rows: last prefill row, then the decode rows
+  if ((rc = af_logits_rows(&lp->w, lp->hidden, rows, 1 + n_dec, lp->logits, lp->ws, lp->ws_bytes, st))) return rc;
+  argmax_rows_kernel<<<1 + n_dec, 256, 0, st>>>(lp->logits, c.vocab, lp->tok);
+  if ((rc = check_launch("argmax_rows_kernel"))) return rc;
+  loop_commit_kernel<<<1, 32, 0, st>>>(lp->ls, lp->tok);
+  return check_launch("loop_commit_kernel");
+}
+
+extern "C" int af_loop_step(af_loop* lp, int32_t use_graph, void* cuda_stream) {
+  if (!lp) return fail(AF_ERR_ARG, "null loop");
+  af_ring* g = lp->g;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const int R = g->rc.n_regions, K = lp->K, L_P = lp->L_P, t = lp->t;
+  const int n_dec = t < K - 1 ? t : K - 1;
+  // host mirror of loop_advance_kernel (same integer rules; the device computes its own copy)
+  int rc = af_ring_reset_slot(g, t % R, -1);
+  if (rc) return rc;
+  af_segment segs[AF_MAX_SEGS];
+  segs[0] = af_segment{t % R, AF_PHASE_PREFILL, 0, L_P};
+  for (int s = 1; s <= n_dec; ++s) segs[s] = af_segment{(t - s) % R, AF_PHASE_DECODE, g->len[(t - s) % R], 1};
+  const bool steady = n_dec == K - 1;
+  const bool graph_ok = steady && use_graph && st != nullptr && !g_prof_on && !g_trace;
+  if (graph_ok && lp->graph) {
+    cudaError_t e = cudaGraphLaunch(lp->graph, st);
+    if (e != cudaSuccess) return fail(AF_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(e));
+    g_launches.fetch_add(lp->graph_nodes, std::memory_order_relaxed);
+    for (int s = 0; s <= n_dec; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;   // a9 on the mirror
+    g->last_T = L_P + n_dec;
+    lp->t = t + 1;
+    return AF_OK;
+  }
+  // the first steady step runs as plain launches (it fills the schedule / tensor-map caches, which allocate); the
+  // second is captured, instantiated and launched; every later one is a replay
+  const bool capture = graph_ok && lp->steady_direct >= 1;
+  if (capture) {
+    cudaError_t e = cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) return fail(AF_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
+  }
+  rc = loop_enqueue(lp, segs, n_dec, st);
+  if (capture) {
+    cudaGraph_t gr = nullptr;
+    cudaError_t e = cudaStreamEndCapture(st, &gr);
+    if (rc) { if (gr) cudaGraphDestroy(gr); return rc; }
+    if (e != cudaSuccess) return fail(AF_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    size_t n_nodes = 0;
+    cudaGraphGetNodes(gr, nullptr, &n_nodes);
+    e = cudaGraphInstantiate(&lp->graph, gr, 0);
+    cudaGraphDestroy(gr);
+    if (e != cudaSuccess) { lp->graph = nullptr; return fail(AF_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+    lp->graph_nodes = static_cast<int64_t>(n_nodes);
+    e = cudaGraphLaunch(lp->graph, st);
+    if (e != cudaSuccess) return fail(AF_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(e));
+  }
+  if (rc) return rc;
+  if (steady) ++lp->steady_direct;
+  lp->t = t + 1;
+  return AF_OK;
+}
+
+extern "C" int32_t af_loop_steps_done(const af_loop* lp) { return lp ? lp->t : -1; }

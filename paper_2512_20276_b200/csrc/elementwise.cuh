@@ -15,7 +15,7 @@ struct SegTableArg {  // the host segment table, passed by value as a kernel par
 // a0: every packed row i -> (req, pos = start_pos + i - row0(seg), slot = req*C + (base_r + pos) mod C), plus the
 // per-segment arrays and the attention work list.  One block; all integer, bit-exact by construction (P:208
 // "precomputed physical address").
-__global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_out) {
+__device__ __forceinline__ void rowmap_body(const SegTableArg& st, StepTables tb, int* n_items_out) {
   __shared__ int row0[AF_MAX_SEGS_K + 1], item0[AF_MAX_SEGS_K + 1];
   if (threadIdx.x == 0) {
     int r = 0, it = 0;
@@ -61,6 +61,61 @@ __global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_
     tb.row_pos[i] = pos;
     tb.row_slot[i] = st.req[s] * st.C + (st.base[s] + pos) % st.C;
   }
+}
+
+__global__ void rowmap_kernel(const SegTableArg st, StepTables tb, int* n_items_out) { rowmap_body(st, tb, n_items_out); }
+
+// The same ingest from a segment table that lives on the DEVICE (written by loop_advance_kernel below).
+__global__ void rowmap_dev_kernel(const SegTableArg* __restrict__ st_dev, StepTables tb, int* n_items_out) {
+  __shared__ SegTableArg st;
+  for (int i = threadIdx.x; i < static_cast<int>(sizeof(SegTableArg) / sizeof(int)); i += blockDim.x)
+    reinterpret_cast<int*>(&st)[i] = reinterpret_cast<const int*>(st_dev)[i];
+  __syncthreads();
+  rowmap_body(st, tb, n_items_out);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// f1: Algorithm 1's pipeline state on the device.  Step t packs the prefill of frame t (region t mod R,
+// recycled first: base <- (base + len) mod C, len <- 0, the same rule as af_ring_reset_slot(new_base = -1)) with decode
+// stage s = 1..min(t, K-1) of frame t - s (region (t - s) mod R) at position len[region] = L_P + s - 1.  All integer.
+struct LoopState {
+  int t;                        // steps completed
+  int L_P, K, R, C;
+  int frame_id;                 // frame whose K tokens sit in frame_tok (-1 before the first frame completes)
+  int frame_tok[AF_MAX_SEGS_K];                  // [K] tokens of the last completed frame (directly after frame_id)
+  int base[AF_MAX_SEGS_K], len[AF_MAX_SEGS_K];   // per region (R <= AF_MAX_SEGS)
+  int seq[AF_MAX_SEGS_K * AF_MAX_SEGS_K];        // A_sequences [R][K] (Alg. 1 l.9), token of stage s of the frame in region r
+};
+
+__global__ void loop_advance_kernel(LoopState* __restrict__ ls, SegTableArg* __restrict__ st) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int t = ls->t, R = ls->R, C = ls->C, K = ls->K;
+  const int r0 = t % R;
+  ls->base[r0] = (ls->base[r0] + ls->len[r0]) % C;
+  ls->len[r0] = 0;
+  const int n_dec = t < K - 1 ? t : K - 1;
+  st->n_segs = 1 + n_dec; st->R = R; st->C = C;
+  for (int s = 0; s <= n_dec; ++s) {
+    const int r = (t - s) % R;
+    const int n = s == 0 ? ls->L_P : 1;
+    st->req[s] = r; st->start[s] = ls->len[r]; st->len[s] = n; st->base[s] = ls->base[r];
+    ls->len[r] += n;             // a9: the commit is a relabelling
+  }
+}
+
+// End of step t: tok[s] is the token of stage s (prediction row s of the step).  Record it in A_sequences; the frame that
+// just took stage K-1 is complete: publish its K tokens.  Then t <- t + 1.
+__global__ void loop_commit_kernel(LoopState* __restrict__ ls, const int* __restrict__ tok) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int t = ls->t, R = ls->R, K = ls->K;
+  const int n_dec = t < K - 1 ? t : K - 1;
+  for (int s = 0; s <= n_dec; ++s) ls->seq[((t - s) % R) * K + s] = tok[s];
+  if (n_dec == K - 1) {
+    const int r = (t - (K - 1)) % R;
+    for (int s = 0; s < K; ++s) ls->frame_tok[s] = ls->seq[r * K + s];
+    ls->frame_id = t - (K - 1);
+  }
+  ls->t = t + 1;
 }
 
 // bf16 embeddings -> fp32 residual stream

@@ -1,0 +1,117 @@
+"""f1: Algorithm 1's pipeline loop with its state on the device (af_loop_*), through the C ABI.
+
+What is unique is compared exactly, what floating point decides is compared in the precision that decided it:
+  * the device-side segment table / ring bookkeeping against the oracle's integer index model, bit-exact, every step;
+  * the graph-replayed loop against the same steps driven from the host through af_packed_forward / af_logits_rows /
+    af_argmax_rows / af_embed_rows on a second ring: bit-identical logits and tokens (the kernels are deterministic);
+  * every token is the oracle's argmax definition applied to the library's own fp32 logits;
+  * every completed frame against oracle.greedy_frame (the frame run alone, unpacked), teacher-forced along the
+    library's tokens: logits within the north-star tolerance, and the oracle's own token wherever its top-2 margin
+    exceeds what that tolerance can flip.
+Run with `pytest -m gpu` on a B200."""
+import pytest
+import torch
+
+from oracle import af_oracle as O
+from paper_2512_20276_b200 import inputs as I
+from af_harness import relmax, TOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2512_20276_b200 import binding as b
+    b.load_library()
+    return b
+
+
+def _table(cfg, seed):
+    g = torch.Generator().manual_seed(seed)
+    return torch.randn(cfg.vocab, cfg.d_model, generator=g).to(torch.bfloat16)
+
+
+@pytest.mark.parametrize("use_graph", [True, False])
+def test_device_loop_tiny(binding, use_graph):
+    cfg, R, C, L_P, K, n_steps = I.CFG_TINY, 5, 128, 40, 4, 14
+    hw = I.make_weights(cfg, seed=0)
+    W = binding.Weights(cfg, hw)
+    table = _table(cfg, 41)
+    table_d = table.cuda()
+    frames = [I.make_embeds(cfg, 41, t, L_P) for t in range(n_steps)]
+    bases = [100, 0, 127, 60, 90]                       # appends cross the wrap in several regions
+
+    ring = binding.Ring(cfg, R, C, max_rows=128)
+    host = binding.Ring(cfg, R, C, max_rows=128)         # the same steps, driven from the host
+    for r, b in enumerate(bases):
+        ring.reset_slot(r, b)
+        host.reset_slot(r, b)
+    loop = binding.Loop(W, ring, table_d, L_P, K)
+    st = torch.cuda.Stream()
+    base, length = list(bases), [0] * R
+    got_tok, got_lg, frames_out = [], [], {}
+    prev_host_tok = None
+    for t in range(n_steps):
+        segs = I.steady_schedule(t, L_P, K, R)
+        n_dec = len(segs) - 1
+        with torch.cuda.stream(st):
+            loop.prefill_embeds.copy_(frames[t].cuda(), non_blocking=False)
+            loop.step(use_graph=use_graph, stream=st)
+        st.synchronize()
+        assert loop.steps_done == t + 1
+        # ---- integer state: device table == index model, bit-exact
+        base[t % R], length[t % R] = O.ring_reset_model(C, base[t % R], length[t % R], -1)
+        mr, mp, ms, length = O.ring_index_model(R, C, base, length, segs)
+        assert ring.row_map(len(mr)) == (mr, mp, ms), f"step {t}: device row map differs from the index model"
+        for r in range(R):
+            assert ring.get_state(r) == (base[r], length[r])
+        tok = loop.tokens[:1 + n_dec].cpu().tolist()
+        lg = loop.logits[:1 + n_dec].cpu()
+        assert tok == O.argmax_rows(lg), f"step {t}: token is not the lowest-index maximum of the library's logits"
+        got_tok.append(tok); got_lg.append(lg)
+        fr = loop.frame.cpu().tolist()
+        if t >= K - 1:
+            assert fr[0] == t - (K - 1)
+            frames_out[fr[0]] = fr[1:]
+        else:
+            assert fr[0] == -1
+        # ---- the same step through the host-driven public calls: bit-identical
+        host.reset_slot(t % R, -1)
+        emb = frames[t].cuda()
+        if n_dec:
+            emb = torch.cat([emb, binding.embed_rows(table_d, prev_host_tok[:n_dec])])
+        hid = host.packed_forward(W, emb, segs)
+        hlg = host.logits_rows(W, hid, I.prediction_rows(segs))
+        prev_host_tok = binding.argmax_rows(hlg)
+        assert torch.equal(hlg.cpu(), lg), f"step {t}: loop logits differ from the host-driven step"
+        assert prev_host_tok.cpu().tolist() == tok
+        assert torch.equal(loop.hidden[:L_P + n_dec].cpu(), hid.cpu())
+
+    # ---- completed frames against the frame run alone by the oracle (A_sequences, Alg. 1 l.9)
+    orc = O.Oracle(cfg, hw, torch.float64)
+    assert sorted(frames_out) == list(range(n_steps - K + 1))
+    n_margin = 0
+    for f, toks in frames_out.items():
+        assert toks == [got_tok[f + s][s] for s in range(K)], "A_sequences differs from the per-step tokens"
+        own, ref = O.greedy_frame(orc, 0, frames[f], table, K, forced=toks)
+        for s in range(K):
+            lg = got_lg[f + s][s].double()
+            assert relmax(lg, ref[s]) <= TOL, (f, s)
+            top2 = torch.topk(ref[s], 2).values
+            if float(top2[0] - top2[1]) > 2 * TOL * float(ref[s].abs().max()):
+                assert toks[s] == own[s], (f, s)
+                n_margin += 1
+    assert n_margin > 0
+    loop.destroy()
+
+
+def test_loop_create_rejects_bad_geometry(binding):
+    cfg = I.CFG_TINY
+    W = binding.Weights(cfg, I.make_weights(cfg, seed=0))
+    table = _table(cfg, 1).cuda()
+    ring = binding.Ring(cfg, 4, 128, max_rows=128)
+    with pytest.raises(binding.AfError):
+        binding.Loop(W, ring, table, 40, 5)               # K > R
+    with pytest.raises(binding.AfError):
+        binding.Loop(W, ring, table, 126, 4)              # L_P + K - 1 > C
+    binding.Loop(W, ring, table, 125, 4).destroy()        # exactly fills a region
