@@ -75,8 +75,12 @@ def attend_row(q: torch.Tensor, Kc: torch.Tensor, Vc: torch.Tensor) -> torch.Ten
 class Oracle:
     """Runs each micro-request separately, unpacked, with a private contiguous KV cache per (layer, request)."""
 
-    def __init__(self, cfg, weights: dict, dtype=torch.float64, cache_widened: bool = True):
+    def __init__(self, cfg, weights: dict, dtype=torch.float64, cache_widened: bool = True, window=None):
         self.cfg = cfg
+        # f3 (P:190 "updates the ring buffer's sliding window, discarding stale tokens"; DESIGN.md A8b): with a window W
+        # the row at position p sees positions max(0, p - W + 1)..p of its own request, nothing older.  The oracle's
+        # cache stays linear and unbounded: "wrap == linear window".  None = the whole prefix (v1 semantics).
+        self.window = window
         self.w = weights            # bf16 (or float) CPU tensors, widened to the working dtype on use
         self.dtype = dtype
         self._wide = {} if cache_widened else None   # id(tensor) -> widened copy (same values, kept between calls)
@@ -129,7 +133,8 @@ class Oracle:
             o = torch.empty(n, H, hd, dtype=dt)
             for i in range(n):                                             # O5: row i sees positions 0..p_i
                 p = start_pos + i
-                o[i] = attend_row(q[i], Kc[: p + 1], Vc[: p + 1])
+                lo = 0 if self.window is None else max(0, p - self.window + 1)
+                o[i] = attend_row(q[i], Kc[lo: p + 1], Vc[lo: p + 1])
             x = x + o.reshape(n, H * hd) @ _w(L["wo"], dt).T               # O6 (reading A1)
             xn2 = rmsnorm(x, _w(L["g_mlp"], dt), cfg.rms_eps)              # O7
             g = xn2 @ _w(L["w_gate"], dt).T
@@ -164,7 +169,7 @@ class Oracle:
 
 
 # ------------------------------------------------------------------------------------- brute-force mode
-def brute_forward(cfg, weights: dict, embeds: torch.Tensor) -> torch.Tensor:
+def brute_forward(cfg, weights: dict, embeds: torch.Tensor, window=None) -> torch.Tensor:
     """Pin P1: ONE request of n tokens recomputed with NO cache — full forward over rows 0..n-1 with an explicit
     n x n causal mask, float64 throughout, written independently of Oracle.run_segment (masked dense softmax
     instead of per-row prefixes; explicit per-pair rotation instead of the vectorised rope())."""
@@ -176,7 +181,7 @@ def brute_forward(cfg, weights: dict, embeds: torch.Tensor) -> torch.Tensor:
     mask = torch.zeros(n, n, dtype=torch.bool)
     for i in range(n):
         for j in range(n):
-            mask[i, j] = j <= i
+            mask[i, j] = j <= i and (window is None or i - j < window)      # banded when a window is given (f3)
     ang = torch.zeros(n, half, dtype=dt)
     for p in range(n):
         for c in range(half):
@@ -210,7 +215,7 @@ def brute_forward(cfg, weights: dict, embeds: torch.Tensor) -> torch.Tensor:
 
 
 # ------------------------------------------------------------------------------------- ring index model
-def ring_index_model(R: int, C: int, base, length, segs):
+def ring_index_model(R: int, C: int, base, length, segs, window=0, max_pos=0):
     """Pure-integer model of step a0 / reading A6 (BASELINE.json north_star: "slot (base_r + pos) mod capacity
     of its request's region").  Returns (row_req, row_pos, row_slot, new_length) or raises ValueError with the
     AF_ERR_* name the library must return.  row_slot = req*C + ((base[req] + pos) mod C)."""
@@ -223,8 +228,15 @@ def ring_index_model(R: int, C: int, base, length, segs):
         if start != length[req]:
             raise ValueError("AF_ERR_POSITION")
     for (req, phase, start, n) in segs:
-        if start + n > C:
-            raise ValueError("AF_ERR_CAPACITY")
+        if window <= 0:
+            if start + n > C:
+                raise ValueError("AF_ERR_CAPACITY")
+        else:
+            # f3: a request may outgrow its region; slot (base + pos) mod C then overwrites position pos - C.  Every row
+            # of the step is appended before any row attends, so the first row's window (start - W + 1 ..) must survive
+            # the last row's append (which evicts start + n - 1 - C): n <= C - W + 1.  Positions stay below max_pos.
+            if start + n > (max_pos if max_pos > 0 else C) or (start + n > C and n > C - window + 1):
+                raise ValueError("AF_ERR_CAPACITY")
     row_req, row_pos, row_slot = [], [], []
     new_len = list(length)
     for (req, phase, start, n) in segs:

@@ -327,3 +327,63 @@ def test_pipelined_loop_equals_sequential_frames():
             assert relerr(lg[i], want[f][1][st]) < 1e-9, (t, st)
         prev = cur
     assert got_tok == [w_[0] for w_ in want]
+
+
+# ---------------------------------------------------------------- f3: sliding window inside a request
+def test_window_oracle_against_banded_bruteforce_and_special_cases():
+    """Oracle(window=W) pinned by (1) the cache-free brute force with an explicit banded mask, fed in chunks that the
+    ring rule allows (chunk <= C - W + 1 is a ring matter; the oracle takes any chunking), (2) W >= n == no window,
+    (3) W = 1: every row sees only itself, so attention returns its own v and the layer has a closed form."""
+    cfg, n = SMALL, 37
+    w = I.make_weights(cfg, seed=9)
+    e = I.make_embeds(cfg, 9, 0, n)
+    for W in (1, 5, 16):
+        ref = O.brute_forward(cfg, w, e, window=W)
+        o = O.Oracle(cfg, w, F64, window=W)
+        got, p = [], 0
+        for chunk in (7, 1, 1, 12, 1, 15):
+            got.append(o.step([(0, 0 if chunk > 1 else 1, p, chunk)], e[p:p + chunk]))
+            p += chunk
+        assert p == n and relerr(torch.cat(got), ref) < 1e-9, W
+    full = O.Oracle(cfg, w, F64).step([(0, 0, 0, n)], e)
+    assert relerr(O.Oracle(cfg, w, F64, window=n).step([(0, 0, 0, n)], e), full) < 1e-12
+    assert relerr(O.Oracle(cfg, w, F64, window=n + 50).step([(0, 0, 0, n)], e), full) < 1e-12
+    assert relerr(O.brute_forward(cfg, w, e, window=n), O.brute_forward(cfg, w, e)) < 1e-12
+    # W = 1 closed form, one layer: o = v (softmax over one key), position-independent (RoPE cancels in q.k, v unrotated)
+    one = I.ModelCfg(d_model=64, n_layers=1, n_heads=4, head_dim=16, ffn=80, vocab=40)
+    w1 = I.make_weights(one, seed=10)
+    L = {k: v.to(F64) for k, v in w1["layers"][0].items()}
+    x = I.make_embeds(one, 10, 0, 6).to(F64)
+    xn = O.rmsnorm(x, L["g_attn"], one.rms_eps)
+    h = x + (xn @ L["wv"].T) @ L["wo"].T
+    hn = O.rmsnorm(h, L["g_mlp"], one.rms_eps)
+    want = h + (O.silu(hn @ L["w_gate"].T) * (hn @ L["w_up"].T)) @ L["w_down"].T
+    assert relerr(O.Oracle(one, w1, F64, window=1).step([(3, 0, 0, 6)], x.to(torch.bfloat16)), want) < 1e-12
+
+
+def test_window_index_model_rules():
+    """f3 ring rule: with a window W a request may outgrow its region; a segment that wraps past C must satisfy
+    len <= C - W + 1 (its first row's window must survive its last row's append); brute force over a small ring that
+    the slot of every position a row may attend still holds that position after the step's appends."""
+    R, C = 2, 8
+    for W in (1, 3, 8):
+        for start in range(0, 20):
+            for n in range(1, 9):
+                base, length = [5, 0], [start, 0]
+                try:
+                    _, pos, slot, new_len = O.ring_index_model(R, C, base, length, [(0, 0, start, n)], window=W, max_pos=24)
+                except ValueError as ex:
+                    assert str(ex) == "AF_ERR_CAPACITY"
+                    assert start + n > 24 or (start + n > C and n > C - W + 1)
+                    continue
+                # contents after the appends: slot -> newest position written there
+                held = {}
+                for p in range(0, start + n):
+                    held[(base[0] + p) % C] = p
+                for p in pos:
+                    for j in range(max(0, p - W + 1), p + 1):
+                        assert held[(base[0] + j) % C] == j, (W, start, n, p, j)
+                assert new_len[0] == start + n
+    # without a window the v1 rule stands
+    with pytest.raises(ValueError):
+        O.ring_index_model(R, C, [0, 0], [7, 0], [(0, 1, 7, 1), (1, 0, 0, 9)])
