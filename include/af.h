@@ -122,10 +122,21 @@ int af_ring_create(const af_model_cfg* cfg, const af_ring_cfg* ring, void* kv_me
  * len = 0 and base = new_base mod C if new_base >= 0, else base = (base + len) mod C (keep rotating). O(1), host only. */
 int af_ring_reset_slot(af_ring* ring, int32_t req_id, int32_t new_base);
 
+/* f3 - sliding window inside a request ("updates the ring buffer's sliding window, discarding stale tokens";
+ * DESIGN.md A8b).  window = 0 (the default after af_ring_create) keeps the v1 rule start_pos + len <= capacity.  With
+ * 1 <= window <= capacity a request may grow up to max_pos (>= capacity; 0 = capacity) tokens: the append at position p
+ * goes to slot (base + p) mod C and overwrites position p - C, and the row at position p attends positions
+ * max(0, p - window + 1)..p of its request only.  All rows of a step are appended before any row attends, so a segment
+ * that ends beyond capacity needs len <= capacity - window + 1 (AF_ERR_CAPACITY otherwise, state unchanged).  Every
+ * region must be empty (AF_ERR_POSITION otherwise).  Rebuilds the library's RoPE table for max_pos positions;
+ * synchronises, not hot path. */
+int af_ring_set_window(af_ring* ring, int32_t window, int32_t max_pos);
+
 /* Algorithm 2 for all layers on one packed step.
  *   packed_embeds : device bf16 [T, d_model], T = sum of segment lens, rows in segment-table order (H_CRS, Eq. 1)
  *   segs          : HOST array [n_segs]; each req_id at most once; start_pos == current len of that request;
- *                   start_pos + len <= capacity; phase == AF_PHASE_DECODE requires len == 1.  n_segs == 0 is a no-op.
+ *                   start_pos + len <= capacity (unless af_ring_set_window relaxed it); phase == AF_PHASE_DECODE
+ *                   requires len == 1.  n_segs == 0 is a no-op.
  *   hidden_out    : device fp32 [T, d_model], the residual stream after the last layer (before the final norm)
  *   workspace     : device, 256-byte aligned, >= af_workspace_bytes(cfg, T, n_segs)
  * On success the ring lengths advance: len_r = start_pos + len for every segment (the "ring commit"). */

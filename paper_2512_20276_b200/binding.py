@@ -48,7 +48,7 @@ class af_weights(C.Structure):
                 ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
 
 
-EXPORTS = ["af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
+EXPORTS = ["af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
            "af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
@@ -85,6 +85,8 @@ def load_library():
     L.af_prepare_gate_up.restype = C.c_int
     L.af_ring_create.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg), vp, sz, C.POINTER(vp)]
     L.af_ring_reset_slot.argtypes = [vp, i32, i32]
+    L.af_ring_set_window.argtypes = [vp, i32, i32]
+    L.af_ring_set_window.restype = C.c_int
     L.af_packed_forward.argtypes = [C.POINTER(af_weights), vp, C.POINTER(af_segment), i32, vp, vp, vp, sz, vp]
     L.af_logits_rows.argtypes = [C.POINTER(af_weights), vp, C.POINTER(i32), i32, vp, vp, sz, vp]
     L.af_ring_destroy.argtypes = [vp]
@@ -196,6 +198,9 @@ class Ring:
 
     def reset_slot(self, req_id: int, new_base: int = -1):
         _check(load_library().af_ring_reset_slot(self.handle, req_id, new_base))
+
+    def set_window(self, window: int, max_pos: int = 0):
+        _check(load_library().af_ring_set_window(self.handle, window, max_pos))
 
     def get_state(self, req_id: int):
         b, n = C.c_int32(), C.c_int32()

@@ -210,6 +210,8 @@ static int gemm_global_init() {
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
+  CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   return AF_OK;
 }
 
@@ -475,6 +477,8 @@ struct af_ring {
   float2* rope_tab = nullptr;   // [C][hd/2]
   int max_rows = 0;
   int last_T = 0;
+  int window = 0;               // f3: 0 = none (start_pos + len <= C), else rows see the last `window` positions
+  int max_pos = 0;              // positions stay below this (rows of the RoPE table); = C without a window
 };
 
 static int check_cfg(const af_model_cfg* c) {
@@ -549,6 +553,7 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   af_ring* g = new af_ring();
   g->cfg = *c; g->rc = *r; g->kv = reinterpret_cast<act_t*>(kv_mem);
   g->base.assign(r->n_regions, 0); g->len.assign(r->n_regions, 0);
+  g->max_pos = r->capacity;
   const long long cap_rows = static_cast<long long>(r->n_regions) * r->capacity;
   g->max_rows = static_cast<int>(cap_rows > 65536 ? 65536 : cap_rows);
   const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 4 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1;
@@ -588,6 +593,30 @@ extern "C" int af_ring_reset_slot(af_ring* g, int32_t req, int32_t new_base) {
   return AF_OK;
 }
 
+extern "C" int af_ring_set_window(af_ring* g, int32_t window, int32_t max_pos) {
+  if (!g) return fail(AF_ERR_ARG, "null ring");
+  const int C = g->rc.capacity;
+  if (window < 0 || window > C) return fail(AF_ERR_ARG, "window %d outside [0, capacity %d]", window, C);
+  if (window == 0) max_pos = C;
+  if (max_pos < C) return fail(AF_ERR_ARG, "max_pos %d < capacity %d", max_pos, C);
+  for (int r = 0; r < g->rc.n_regions; ++r)
+    if (g->len[r] != 0) return fail(AF_ERR_POSITION, "af_ring_set_window needs every region empty (request %d has %d tokens)", r, g->len[r]);
+  if (max_pos != g->max_pos) {   // the RoPE table has one row per position
+    float2* tab = nullptr;
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMalloc(&tab, static_cast<size_t>(max_pos) * (g->cfg.head_dim / 2) * sizeof(float2)));
+    const int n = max_pos * (g->cfg.head_dim / 2);
+    rope_table_kernel<<<(n + 255) / 256, 256>>>(tab, max_pos, g->cfg.head_dim, static_cast<double>(g->cfg.rope_theta));
+    int rc = check_launch("rope_table_kernel");
+    if (rc == AF_OK && cudaDeviceSynchronize() != cudaSuccess) rc = fail(AF_ERR_CUDA, "rope table build failed");
+    if (rc) { cudaFree(tab); return rc; }
+    cudaFree(g->rope_tab);
+    g->rope_tab = tab;
+  }
+  g->window = window; g->max_pos = max_pos;
+  return AF_OK;
+}
+
 extern "C" int af_ring_get_state(const af_ring* g, int32_t req, int32_t* base, int32_t* len) {
   if (!g) return fail(AF_ERR_ARG, "null ring");
   if (req < 0 || req >= g->rc.n_regions) return fail(AF_ERR_SEGMENT, "req_id %d outside [0,%d)", req, g->rc.n_regions);
@@ -599,7 +628,7 @@ extern "C" int af_ring_get_state(const af_ring* g, int32_t req, int32_t* base, i
 extern "C" int af_debug_set_len(af_ring* g, int32_t req, int32_t len) {
   if (!g) return fail(AF_ERR_ARG, "null ring");
   if (req < 0 || req >= g->rc.n_regions) return fail(AF_ERR_SEGMENT, "req_id %d outside [0,%d)", req, g->rc.n_regions);
-  if (len < 0 || len > g->rc.capacity) return fail(AF_ERR_CAPACITY, "len %d outside [0,%d]", len, g->rc.capacity);
+  if (len < 0 || len > g->max_pos) return fail(AF_ERR_CAPACITY, "len %d outside [0,%d]", len, g->max_pos);
   g->len[req] = len;
   return AF_OK;
 }
@@ -718,9 +747,16 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     if (segs[s].start_pos != g->len[segs[s].req_id])
       return fail(AF_ERR_POSITION, "segment %d: start_pos %d != current length %d of request %d", s, segs[s].start_pos,
                   g->len[segs[s].req_id], segs[s].req_id);
-  for (int s = 0; s < n_segs; ++s)
-    if (static_cast<long long>(segs[s].start_pos) + segs[s].len > C)
-      return fail(AF_ERR_CAPACITY, "segment %d: start_pos %d + len %d > capacity %d", s, segs[s].start_pos, segs[s].len, C);
+  for (int s = 0; s < n_segs; ++s) {
+    const long long end = static_cast<long long>(segs[s].start_pos) + segs[s].len;
+    if (g->window <= 0) {
+      if (end > C) return fail(AF_ERR_CAPACITY, "segment %d: start_pos %d + len %d > capacity %d", s, segs[s].start_pos, segs[s].len, C);
+    } else if (end > g->max_pos || (end > C && segs[s].len > C - g->window + 1)) {
+      // f3: every row is appended before any row attends, so a wrapping segment's first row must keep its whole window
+      return fail(AF_ERR_CAPACITY, "segment %d: start_pos %d + len %d exceeds max_pos %d, or wraps with len > capacity %d - window %d + 1",
+                  s, segs[s].start_pos, segs[s].len, g->max_pos, C, g->window);
+    }
+  }
   if (T64 > g->max_rows) return fail(AF_ERR_CAPACITY, "%lld packed rows > ring rows %d", T64, g->max_rows);
   const int T = static_cast<int>(T64);
   if (!packed_embeds || !hidden_out) return fail(AF_ERR_ARG, "null embeds / hidden_out");
@@ -788,14 +824,13 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
               static_cast<const act_t*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
               H, hd, R, C);
     // a4: segment-masked causal attention over the ring
-    if (hd == 128)
-      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<128>, dim3(H, n_items), dim3(ATT_THREADS),
-                att_smem_bytes(128), st, static_cast<const act_t*>(ws.q_rot),
-                static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
-    else
-      AF_LAUNCH(PC_ATTENTION, "attention_kernel", attention_kernel<64>, dim3(H, n_items), dim3(ATT_THREADS),
-                att_smem_bytes(64), st, static_cast<const act_t*>(ws.q_rot),
-                static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2);
+    {
+      auto att = hd == 128 ? (g->window > 0 ? attention_kernel<128, true> : attention_kernel<128, false>)
+                           : (g->window > 0 ? attention_kernel<64, true> : attention_kernel<64, false>);
+      AF_LAUNCH(PC_ATTENTION, "attention_kernel", att, dim3(H, n_items), dim3(ATT_THREADS), att_smem_bytes(hd), st,
+                static_cast<const act_t*>(ws.q_rot), static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2,
+                g->window);
+    }
     // a5: O projection, split-K slabs (added to the residual by the next kernel)
     {
       GemmParams gp{};

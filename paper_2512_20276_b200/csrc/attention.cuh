@@ -65,12 +65,14 @@ __device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
   return static_cast<uint32_t>(row * (HD * 2) + ((chunk ^ (row & 7)) << 4));
 }
 
-template <int HD>
+// WIN (f3): rows see only the last `window` positions, max(0, p - window + 1)..p; positions may exceed C, slot
+// (base + j) mod C then holds the newest position congruent to j (af.h: af_ring_set_window).  WIN = false is the v1 kernel.
+template <int HD, bool WIN = false>
 __global__ void __launch_bounds__(ATT_THREADS, 3)
 attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
                  const act_t* __restrict__ kv,    // ring, layer base: [2][R][H][C][HD]
                  act_t* __restrict__ out,         // [T, H*HD]
-                 StepTables tb, int H, int R, int C, float scale_log2) {
+                 StepTables tb, int H, int R, int C, float scale_log2, int window = 0) {
   constexpr int CH = HD / 8;                  // 16-byte chunks per row
   constexpr int TILE_BYTES = ATT_BKV * HD * 2;
   extern __shared__ __align__(128) uint8_t att_smem[];
@@ -87,6 +89,9 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   const int nq = min(ATT_BQ, len - q0);
   const int kv_end = start + q0 + nq;         // positions [0, kv_end) are visible to the tile's last row
   const int n_tiles = (kv_end + ATT_BKV - 1) / ATT_BKV;
+  const int kv_lo = WIN ? max(0, start + q0 - window + 1) : 0;   // lowest position visible to the tile's first row
+  const int tile_lo = WIN ? kv_lo / ATT_BKV : 0;
+  const int W = WIN ? window : (1 << 30);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3;
 
@@ -106,9 +111,10 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
     for (int i = tid; i < ATT_BKV * CH; i += ATT_THREADS) {
       const int r = i / CH, c = i % CH;
       const int j = j0 + r;
-      const bool ok = j < kv_end;
+      const bool ok = j < kv_end && j >= kv_lo;
       int slot = base + (ok ? j : 0);
-      slot = slot >= C ? slot - C : slot;   // (base + j) mod C, base < C and j < C
+      if (WIN) slot %= C;                   // positions may exceed C
+      else slot = slot >= C ? slot - C : slot;   // (base + j) mod C, base < C and j < C
       const size_t off = static_cast<size_t>(slot) * HD + c * 8;
       cp_async16(sK + stage * TILE_BYTES + sw_off<HD>(r, c), kbase + off, ok);
       cp_async16(sV + stage * TILE_BYTES + sw_off<HD>(r, c), vbase + off, ok);
@@ -116,7 +122,7 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   };
 #pragma unroll
   for (int t = 0; t < ATT_STAGES - 1; ++t) {   // prologue: the first ATT_STAGES - 1 tiles (a group each, empty past the end)
-    if (t < n_tiles) load_kv(t, t);
+    if (tile_lo + t < n_tiles) load_kv(tile_lo + t, t);
     cp_async_commit();
   }
 
@@ -130,14 +136,14 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   const int p_lo = start + q0 + warp * 16 + g;   // position of this thread's first row (second = +8)
   const int warp_pmin = start + q0 + warp * 16, warp_pmax = warp_pmin + 15;
 
-  for (int tile = 0; tile < n_tiles; ++tile) {
-    const int stage = tile % ATT_STAGES;
+  for (int tile = tile_lo; tile < n_tiles; ++tile) {
+    const int stage = (tile - tile_lo) % ATT_STAGES;
     // the stage of tile + STAGES - 1 was released at the end of tile - 1
-    if (tile + ATT_STAGES - 1 < n_tiles) load_kv(tile + ATT_STAGES - 1, (tile + ATT_STAGES - 1) % ATT_STAGES);
+    if (tile + ATT_STAGES - 1 < n_tiles) load_kv(tile + ATT_STAGES - 1, (tile - tile_lo + ATT_STAGES - 1) % ATT_STAGES);
     cp_async_commit();
     cp_async_wait<ATT_STAGES - 1>();
     __syncthreads();
-    if (tile == 0) {
+    if (tile == tile_lo) {
 #pragma unroll
       for (int kk = 0; kk < HD / 16; ++kk) {
         const int r = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
@@ -146,7 +152,7 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
       }
     }
     const int j0 = tile * ATT_BKV;
-    if (warp_active && j0 <= warp_pmax) {
+    if (warp_active && j0 <= warp_pmax && (!WIN || j0 + ATT_BKV - 1 > warp_pmin - W)) {
       const uint8_t* cK = sK + stage * TILE_BYTES;
       const uint8_t* cV = sV + stage * TILE_BYTES;
       float s[ATT_BKV / 8][4];
@@ -166,14 +172,14 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
       }
       // ---- causal mask within the request + online softmax (base-2 exponent) ----
       float mx[2] = {-INFINITY, -INFINITY};
-      if (j0 + ATT_BKV - 1 > warp_pmin) {   // the tile crosses the diagonal of one of the warp's rows
+      if (j0 + ATT_BKV - 1 > warp_pmin || (WIN && j0 <= warp_pmax - W)) {   // the tile crosses the diagonal (or the window's lower edge) of one of the warp's rows
 #pragma unroll
         for (int nb = 0; nb < ATT_BKV / 8; ++nb) {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const int j = j0 + nb * 8 + 2 * t + (e & 1);
             const int p = p_lo + (e >> 1) * 8;
-            const float v = (j <= p) ? s[nb][e] * scale_log2 : -INFINITY;
+            const float v = (j <= p && (!WIN || j > p - W)) ? s[nb][e] * scale_log2 : -INFINITY;
             s[nb][e] = v;
             mx[e >> 1] = fmaxf(mx[e >> 1], v);
           }

@@ -20,13 +20,17 @@ def relmax(got: torch.Tensor, ref: torch.Tensor) -> float:
 class Pair:
     """One CUDA ring + one oracle fed the same steps; checks bookkeeping bit-exactly and tensors to TOL."""
 
-    def __init__(self, cfg, host_weights, R, C, max_rows, bases=None, oracle_dtype=torch.float64, dev_weights=None):
+    def __init__(self, cfg, host_weights, R, C, max_rows, bases=None, oracle_dtype=torch.float64, dev_weights=None,
+                 window=0, max_pos=0):
         from paper_2512_20276_b200 import binding
         self.binding = binding
         self.cfg, self.R, self.C = cfg, R, C
         self.W = dev_weights if dev_weights is not None else binding.Weights(cfg, host_weights)
         self.ring = binding.Ring(cfg, R, C, max_rows=max_rows)
-        self.orc = O.Oracle(cfg, host_weights, oracle_dtype)
+        self.window, self.max_pos = window, max_pos
+        if window:
+            self.ring.set_window(window, max_pos)                      # f3: sliding window inside a request
+        self.orc = O.Oracle(cfg, host_weights, oracle_dtype, window=window or None)
         self.base = [0] * R
         self.len = [0] * R
         if bases is not None:
@@ -42,7 +46,7 @@ class Pair:
     def step(self, segs, embeds, check=True, oracle=True):
         """Returns (gpu_hidden, oracle_hidden or None)."""
         hid = self.ring.packed_forward(self.W, embeds.cuda(), segs)
-        mr, mp, ms, new_len = O.ring_index_model(self.R, self.C, self.base, self.len, segs)
+        mr, mp, ms, new_len = O.ring_index_model(self.R, self.C, self.base, self.len, segs, self.window, self.max_pos)
         rr, rp, rs = self.ring.row_map(len(mr))
         assert (rr, rp, rs) == (mr, mp, ms), "device row map differs from the index model (must be bit-exact)"
         self.len = new_len
@@ -65,8 +69,10 @@ class Pair:
                 n = self.len[r]
                 if n == 0:
                     continue
-                slots = torch.tensor([(self.base[r] + j) % self.C for j in range(n)], device=kv.device)
+                lo = max(0, n - self.C)                                # older positions were overwritten (f3)
+                slots = torch.tensor([(self.base[r] + j) % self.C for j in range(lo, n)], device=kv.device)
                 Kc, Vc = self.orc.cache(l, r)
+                Kc, Vc = Kc[lo:], Vc[lo:]
                 k_gpu = kv[l, 0, r].index_select(1, slots).permute(1, 0, 2)     # [n, H, hd]
                 v_gpu = kv[l, 1, r].index_select(1, slots).permute(1, 0, 2)
                 worst = max(worst, relmax(k_gpu, Kc), relmax(v_gpu, Vc))

@@ -115,3 +115,72 @@ def test_loop_create_rejects_bad_geometry(binding):
     with pytest.raises(binding.AfError):
         binding.Loop(W, ring, table, 126, 4)              # L_P + K - 1 > C
     binding.Loop(W, ring, table, 125, 4).destroy()        # exactly fills a region
+
+
+# ------------------------------------------------------------------------------------------------ f3: sliding window
+@pytest.mark.parametrize("W", [128, 40, 1])
+def test_f3_sliding_window_tiny(binding, W):
+    """A request outgrows its region: appends overwrite the oldest slots, rows attend the last W positions.  The oracle
+    keeps a linear unbounded cache and a banded mask ("wrap == linear window").  Covers W = C (decode-only sliding),
+    W < C with wrapping prefill chunks of the largest legal length C - W + 1, W = 1, rejected segments, and the
+    live C positions of the ring against the oracle's cache."""
+    from af_harness import Pair
+    cfg, R, C, max_pos = I.CFG_TINY, 3, 128, 400
+    hw = I.make_weights(cfg, seed=0)
+    P = Pair(cfg, hw, R, C, max_rows=3 * C, bases=[100, 0, 77], window=W, max_pos=max_pos)
+    big = C - W + 1                                        # largest chunk that may wrap
+    pos = [0, 0, 0]
+    step = [0]
+
+    def run(segs):
+        T = sum(s[3] for s in segs)
+        hid, ref = P.step(segs, I.make_embeds(cfg, 6, step[0], T))
+        step[0] += 1
+        for s in segs:
+            pos[s[0]] += s[3]
+        return hid, ref
+
+    run([(0, 0, 0, 100), (1, 0, 0, 128), (2, 0, 0, 60)])                   # inside the regions: v1 behaviour (+ window)
+    # request 1 is full: one more token is legal only through the window rule
+    for _ in range(3):
+        run([(0, 1, pos[0], 1), (1, 1, pos[1], 1), (2, 1, pos[2], 1)])
+    if big > 1:                                                           # a wrapping chunk of the largest legal length
+        n = min(big, 120)
+        run([(0, 0, pos[0], n), (1, 1, pos[1], 1)])
+        with pytest.raises(binding.AfError):                              # one row more than the rule allows
+            P.ring.packed_forward(P.W, I.make_embeds(cfg, 6, 99, big + 1).cuda(), [(1, 0, pos[1], big + 1)])
+    else:
+        with pytest.raises(binding.AfError):                              # W = C: only single tokens may slide
+            P.ring.packed_forward(P.W, I.make_embeds(cfg, 6, 99, 2).cuda(), [(1, 0, pos[1], 2)])
+    for r in range(R):
+        assert P.ring.get_state(r) == (P.base[r], P.len[r])               # a rejected step leaves the state unchanged
+    hid = ref = None
+    for _ in range(4):                                                    # keep sliding: decodes + small chunks
+        segs = [(1, 1, pos[1], 1), (2, 0, pos[2], min(big, 33))]
+        hid, ref = run(segs)
+    assert pos[1] > C
+    P.check_ring([0, 1, 2])
+    P.check_logits(hid, ref, I.prediction_rows(segs))
+    with pytest.raises(binding.AfError):                                  # positions stay below max_pos
+        P.ring.set_len(1, max_pos - 1)
+        P.ring.packed_forward(P.W, I.make_embeds(cfg, 6, 98, 2).cuda(), [(1, 0, max_pos - 1, 2)])
+
+
+def test_f3_window_base_invariance_and_reset(binding):
+    """Bitwise: the windowed path gives identical results for any base rotation (KV tiles are walked in logical order),
+    and af_ring_set_window refuses a non-empty ring."""
+    cfg, C, W = I.CFG_TINY, 128, 64
+    W_dev = binding.Weights(cfg, I.make_weights(cfg, seed=0))
+    outs = []
+    for b in (0, 93):
+        ring = binding.Ring(cfg, 2, C, max_rows=C)
+        ring.set_window(W, 300)
+        ring.reset_slot(0, b)
+        p, hid = 0, None
+        for i, n in enumerate((128, 1, 40, 1, 65, 1)):
+            hid = ring.packed_forward(W_dev, I.make_embeds(cfg, 8, i, n).cuda(), [(0, 0 if n > 1 else 1, p, n)])
+            p += n
+        outs.append(hid.cpu())
+        with pytest.raises(binding.AfError):
+            ring.set_window(0, 0)
+    assert torch.equal(outs[0], outs[1])
