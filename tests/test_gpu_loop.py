@@ -184,3 +184,62 @@ def test_f3_window_base_invariance_and_reset(binding):
         with pytest.raises(binding.AfError):
             ring.set_window(0, 0)
     assert torch.equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------------------------------------ 7B shapes (hd = 128)
+def test_f3_sliding_window_single_7b_layer(binding):
+    """f3 at the Llama-2-7B layer shape (hd = 128 instantiation of the windowed attention kernel), ring 4 x 512,
+    W = 256: the paper's 276-row prefill, then the request keeps growing past the region by decodes and by wrapping
+    chunks of the largest legal length (257), packed with a second request that stays inside its region; fp32 oracle."""
+    from af_harness import Pair
+    cfg, C, W = I.CFG_7B_1L, 512, 256
+    hw = I.make_weights(cfg, seed=1)
+    P = Pair(cfg, hw, R=4, C=C, max_rows=320, bases=[400, 0, 17, 511], oracle_dtype=torch.float32, window=W, max_pos=1200)
+    P.step([(0, 0, 0, 276), (1, 0, 0, 40)], I.make_embeds(cfg, 3, 0, 316))
+    P.step([(0, 0, 276, 230), (1, 1, 40, 1)], I.make_embeds(cfg, 3, 1, 231))           # ends at 506, inside the region
+    P.step([(0, 0, 506, 257), (1, 1, 41, 1)], I.make_embeds(cfg, 3, 2, 258))           # wraps: len = C - W + 1
+    P.step([(0, 1, 763, 1), (1, 1, 42, 1)], I.make_embeds(cfg, 3, 3, 2))
+    segs = [(0, 0, 764, 130), (1, 1, 43, 1), (2, 0, 0, 100)]
+    hid, ref = P.step(segs, I.make_embeds(cfg, 3, 4, 231))
+    P.check_ring([0, 1, 2])
+    P.check_logits(hid, ref, I.prediction_rows(segs))
+    with pytest.raises(binding.AfError):
+        P.ring.packed_forward(P.W, I.make_embeds(cfg, 3, 5, 258).cuda(), [(0, 0, 894, 258)])
+
+
+def test_device_loop_7b_shape_equals_host_driven_steps(binding):
+    """f1 at bench.py's launch configuration (8-layer slice of the 7B shape, L_P = 276, K = 7, ring 8 x 512, graph
+    replay): pipeline fill, the captured step and 6 replays with a region recycle are bit-identical (hidden, logits,
+    tokens, row map) to the same steps issued through the host-driven calls, whose parity against the oracle is
+    tests/test_gpu_7b.py's subject."""
+    cfg = I.cfg_7b_layers(8)
+    L_P, K, R, C, n_steps = 276, 7, 8, 512, 14
+    W = binding.Weights(cfg, I.make_weights(cfg, seed=2, threads=16))
+    table = (0.5 * torch.randn(cfg.vocab, cfg.d_model, generator=torch.Generator().manual_seed(9))).to(torch.bfloat16).cuda()
+    ring, host = binding.Ring(cfg, R, C, max_rows=288), binding.Ring(cfg, R, C, max_rows=288)
+    loop = binding.Loop(W, ring, table, L_P, K)
+    st = torch.cuda.Stream()
+    base, length, prev = [0] * R, [0] * R, None
+    for t in range(n_steps):
+        segs = I.steady_schedule(t, L_P, K, R)
+        n_dec = len(segs) - 1
+        e = I.make_embeds(cfg, 2, t, L_P).cuda()
+        with torch.cuda.stream(st):
+            loop.prefill_embeds.copy_(e)
+            loop.step(use_graph=True, stream=st)
+        st.synchronize()
+        base[t % R], length[t % R] = O.ring_reset_model(C, base[t % R], length[t % R], -1)
+        mr, mp, ms, length = O.ring_index_model(R, C, base, length, segs)
+        assert ring.row_map(len(mr)) == (mr, mp, ms)
+        host.reset_slot(t % R, -1)
+        emb = torch.cat([e, binding.embed_rows(table, prev[:n_dec])]) if n_dec else e
+        hid = host.packed_forward(W, emb, segs)
+        lg = host.logits_rows(W, hid, I.prediction_rows(segs))
+        prev = binding.argmax_rows(lg)
+        assert torch.equal(loop.hidden[:L_P + n_dec], hid), t
+        assert torch.equal(loop.logits[:1 + n_dec], lg), t
+        assert torch.equal(loop.tokens[:1 + n_dec], prev), t
+        assert loop.tokens[:1 + n_dec].cpu().tolist() == O.argmax_rows(lg.cpu())
+    fr = loop.frame.cpu().tolist()
+    assert fr[0] == n_steps - K
+    loop.destroy()
