@@ -147,6 +147,59 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------- library GEMM context
+def run_library_gemm(args):
+    """Context for roofline.frac, not a product path: what the vendor library (cuBLAS through torch.matmul, fp16 in,
+    fp32 accumulate) reaches on the step's own projection shapes, T = 282 packed rows against [out, in] weights, with a
+    different weight matrix every call (8 per shape, > L2 in total) as in a real step.  Same GPU, same process, CUDA
+    events around 64 back-to-back calls after 16 warm-up calls.  Prints one JSON line; summarised in profiles/."""
+    import torch
+    torch.cuda.set_device(0)
+    T, D, F = L_P + K_STAGES - 1, 4096, 11008
+    shapes = [("qkv", 3 * D, D), ("o", D, D), ("gate_up", 2 * F, D), ("down", D, F)]
+    g = torch.Generator(device="cuda").manual_seed(SEED)
+    ws = {n: [(0.02 * torch.randn(o, k, generator=g, device="cuda")).half() for _ in range(8)] for n, o, k in shapes}
+    xs = {n: torch.randn(T, k, generator=g, device="cuda").half() for n, o, k in shapes}
+
+    def layers(n_layers, events=None):
+        for l in range(n_layers):
+            for name, _, _ in shapes:
+                if events is not None:
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                torch.matmul(xs[name], ws[name][l % 8].t())
+                if events is not None:
+                    e1.record()
+                    events[name].append((e0, e1))
+
+    sampler = ClockSampler(0)
+    layers(32 * 300)                                     # ~1.3 s: reach the power-capped clock a long step runs at
+    torch.cuda.synchronize()
+    sampler.start()
+    # (a) back to back, as a library user would chain them: one pair of events around 32 x 64 layers
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    layers(32 * 64)
+    e1.record()
+    torch.cuda.synchronize()
+    chained_us = e0.elapsed_time(e1) / (32 * 64) * 1e3
+    # (b) per launch events, the way bench.py's kernel_ms_per_step times this library's own GEMM launches
+    ev = {n: [] for n, _, _ in shapes}
+    layers(32 * 20, ev)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    out = {}
+    for name, n_out, k in shapes:
+        us = sum(a.elapsed_time(b) for a, b in ev[name]) / len(ev[name]) * 1e3
+        out[name] = {"us_per_call": us, "tflops": 2.0 * T * n_out * k / us / 1e6, "weight_gbs": 2.0 * n_out * k / us / 1e3}
+    layer_us = sum(v["us_per_call"] for v in out.values())
+    flops = 2.0 * T * (4 * D * D + 3 * D * F)
+    print(json.dumps({"what": "cuBLAS (torch.matmul fp16) on the step's projection shapes, T = 282, cold weights",
+                      "per_shape_event_timed": out, "layer_gemm_us_event_timed": layer_us,
+                      "layer_tflops_event_timed": flops / layer_us / 1e6, "layer_gemm_us_chained": chained_us,
+                      "layer_tflops_chained": flops / chained_us / 1e6, "clocks": clocks}), flush=True)
+
+
 # ---------------------------------------------------------------------------------------------- cfg5 sweep
 def run_sweep(args):
     """BASELINE.json configs[4]: concurrent decodes x prefill length at the 7B shape.  Prints one markdown table row per
@@ -216,9 +269,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
     ap.add_argument("--chunks", action="store_true", help="with --sweep: the longer-action-chunk points K = 7, 16, 24, 32 (276-row prefill + K - 1 decodes)")
+    ap.add_argument("--library-gemm", action="store_true", help="context only: cuBLAS on the step's projection shapes (one JSON line)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.library_gemm:
+        return run_library_gemm(args)
     if args.sweep or args.chunks:
         return run_sweep(args)
 
