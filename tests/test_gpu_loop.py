@@ -243,3 +243,39 @@ def test_device_loop_7b_shape_equals_host_driven_steps(binding):
     fr = loop.frame.cpu().tolist()
     assert fr[0] == n_steps - K
     loop.destroy()
+
+
+@pytest.mark.parametrize("K,R,L_P", [(1, 1, 128), (2, 2, 17), (5, 5, 1)])
+def test_device_loop_edge_shapes(binding, K, R, L_P):
+    """Degenerate pipelines: no decode stage at all (K = 1, a region that is filled exactly and recycled every step),
+    as many stages as regions (every region recycled the step after its frame completes), one-row prefills.
+    Tokens and logits bit-identical to the host-driven steps, device table == index model."""
+    cfg, C, n_steps = I.CFG_TINY, 128, 9
+    W = binding.Weights(cfg, I.make_weights(cfg, seed=0))
+    table = _table(cfg, 43).cuda()
+    ring, host = binding.Ring(cfg, R, C, max_rows=128), binding.Ring(cfg, R, C, max_rows=128)
+    loop = binding.Loop(W, ring, table, L_P, K)
+    st = torch.cuda.Stream()
+    base, length, prev = [0] * R, [0] * R, None
+    for t in range(n_steps):
+        segs = I.steady_schedule(t, L_P, K, R)
+        n_dec = len(segs) - 1
+        e = I.make_embeds(cfg, 43, t, L_P).cuda()
+        with torch.cuda.stream(st):
+            loop.prefill_embeds.copy_(e)
+            loop.step(use_graph=True, stream=st)
+        st.synchronize()
+        base[t % R], length[t % R] = O.ring_reset_model(C, base[t % R], length[t % R], -1)
+        mr, mp, ms, length = O.ring_index_model(R, C, base, length, segs)
+        assert ring.row_map(len(mr)) == (mr, mp, ms)
+        host.reset_slot(t % R, -1)
+        emb = torch.cat([e, binding.embed_rows(table, prev[:n_dec])]) if n_dec else e
+        hid = host.packed_forward(W, emb, segs)
+        lg = host.logits_rows(W, hid, I.prediction_rows(segs))
+        prev = binding.argmax_rows(lg)
+        assert torch.equal(loop.logits[:1 + n_dec], lg) and torch.equal(loop.tokens[:1 + n_dec], prev), t
+        fr = loop.frame.cpu().tolist()
+        assert fr[0] == (t - (K - 1) if t >= K - 1 else -1)
+        if t >= K - 1:
+            assert fr[K] == int(prev[K - 1])
+    loop.destroy()
