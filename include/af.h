@@ -185,7 +185,9 @@ int af_embed_rows(const void* table, int32_t vocab, int32_t d_model, const int32
  *     logits = fp32 [1 + n_dec, vocab] of the last step (prediction rows in stage order); tokens = int32 [1 + n_dec]
  *     tokens of the last step by stage; frame = int32 [1 + chunk_k]: {frame id, its chunk_k tokens} of the last
  *     COMPLETED frame (id -1 while the pipeline fills).
- *   af_loop_step : enqueues step t on cuda_stream and advances the host mirror. */
+ *   af_loop_step : enqueues step t on cuda_stream and advances the host mirror.  If a launch fails (AF_ERR_CUDA) the
+ *     loop and its ring are left in an unspecified state and must be destroyed.
+ *   af_loop_steps_done : t, the number of steps enqueued so far (-1 for a NULL loop). */
 typedef struct af_loop af_loop;
 int af_loop_create(const af_weights* w, af_ring* ring, const void* embed_table, int32_t prefill_len, int32_t chunk_k,
                    void* workspace, size_t ws_bytes, af_loop** out);
