@@ -148,13 +148,14 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------- library GEMM context
-def run_library_gemm(args):
+def run_library_gemm(args, emit=True):
     """Context for roofline.frac, not a product path: what the vendor library (cuBLAS through torch.matmul, fp16 in,
     fp32 accumulate) reaches on the step's own projection shapes, T = 282 packed rows against [out, in] weights, with a
     different weight matrix every call (8 per shape, > L2 in total) as in a real step.  Same GPU, same process, CUDA
     events around 64 back-to-back calls after 16 warm-up calls.  Prints one JSON line; summarised in profiles/."""
     import torch
-    torch.cuda.set_device(0)
+    if emit:
+        torch.cuda.set_device(0)
     T, D, F = L_P + K_STAGES - 1, 4096, 11008
     shapes = [("qkv", 3 * D, D), ("o", D, D), ("gate_up", 2 * F, D), ("down", D, F)]
     g = torch.Generator(device="cuda").manual_seed(SEED)
@@ -172,7 +173,7 @@ def run_library_gemm(args):
                     e1.record()
                     events[name].append((e0, e1))
 
-    sampler = ClockSampler(0)
+    sampler = ClockSampler(torch.cuda.current_device())
     layers(32 * 300)                                     # ~1.3 s: reach the power-capped clock a long step runs at
     torch.cuda.synchronize()
     sampler.start()
@@ -194,10 +195,13 @@ def run_library_gemm(args):
         out[name] = {"us_per_call": us, "tflops": 2.0 * T * n_out * k / us / 1e6, "weight_gbs": 2.0 * n_out * k / us / 1e3}
     layer_us = sum(v["us_per_call"] for v in out.values())
     flops = 2.0 * T * (4 * D * D + 3 * D * F)
-    print(json.dumps({"what": "cuBLAS (torch.matmul fp16) on the step's projection shapes, T = 282, cold weights",
-                      "per_shape_event_timed": out, "layer_gemm_us_event_timed": layer_us,
-                      "layer_tflops_event_timed": flops / layer_us / 1e6, "layer_gemm_us_chained": chained_us,
-                      "layer_tflops_chained": flops / chained_us / 1e6, "clocks": clocks}), flush=True)
+    res = {"what": "cuBLAS (torch.matmul fp16) on the step's projection shapes, T = 282, cold weights",
+           "per_shape_event_timed": out, "layer_gemm_us_event_timed": layer_us,
+           "layer_tflops_event_timed": flops / layer_us / 1e6, "layer_gemm_us_chained": chained_us,
+           "layer_tflops_chained": flops / chained_us / 1e6, "clocks": clocks}
+    if emit:
+        print(json.dumps(res), flush=True)
+    return res
 
 
 # ---------------------------------------------------------------------------------------------- cfg5 sweep
@@ -269,6 +273,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
     ap.add_argument("--chunks", action="store_true", help="with --sweep: the longer-action-chunk points K = 7, 16, 24, 32 (276-row prefill + K - 1 decodes)")
+    ap.add_argument("--no-library-context", action="store_true", help="skip the cuBLAS same-shape context pass of the bench line")
     ap.add_argument("--library-gemm", action="store_true", help="context only: cuBLAS on the step's projection shapes (one JSON line)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -448,6 +453,16 @@ def main():
                            "kernel_nodes_per_step": launches_graph / args.steps},
         "gpu_launches": launches, "clocks": clocks,
     }
+    if world == 1 and args.layers == 32 and not args.no_library_context:
+        # context, not a product path: the vendor library's GEMMs on the same four shapes, timed the same way
+        # (per-launch CUDA events, power-capped clock); see profiles/library_gemm_r1.md
+        lib = run_library_gemm(args, emit=False)
+        ours_layer_us = sum(prof[k][0] for k in gemm_classes[:4]) / n_prof / cfg.n_layers * 1e3
+        line["roofline"]["library_same_shapes"] = {
+            "what": "cuBLAS fp16 (torch.matmul) on QKV / O / gate|up / down at T = 282, cold weights, event-timed per launch",
+            "layer_gemm_us": lib["layer_gemm_us_event_timed"], "tflops": lib["layer_tflops_event_timed"],
+            "frac_of_peak": lib["layer_tflops_event_timed"] / peaks["tf_sustained"],
+            "this_library_layer_gemm_us": ours_layer_us, "sm_mhz": lib["clocks"]["sm_mhz"]}
     if not args.no_cpu_baseline:
         from oracle import af_oracle as O
         n_sl = 2
