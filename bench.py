@@ -204,6 +204,59 @@ def run_library_gemm(args, emit=True):
     return res
 
 
+# ---------------------------------------------------------------------------------------------- GEMM timeline
+def run_gemm_timeline(args):
+    """Report for profiles/: af_debug_trace's %globaltimer stamps of the GEMM launches of two steady cfg3 steps on a
+    2-layer slice (same shapes and launch configuration as the bench step), as min / median / max over CTAs in us
+    after the launch's first CTA starts.  One markdown table row per launch."""
+    import ctypes as C
+    import numpy as np
+    import torch
+    from paper_2512_20276_b200 import binding, inputs as I
+    torch.cuda.set_device(0)
+    L = binding.load_library()
+    cfg = I.cfg_7b_layers(2)
+    W = binding.Weights(cfg, I.make_weights(cfg, SEED, threads=16))
+    ring = binding.Ring(cfg, R_REGIONS, CAPACITY, max_rows=288)
+
+    def step(t):
+        ring.reset_slot(t % R_REGIONS, -1)
+        segs = I.steady_schedule(t, L_P, K_STAGES, R_REGIONS)
+        ring.packed_forward(W, I.make_embeds(cfg, SEED, t, I.total_rows(segs)).cuda(), segs)
+
+    for t in range(12):
+        step(t)
+    torch.cuda.synchronize()
+    L.af_debug_trace.argtypes, L.af_debug_trace.restype = [C.c_int], C.c_int
+    L.af_debug_trace_read.argtypes, L.af_debug_trace_read.restype = [C.c_void_p, C.c_void_p], C.c_int
+    L.af_debug_trace(1)
+    step(12)
+    step(13)
+    torch.cuda.synchronize()
+    st, meta = np.zeros((16, 160, 32), dtype=np.int64), np.zeros((16, 2), dtype=np.int32)
+    L.af_debug_trace_read(st.ctypes.data, meta.ctypes.data)
+    L.af_debug_trace(0)
+    cols = [("released (producer past griddepcontrol.wait)", 25), ("producer requested its last stage", 26),
+            ("piece 0: accumulator ready", 3), ("piece 0: drained", 5), ("piece 1: accumulator ready", 7),
+            ("piece 1: fix-up loaded", 8), ("piece 1: drained", 9)]
+    names = ["QKV", "O", "gate/up", "down", "LM head"]
+    print("| launch | grid | first CTA .. last CTA start | " + " | ".join(c[0] for c in cols) + " |")
+    print("|---|---|---|" + "---|" * len(cols))
+    for li in range(16):
+        cat, grid = int(meta[li][0]), int(meta[li][1])
+        if grid <= 0 or li >= 8:
+            continue
+        s = st[li, :grid]
+        t0 = s[:, 0][s[:, 0] > 0].min()
+
+        def rel(col):
+            v = s[:, col].astype(np.float64)
+            v[s[:, col] == 0] = np.nan
+            v = (v - t0) / 1e3
+            return "-" if np.all(np.isnan(v)) else f"{np.nanmin(v):.1f} / {np.nanmedian(v):.1f} / {np.nanmax(v):.1f}"
+        print(f"| {names[cat] if cat < 5 else cat} | {grid} | {rel(0)} | " + " | ".join(rel(c[1]) for c in cols) + " |")
+
+
 # ---------------------------------------------------------------------------------------------- cfg5 sweep
 def run_sweep(args):
     """BASELINE.json configs[4]: concurrent decodes x prefill length at the 7B shape.  Prints one markdown table row per
@@ -274,12 +327,15 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
     ap.add_argument("--chunks", action="store_true", help="with --sweep: the longer-action-chunk points K = 7, 16, 24, 32 (276-row prefill + K - 1 decodes)")
     ap.add_argument("--no-library-context", action="store_true", help="skip the cuBLAS same-shape context pass of the bench line")
+    ap.add_argument("--gemm-timeline", action="store_true", help="report only: af_debug_trace timeline of the GEMM launches of a steady step (markdown table)")
     ap.add_argument("--library-gemm", action="store_true", help="context only: cuBLAS on the step's projection shapes (one JSON line)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.library_gemm:
         return run_library_gemm(args)
+    if args.gemm_timeline:
+        return run_gemm_timeline(args)
     if args.sweep or args.chunks:
         return run_sweep(args)
 
