@@ -92,55 +92,75 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------------------------- reference arm
-def oracle_frame_sample(cfg_full, host_weights_slice, n_layers_slice, prefill_rows, n_decodes, seed, torch, O, I):
-    """One frame of the paper's Baseline schedule on an n-layer slice: prefill, then decodes one by one,
-    then the LM head on the prediction rows.  Returns seconds."""
-    cfg = I.ModelCfg(**{**cfg_full.as_dict(), "n_layers": n_layers_slice})
-    orc = O.Oracle(cfg, host_weights_slice, torch.float32)
-    e = I.make_embeds(cfg, seed, 0, prefill_rows + n_decodes)
+def bench_config(layers=32):
+    """The `config` object of the bench line; the reference arm prints the same one (same workload, same keys)."""
+    return {"workload": WORKLOAD if layers == 32 else f"DEBUG {layers}-layer slice of " + WORKLOAD,
+            "precision": "bf16-valued weights stored as fp16 (af_convert_bf16_to_fp16 at load; exact for 2^-14 <= |w| <= "
+                         "65504, smaller values round to fp16 subnormals, abs err <= 2^-25), fp16 activations and KV "
+                         "ring, fp32 accumulate / residual / logits (tcgen05 kind::f16)",
+            "packed_rows": L_P + K_STAGES - 1, "ring": f"{R_REGIONS} regions x {CAPACITY}",
+            "multi_gpu": "independent replicas",
+            "l2": "inputs larger than L2 (13.2 GB of weights streamed per step vs 126 MB L2)"}
+
+
+def oracle_frame(orc, cfg, seed, frame, torch, I):
+    """One WHOLE frame of the paper's Baseline schedule through the oracle as it stands: the 276-row prefill,
+    then the 6 decodes one by one (each alone, unpacked), then the LM head on the 7 prediction rows.  Returns seconds."""
+    n_dec = K_STAGES - 1
+    e = I.make_embeds(cfg, seed, frame, L_P + n_dec)
     t0 = time.perf_counter()
-    hid = [orc.step([(0, 0, 0, prefill_rows)], e[:prefill_rows])[-1:]]
-    for s in range(n_decodes):
-        hid.append(orc.step([(0, 1, prefill_rows + s, 1)], e[prefill_rows + s:prefill_rows + s + 1]))
-    t_layers = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    orc.logits(torch.cat(hid), list(range(1 + n_decodes)))
-    return t_layers, time.perf_counter() - t0
+    orc.reset(0)
+    hid = [orc.step([(0, 0, 0, L_P)], e[:L_P])[-1:]]
+    for s in range(n_dec):
+        hid.append(orc.step([(0, 1, L_P + s, 1)], e[L_P + s:L_P + s + 1]))
+    orc.logits(torch.cat(hid), list(range(1 + n_dec)))
+    return time.perf_counter() - t0
+
+
+def oracle_cores():
+    return max(1, (os.cpu_count() or 4) - 2)       # leave two cores free: an oversubscribed OpenMP pool collapses
 
 
 def run_reference(args):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  A step is one whole 32-layer frame
+    (nothing is extrapolated); only when steps + warmup whole frames would not end within ~4 minutes is the layer count
+    of every step's sample reduced, and the line then says so."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     import torch
     from oracle import af_oracle as O
     from paper_2512_20276_b200 import inputs as I
-    cfg = I.CFG_7B
-    slice_cfg = I.cfg_7b_layers(1)
-    hw = I.make_weights(slice_cfg, SEED)
-    cores = max(1, (os.cpu_count() or 4) - 2)      # leave two cores free: an oversubscribed OpenMP pool collapses
+    cores = oracle_cores()
     torch.set_num_threads(cores)
-    # size the per-step sample so K+W steps end within ~150 s: time the full 1-layer frame once, shrink rows if needed
-    t_full, t_lm = oracle_frame_sample(cfg, hw, 1, L_P, K_STAGES - 1, SEED, torch, O, I)
-    budget = 150.0 / max(1, args.steps + args.warmup)
-    rows = L_P if t_full + t_lm <= budget else max(8, int(L_P * budget / (t_full + t_lm)))
-    ndec = K_STAGES - 1 if rows == L_P else max(1, int((K_STAGES - 1) * rows / L_P))
-    times = []
-    for i in range(args.warmup + args.steps):
-        tl, tm = oracle_frame_sample(cfg, hw, 1, rows, ndec, SEED, torch, O, I)
-        if i >= args.warmup:
-            times.append((tl, tm))
-    tl = sum(t[0] for t in times) / len(times)
-    tm = sum(t[1] for t in times) / len(times)
-    # scale the sample to one full frame: layers x (rows ratio) for the layer stack, LM head once
-    frame_s = cfg.n_layers * tl * (L_P + K_STAGES - 1) / (rows + ndec) + tm
-    fps = 1.0 / frame_s
-    sample = (f"1 of 32 layers, {rows}-row prefill + {ndec} sequential decodes + LM head on {1 + ndec} rows per step; "
-              f"frame time = 32 x layer time x {(L_P + K_STAGES - 1)}/{rows + ndec} + LM head")
+    warmup = max(1, args.warmup)
+    cfg = I.cfg_7b_layers(args.layers)
+    hw = I.make_weights(cfg, SEED, threads=max(4, os.cpu_count() or 8))
+    orc = O.Oracle(cfg, hw, torch.float32)
+    t_first = oracle_frame(orc, cfg, SEED, 0, torch, I)              # warm-up frame 1 (also sizes the run)
+    n_layers = cfg.n_layers
+    budget = 240.0
+    if t_first * (args.steps + warmup) > budget and n_layers > 1:
+        n_layers = max(1, int(cfg.n_layers * budget / (t_first * (args.steps + warmup))))
+        cfg_s = I.cfg_7b_layers(n_layers)
+        orc = O.Oracle(cfg_s, {"layers": hw["layers"][:n_layers], "g_final": hw["g_final"], "w_lm": hw["w_lm"]}, torch.float32)
+    else:
+        cfg_s = cfg
+    for i in range(1, warmup):
+        oracle_frame(orc, cfg_s, SEED, i, torch, I)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        oracle_frame(orc, cfg_s, SEED, warmup + i, torch, I)
+    step_s = (time.perf_counter() - t0) / args.steps
+    fps = 1.0 / step_s
+    sample = (f"{n_layers} of {cfg.n_layers} layers; every step is one whole frame through the oracle (276-row prefill + 6 "
+              f"sequential single-row decodes + LM head on 7 rows), {args.steps} timed frames after {warmup} warm-up frames")
+    if n_layers != cfg.n_layers:
+        sample += f"; REDUCED SAMPLE: value and ms_per_step are those of the {n_layers}-layer frame actually run, not of the full stack"
     line = {"impl": "reference", "metric": "action_frames_per_s", "value": fps, "unit": "frames/s", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": frame_s * 1e3, "higher_is_better": True,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_s * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "oracle": "unpacked sequential fp32 CPU oracle (oracle/af_oracle.py)"},
+            "config": bench_config(args.layers),
+            "reference": "unpacked sequential fp32 CPU oracle (oracle/af_oracle.py, Python + torch CPU ops), as it stands",
             "packed_tok_per_s": fps * (L_P + K_STAGES - 1),
             "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -326,7 +346,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="print the cfg5 scheduling-shape sweep table instead of the bench line")
     ap.add_argument("--chunks", action="store_true", help="with --sweep: the longer-action-chunk points K = 7, 16, 24, 32 (276-row prefill + K - 1 decodes)")
-    ap.add_argument("--no-library-context", action="store_true", help="skip the cuBLAS same-shape context pass of the bench line")
+    ap.add_argument("--library-context", action="store_true", help="add roofline.library_same_shapes: cuBLAS on the step's four projection shapes, same run (context, ~1.5 s of library GEMMs; off by default so that the bench line runs only the product)")
     ap.add_argument("--gemm-timeline", action="store_true", help="report only: af_debug_trace timeline of the GEMM launches of a steady step (markdown table)")
     ap.add_argument("--library-gemm", action="store_true", help="context only: cuBLAS on the step's projection shapes (one JSON line)")
     args = ap.parse_args()
@@ -478,11 +498,7 @@ def main():
         "metric": "action_frames_per_s", "value": fps, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
         "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f16", "data": "synthetic",
-        "config": {"workload": WORKLOAD if args.layers == 32 else f"DEBUG {args.layers}-layer slice of " + WORKLOAD,
-                   "precision": "bf16-valued weights stored as fp16 (af_convert_bf16_to_fp16 at load, exact), fp16 "
-                                "activations and KV ring, fp32 accumulate / residual / logits (tcgen05 kind::f16)",
-                   "packed_rows": T, "ring": f"{R_REGIONS} regions x {CAPACITY}", "multi_gpu": "independent replicas",
-                   "l2": "inputs larger than L2 (13.2 GB of weights streamed per step vs 126 MB L2)"},
+        "config": bench_config(args.layers),
         "packed_tok_per_s": fps * T,
         "step_roofline": {"ms_measured_peaks": max(roof_hbm_ms, roof_tc_ms), "hbm_ms": roof_hbm_ms, "tensor_ms": roof_tc_ms,
                           "frac_of_measured": max(roof_hbm_ms, roof_tc_ms) / ms_step,
@@ -509,7 +525,7 @@ def main():
                            "kernel_nodes_per_step": launches_graph / args.steps},
         "gpu_launches": launches, "clocks": clocks,
     }
-    if world == 1 and args.layers == 32 and not args.no_library_context:
+    if world == 1 and args.layers == 32 and args.library_context:
         # context, not a product path: the vendor library's GEMMs on the same four shapes, timed the same way
         # (per-launch CUDA events, power-capped clock); see profiles/library_gemm_r1.md
         lib = run_library_gemm(args, emit=False)
@@ -520,16 +536,18 @@ def main():
             "frac_of_peak": lib["layer_tflops_event_timed"] / peaks["tf_sustained"],
             "this_library_layer_gemm_us": ours_layer_us, "sm_mhz": lib["clocks"]["sm_mhz"]}
     if not args.no_cpu_baseline:
+        # the oracle as it stands, whole 32-layer frames on this box's host cores: 1 warm-up + 2 timed (~5 s each)
         from oracle import af_oracle as O
-        n_sl = 2
-        torch.set_num_threads(max(1, (os.cpu_count() or 4) - 2))
-        sl = {"layers": hw["layers"][:n_sl], "g_final": hw["g_final"], "w_lm": hw["w_lm"]}
-        tl, tm = oracle_frame_sample(cfg, sl, n_sl, L_P, K_STAGES - 1, SEED, torch, O, I)
-        frame_s = tl * cfg.n_layers / n_sl + tm
+        torch.set_num_threads(oracle_cores())
+        orc = O.Oracle(cfg, hw, torch.float32)
+        oracle_frame(orc, cfg, SEED, 0, torch, I)
+        n_fr = 2
+        frame_s = sum(oracle_frame(orc, cfg, SEED, 1 + i, torch, I) for i in range(n_fr)) / n_fr
         line["cpu_baseline"] = {"value": 1.0 / frame_s, "unit": "frames/s", "cores": torch.get_num_threads(),
                                 "kind": "oracle",
-                                "sample": f"{n_sl} of {cfg.n_layers} layers of one frame (276-row prefill, 6 sequential "
-                                          f"decodes, LM head on 7 rows); layer time scaled x{cfg.n_layers / n_sl:g}"}
+                                "sample": f"{cfg.n_layers} of {cfg.n_layers} layers: {n_fr} whole frames timed after 1 warm-up "
+                                          "frame (276-row prefill, 6 sequential single-row decodes, LM head on 7 rows), "
+                                          "nothing scaled"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
