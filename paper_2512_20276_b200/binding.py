@@ -54,7 +54,7 @@ EXPORTS = ["af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_s
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
 PROFILE_CLASSES = ["gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm", "attention", "rope_append",
-                   "rmsnorm", "silu_mul", "other"]
+                   "rmsnorm", "chain", "other"]
 
 _lib = None
 

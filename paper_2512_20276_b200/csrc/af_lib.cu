@@ -16,6 +16,7 @@
 
 namespace af { constexpr int AF_MAX_SEGS_K = AF_MAX_SEGS; }
 #include "gemm_tcgen05.cuh"
+#include "chain.cuh"
 #include "elementwise.cuh"
 
 using namespace af;
@@ -48,9 +49,10 @@ static int check_launch(const char* what) {
 // ------------------------------------------------------------------------------------------------ per-kernel timing
 // Optional CUDA-event timing of every launch, by kernel class, on the launching stream (bench.py's roofline leg).
 enum ProfCat { PC_GEMM_QKV = 0, PC_GEMM_O, PC_GEMM_GATEUP, PC_GEMM_DOWN, PC_GEMM_LM, PC_ATTENTION, PC_ROPE_APPEND,
-               PC_RMSNORM, PC_SILU_MUL, PC_OTHER, PC_COUNT };
+               PC_RMSNORM, PC_CHAIN, PC_OTHER, PC_COUNT };
 struct ProfRec { cudaEvent_t a, b; int cat; };
 static bool g_prof_on = false;
+static bool g_prof_stages = false;   // af_debug_profile(2): time the per-stage path (one kernel per stage) instead of the layer chain
 static std::vector<ProfRec> g_prof;
 struct ProfScope {
   cudaStream_t st; ProfRec r; bool on;
@@ -60,7 +62,7 @@ struct ProfScope {
   }
   ~ProfScope() { if (on) { cudaEventRecord(r.b, st); g_prof.push_back(r); } }
 };
-extern "C" int af_debug_profile(int enable) { g_prof_on = enable != 0; return AF_OK; }
+extern "C" int af_debug_profile(int enable) { g_prof_on = enable != 0; g_prof_stages = enable == 2; return AF_OK; }
 extern "C" int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n) {
   if (!ms_sum || !counts || n < PC_COUNT) return fail(AF_ERR_ARG, "need %d slots", (int)PC_COUNT);
   CUDA_TRY(cudaDeviceSynchronize());
@@ -154,88 +156,156 @@ static int get_out_map(const OutView& o, int stg_bytes, CUtensorMap* out) {
 // Every kernel of the step is launched with programmatic dependent launch: its prologue (barrier init, TMEM
 // allocation, tensor-map prefetch, the first weight tiles) overlaps the previous kernel's tail, and each kernel
 // executes griddepcontrol.wait before it touches anything the previous kernel wrote.
-static bool g_use_pdl = true;
-static int g_staging_first = 0;   // AF_STAGING=0/1/2: first epilogue staging candidate tried (2x4 KB, 2x2 KB, 1x2 KB)
-static int g_w_pre = 3;           // AF_WPRE: weight stages requested before griddepcontrol.wait (measured: 3 beats all 6 by 0.6 % -
-                                  // a resident CTA's prefetch competes for HBM with the tail of the kernel it is waiting for)
-static int g_min_stages = 5;      // AF_MIN_STAGES: shrink the staging until the ring has this many stages
-static int g_gemm_mma2 = 1;      // AF_MMA2=0: keep cta_group::1 MMAs (with multicast) in the 2-CTA clusters
-static int g_gemm_cluster = 2;   // AF_CLUSTER=1 switches the 2-CTA activation multicast off
-static int g_launch_cluster = 1;  // cluster size of the next launch_k call (set by launch_gemm, reset after the launch)
+// Tuning constants (each was an environment knob while it was being measured on B200; DESIGN.md 6.1 has the numbers):
+constexpr int kWeightStagesBeforeWait = 3;   // weight stages a GEMM requests before griddepcontrol.wait: 3 beats all 6 by 0.6 %
+                                             // (a resident CTA's prefetch competes for HBM with the tail of the kernel it waits for)
+constexpr int kMinStages = 5;                // fp32-output GEMMs shrink their epilogue staging until the ring has this many stages
 template <typename... KArgs, typename... Args>
-static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int cluster, Args... args) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
   cudaLaunchAttribute at[2];
   int n = 0;
-  if (g_use_pdl) {
-    at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[n].val.programmaticStreamSerializationAllowed = 1;
-    ++n;
-  }
-  if (g_launch_cluster > 1) {
+  at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[n].val.programmaticStreamSerializationAllowed = 1;
+  ++n;
+  if (cluster > 1) {
     at[n].id = cudaLaunchAttributeClusterDimension;
-    at[n].val.clusterDim.x = g_launch_cluster; at[n].val.clusterDim.y = 1; at[n].val.clusterDim.z = 1;
+    at[n].val.clusterDim.x = cluster; at[n].val.clusterDim.y = 1; at[n].val.clusterDim.z = 1;
     ++n;
   }
   cfg.attrs = at; cfg.numAttrs = n;
   return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
-static int g_num_sms = 0;
-static int* g_flags = nullptr;  // [GEMM_MAX_GRID] stream-K ready flags (0/1)
-constexpr int GEMM_MAX_GRID = 160;
-constexpr int GEMM_MAX_SPLITS = 4;
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k1(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  return launch_k(kern, grid, block, smem, st, 1, args...);
+}
 
-static int gemm_global_init() {
-  std::lock_guard<std::mutex> lk(g_mu);
-  if (g_flags) return AF_OK;
+constexpr int GEMM_MAX_GRID = 160;
+constexpr int GEMM_MAX_SPLITS = GEMM_MAX_SLABS_K;
+constexpr int QKV_MAX_SLABS = QKV_MAX_SLABS_K;    // pieces per weight tile of the chain's QKV projection (slabs added by the RoPE stage)
+
+// ------------------------------------------------------------------------------------------------ per-device / per-stream state
+// Nothing the kernels synchronise through is process-global: the GEMM schedule tables live per DEVICE, the stream-K
+// ready flags, the chain kernel's grid barrier and the partial-exchange state per (device, STREAM) - two rings driven on
+// two streams never share a flag.  Kernels that wait inside themselves (stream-K owners, the chain's grid barrier) need
+// their whole grid resident, so steps enqueued on different streams of one device are ordered behind each other with an
+// event (serialise_on): they never run concurrently, whatever the caller's streams allow.
+struct SchedKey {
+  int split, n_pairs, nkb, max_cl, splits;
+  bool operator<(const SchedKey& o) const { return memcmp(this, &o, sizeof(SchedKey)) < 0; }
+};
+struct Sched { GemmPiece* dev; int n_cl; int* pair_slabs; int max_slabs; };
+struct StreamCtx { int* flags; unsigned long long* bar; };
+struct DevCtx {
+  int dev = -1, num_sms = 0, max_clusters = 0;       // max_clusters: co-resident 2-CTA clusters of the GEMM / chain kernels
+  std::map<SchedKey, Sched> scheds;
+  std::map<cudaStream_t, StreamCtx> streams;
+  cudaStream_t last_stream = nullptr; bool has_last = false;
+  cudaEvent_t last_done = nullptr;
+};
+static std::mutex g_ctx_mu;
+static std::map<int, DevCtx*> g_ctx;
+
+static int get_ctx(DevCtx** out) {
   int dev = 0;
   CUDA_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  auto it = g_ctx.find(dev);
+  if (it != g_ctx.end()) { *out = it->second; return AF_OK; }
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
-  if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device is sm_%d%d)", prop.major, prop.minor);
-  g_num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
-  if (const char* e = getenv("AF_NO_PDL")) g_use_pdl = atoi(e) == 0;
-  if (const char* e = getenv("AF_STAGING")) g_staging_first = atoi(e) < 0 ? 0 : (atoi(e) > 2 ? 2 : atoi(e));
-  if (const char* e = getenv("AF_MIN_STAGES")) g_min_stages = atoi(e);
-  if (const char* e = getenv("AF_WPRE")) g_w_pre = atoi(e);
-  if (const char* e = getenv("AF_MMA2")) g_gemm_mma2 = atoi(e) != 0;
-  if (const char* e = getenv("AF_CLUSTER")) g_gemm_cluster = atoi(e) == 1 ? 1 : 2;
-  CUDA_TRY(cudaMalloc(&g_flags, 256 * sizeof(int)));
-  CUDA_TRY(cudaMemset(g_flags, 0, 256 * sizeof(int)));
+  if (prop.major != 10) return fail(AF_ERR_UNSUPPORTED, "this library is built for sm_100a only (device %d is sm_%d%d)", dev, prop.major, prop.minor);
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
+  DevCtx* c = new DevCtx();
+  c->dev = dev;
+  c->num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
+  // Stream-K owners and the chain's grid barrier wait for other CTAs of their own grid: size the persistent grids by what
+  // the device can hold at once for the actual launch configuration (MPS / green contexts may expose fewer SMs than
+  // multiProcessorCount), never by the SM count alone.
+  int max_cl = 0;
+  {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(2 * GEMM_MAX_GRID); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = GEMM_SMEM_BUDGET;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    if (cudaOccupancyMaxActiveClusters(&max_cl, layer_chain_kernel, &cfg) != cudaSuccess || max_cl < 1) { cudaGetLastError(); max_cl = c->num_sms / 2; }
+  }
+  c->max_clusters = max_cl < c->num_sms / 2 ? max_cl : c->num_sms / 2;
+  if (c->max_clusters < 1) c->max_clusters = 1;
+  if (cudaEventCreateWithFlags(&c->last_done, cudaEventDisableTiming) != cudaSuccess) { delete c; return fail(AF_ERR_CUDA, "cudaEventCreate failed"); }
+  g_ctx[dev] = c;
+  *out = c;
   return AF_OK;
 }
 
-// debug timeline of the last TRACE_LAUNCHES GEMM launches (globaltimer stamps per CTA), off unless af_debug_trace(1)
+static int get_stream_ctx(DevCtx* c, cudaStream_t st, StreamCtx* out) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  auto it = c->streams.find(st);
+  if (it != c->streams.end()) { *out = it->second; return AF_OK; }
+  StreamCtx sc{};
+  uint8_t* mem = nullptr;
+  CUDA_TRY(cudaMalloc(&mem, 2048));
+  CUDA_TRY(cudaMemset(mem, 0, 2048));
+  sc.flags = reinterpret_cast<int*>(mem);                 // [2 * GEMM_MAX_GRID <= 320] ints
+  sc.bar = reinterpret_cast<unsigned long long*>(mem + 1536);   // the chain kernel's grid-barrier arrival counter
+  c->streams[st] = sc;
+  *out = sc;
+  return AF_OK;
+}
+
+// Order this call's work behind the library work last enqueued on ANOTHER stream of the device (see above).
+static int serialise_on(DevCtx* c, cudaStream_t st) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cs);
+  if (cs != cudaStreamCaptureStatusNone) return AF_OK;   // a graph being captured orders itself; its replays are the caller's to order
+  if (c->has_last && c->last_stream != st) CUDA_TRY(cudaStreamWaitEvent(st, c->last_done, 0));
+  return AF_OK;
+}
+static int serialise_done(DevCtx* c, cudaStream_t st) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cs);
+  if (cs == cudaStreamCaptureStatusNone) CUDA_TRY(cudaEventRecord(c->last_done, st));   // (a captured step replays on its own stream)
+  c->last_stream = st; c->has_last = true;
+  return AF_OK;
+}
+
+// debug timeline of the last TRACE_LAUNCHES layer_chain_kernel launches (globaltimer stamps per CTA at every phase end
+// and grid-barrier exit), off unless af_debug_trace(1)
 constexpr int TRACE_LAUNCHES = 16;
 static long long* g_trace = nullptr;
 static int g_trace_n = 0;
-struct TraceMeta { int cat, grid; };
+struct TraceMeta { int n_phases, grid; };
 static TraceMeta g_trace_meta[TRACE_LAUNCHES];
 extern "C" int af_debug_trace(int enable) {
+  CUDA_TRY(cudaDeviceSynchronize());   // no launch in flight may still hold the buffer
   if (enable && !g_trace) {
-    CUDA_TRY(cudaMalloc(&g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32));
-    CUDA_TRY(cudaMemset(g_trace, 0, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32));
+    CUDA_TRY(cudaMalloc(&g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * CH_TRACE_SLOTS));
+    CUDA_TRY(cudaMemset(g_trace, 0, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * CH_TRACE_SLOTS));
   }
   if (!enable && g_trace) { cudaFree(g_trace); g_trace = nullptr; }
   g_trace_n = 0;
   return AF_OK;
 }
-// out: [TRACE_LAUNCHES][160][32] int64 stamps; meta: [TRACE_LAUNCHES][2] (class, grid); returns launches recorded
 extern "C" int af_debug_trace_read(long long* out, int* meta) {
   if (!g_trace || !out || !meta) return fail(AF_ERR_ARG, "trace is off");
   CUDA_TRY(cudaDeviceSynchronize());
-  CUDA_TRY(cudaMemcpy(out, g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * 32, cudaMemcpyDeviceToHost));
-  for (int i = 0; i < TRACE_LAUNCHES; ++i) { meta[2 * i] = g_trace_meta[i].cat; meta[2 * i + 1] = g_trace_meta[i].grid; }
+  CUDA_TRY(cudaMemcpy(out, g_trace, sizeof(long long) * TRACE_LAUNCHES * GEMM_MAX_GRID * CH_TRACE_SLOTS, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < TRACE_LAUNCHES; ++i) { meta[2 * i] = g_trace_meta[i].n_phases; meta[2 * i + 1] = g_trace_meta[i].grid; }
   return g_trace_n;
 }
 
@@ -244,10 +314,10 @@ extern "C" int af_debug_trace_read(long long* out, int* meta) {
 static int row_threads_for(int D) { int t = (D / 8 + 31) / 32 * 32; return t < 64 ? 64 : (t > 512 ? 512 : t); }
 
 // split-K pieces per tile of the O / down projections (also the number of slabs the next residual kernel adds)
-static int gemm_split_count(int n_tiles, int K) {
-  const int cluster = (g_gemm_cluster > 1 && n_tiles >= 2) ? 2 : 1;
+static int gemm_split_count(const DevCtx* ctx, int n_tiles, int K) {
+  const int cluster = n_tiles >= 2 ? 2 : 1;
   const int n_pairs = (n_tiles + cluster - 1) / cluster, nkb = (K + GEMM_BK - 1) / GEMM_BK;
-  int s = (g_num_sms / cluster) / n_pairs;
+  int s = (cluster == 2 ? ctx->max_clusters : ctx->num_sms) / n_pairs;
   if (s > GEMM_MAX_SPLITS) s = GEMM_MAX_SPLITS;
   if (s > nkb) s = nkb;
   return s < 1 ? 1 : s;
@@ -297,22 +367,22 @@ static int streamk_partition(int total, int nkb, int n_max, int* ub) {
 // who reduces what.  Built once per (split mode, tile pairs, k-blocks, clusters) and kept on the device.
 //   SPLIT_K       one PK_PLAIN piece per cluster: slab `mid` of tile pair c / splits.
 //   stream-K      contiguous unit ranges; a range's k-tail piece is its first piece, its k-head piece its last.
+//   SPLIT_SLABS   (layer_chain_kernel) contiguous unit ranges of equal length; EVERY piece is a PK_PLAIN piece stored as
+//                 slab `mid` = its ordinal inside its tile pair, and the row stage that follows adds a pair's slabs in
+//                 that order (pair_slabs[pair] of them, at most `splits`): no CTA waits on another, no fix-up.
 // (Two hand-made schedules for the QKV and gate/up shapes - owners with a single piece plus clusters made of
 //  contributor pieces only - were built on this table and measured no faster than the ranges; removed.)
-struct SchedKey {
-  int split, n_pairs, nkb, max_cl, splits;
-  bool operator<(const SchedKey& o) const { return memcmp(this, &o, sizeof(SchedKey)) < 0; }
-};
-struct Sched { GemmPiece* dev; int n_cl; };
-static std::map<SchedKey, Sched> g_scheds;
+constexpr int SPLIT_SLABS = 2;
 
 // Pure host part: the flat [n_cl][GEMM_MAX_PIECES] table (also what af_debug_gemm_schedule returns, for CPU tests).
-static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, std::vector<GemmPiece>* flat_out, int* n_cl_out) {
+static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, std::vector<GemmPiece>* flat_out, int* n_cl_out,
+                         std::vector<int>* pair_slabs_out = nullptr) {
   if (n_pairs < 1 || nkb < 1 || max_cl < 1 || splits < 1) return fail(AF_ERR_ARG, "bad schedule shape");
   std::vector<std::vector<GemmPiece>> cl;    // pieces per cluster
   auto piece = [](int pair, int kb0, int kb1, int kind, int slot, int n_contrib, int mid) {
     return GemmPiece{pair, kb0, kb1, kind, slot, n_contrib, mid, 0};
   };
+  std::vector<int> pair_slabs(n_pairs, 1);
   if (split == SPLIT_K) {
     cl.resize(static_cast<size_t>(n_pairs) * splits);
     for (int c = 0; c < n_pairs * splits; ++c) {
@@ -320,6 +390,29 @@ static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits
       cl[c].push_back(piece(t, static_cast<int>(1LL * s * nkb / splits), static_cast<int>(1LL * (s + 1) * nkb / splits),
                             PK_PLAIN, 0, 0, s));
     }
+    pair_slabs.assign(n_pairs, splits);
+  } else if (split == SPLIT_SLABS) {
+    // range length: all clusters busy, but never more than `splits` pieces of one tile pair
+    const int total = n_pairs * nkb;
+    int len = (total + max_cl - 1) / max_cl;
+    if (splits > 1) { const int lmin = (nkb - 1 + splits - 2) / (splits - 1); if (len < lmin) len = lmin; }
+    else len = nkb > len ? nkb : (len + nkb - 1) / nkb * nkb;
+    if (len < 1) len = 1;
+    const int n = (total + len - 1) / len;
+    cl.resize(n);
+    pair_slabs.assign(n_pairs, 0);
+    for (int c = 0; c < n; ++c) {
+      int u = c * len;
+      const int end = (c + 1) * len < total ? (c + 1) * len : total;
+      while (u < end) {
+        const int t = u / nkb, kb0 = u - t * nkb;
+        const int kb1 = end - t * nkb < nkb ? end - t * nkb : nkb;
+        cl[c].push_back(piece(t, kb0, kb1, PK_PLAIN, 0, 0, pair_slabs[t]++));
+        u = t * nkb + kb1;
+      }
+    }
+    for (int t = 0; t < n_pairs; ++t)
+      if (pair_slabs[t] > splits) return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: %d slabs of one tile pair (max %d)", pair_slabs[t], splits);
   } else {
     // stream-K ranges (cost-balanced when a range is longer than a tile)
     const int total = n_pairs * nkb;
@@ -353,22 +446,30 @@ static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits
     for (size_t i = 0; i < cl[c].size(); ++i) flat[static_cast<size_t>(c) * GEMM_MAX_PIECES + i] = cl[c][i];
   }
   *n_cl_out = n_cl;
+  if (pair_slabs_out) *pair_slabs_out = pair_slabs;
   return AF_OK;
 }
 
-static int build_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
-  std::lock_guard<std::mutex> lk(g_mu);
+// The device copy has at least max_cl rows (clusters beyond n_cl find an empty list), so that kernels whose grid is the
+// whole device (layer_chain_kernel) can index it with any cluster id.
+static int build_schedule(DevCtx* ctx, int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
   const SchedKey key{split, n_pairs, nkb, max_cl, splits};
-  auto it = g_scheds.find(key);
-  if (it != g_scheds.end()) { *out = it->second; return AF_OK; }
+  auto it = ctx->scheds.find(key);
+  if (it != ctx->scheds.end()) { *out = it->second; return AF_OK; }
   std::vector<GemmPiece> flat;
+  std::vector<int> pair_slabs;
   int n_cl = 0;
-  const int rc = make_schedule(split, n_pairs, nkb, max_cl, splits, &flat, &n_cl);
+  const int rc = make_schedule(split, n_pairs, nkb, max_cl, splits, &flat, &n_cl, &pair_slabs);
   if (rc) return rc;
-  Sched sc{nullptr, n_cl};
+  if (n_cl < max_cl) flat.resize(static_cast<size_t>(max_cl) * GEMM_MAX_PIECES, GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
+  Sched sc{nullptr, n_cl, nullptr, 0};
+  for (int v : pair_slabs) sc.max_slabs = v > sc.max_slabs ? v : sc.max_slabs;
   CUDA_TRY(cudaMalloc(&sc.dev, flat.size() * sizeof(GemmPiece)));
   CUDA_TRY(cudaMemcpy(sc.dev, flat.data(), flat.size() * sizeof(GemmPiece), cudaMemcpyHostToDevice));
-  g_scheds[key] = sc;
+  CUDA_TRY(cudaMalloc(&sc.pair_slabs, pair_slabs.size() * sizeof(int)));
+  CUDA_TRY(cudaMemcpy(sc.pair_slabs, pair_slabs.data(), pair_slabs.size() * sizeof(int), cudaMemcpyHostToDevice));
+  ctx->scheds[key] = sc;
   *out = sc;
   return AF_OK;
 }
@@ -379,9 +480,12 @@ static size_t gemm_partial_bytes() { return static_cast<size_t>(GEMM_MAX_GRID) *
 // layout (n_parts / part_rows / a_pair), the split mode and the epilogue fields; the decomposition is filled here.
 static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView& ov, /* proto.w_fp16 set by the caller */ const void* x, int x_rows_cap,
                        const void* const* w, int T) {
-  int rc = gemm_global_init();
+  DevCtx* ctx = nullptr;
+  int rc = get_ctx(&ctx);
   if (rc) return rc;
   if (T <= 0) return AF_OK;
+  StreamCtx sctx;
+  if ((rc = get_stream_ctx(ctx, st, &sctx))) return rc;
   const int n_chunks = (T + GEMM_MAX_TOK - 1) / GEMM_MAX_TOK;
   const int chunk = (T + n_chunks - 1) / n_chunks;
   for (int tok0 = 0; tok0 < T; tok0 += chunk) {
@@ -396,15 +500,16 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     p.num_kb = (p.K + GEMM_BK - 1) / GEMM_BK; p.T = Tc; p.tok0 = tok0;
     p.xh = p.n2 > 0 ? p.n1 : p.n1 / 2;
     p.n_tiles = n_tiles;
-    p.cluster = (g_gemm_cluster > 1 && n_tiles >= 2) ? 2 : 1;
+    p.cluster = n_tiles >= 2 ? 2 : 1;
     const int n_pairs = (n_tiles + p.cluster - 1) / p.cluster;     // work units are (tile pair, k-block) per cluster
-    const int max_cl = g_num_sms / p.cluster;
-    p.splits = p.split == SPLIT_K ? gemm_split_count(n_tiles, p.K) : 1;
+    const int max_cl = p.cluster == 2 ? ctx->max_clusters : ctx->num_sms;
+    p.splits = p.split == SPLIT_K ? gemm_split_count(ctx, n_tiles, p.K) : 1;
     Sched sc;
-    if ((rc = build_schedule(p.split, n_pairs, p.num_kb, max_cl, p.splits, &sc))) return rc;
+    if ((rc = build_schedule(ctx, p.split, n_pairs, p.num_kb, max_cl, p.splits, &sc))) return rc;
     p.sched = sc.dev;
+    p.n_cl = sc.n_cl;
     const int grid = sc.n_cl * p.cluster;
-    p.mma2 = (g_gemm_mma2 && p.cluster == 2 && p.w_fp16) ? 1 : 0;
+    p.mma2 = (p.cluster == 2 && p.w_fp16) ? 1 : 0;
     const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (p.mma2 ? n_pad / 2 : n_pad) * GEMM_BK * 2;
     // epilogue staging: two 4 KB buffers per warp, or one 2 KB buffer when that buys a pipeline stage (the main loop
     // is bound by TMA latency x stages in flight)
@@ -412,25 +517,24 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     // ~160 KB of loads in flight), down to one 2 KB buffer per warp
     const int cand[3][2] = {{4096, 2}, {2048, 2}, {2048, 1}};
     if (ov.elem_bytes == 2) return fail(AF_ERR_UNSUPPORTED, "GEMM outputs are fp16 or fp32");
-    p.out_bf16 = ov.elem_bytes == -2 ? 2 : 0;
-    p.part_f16 = p.out_bf16 ? 1 : 0;   // fp16 outputs take fp16 partials (both in the fragment layout), fp32 take fp32
-    if (p.out_bf16) {
+    p.out_f16 = ov.elem_bytes == -2 ? 2 : 0;
+    p.part_f16 = p.out_f16 ? 1 : 0;   // fp16 outputs take fp16 partials (both in the fragment layout), fp32 take fp32
+    if (p.out_f16) {
       if (ov.features % 8 || ov.ld_tok % 8 || ov.ld_mid % 8 || (reinterpret_cast<uintptr_t>(ov.ptr) & 15))
         return fail(AF_ERR_ARG, "fp16 GEMM output needs 16-byte aligned rows (features %d, ld %lld/%lld)", ov.features, ov.ld_tok, ov.ld_mid);
       p.out = ov.ptr; p.out_ld_tok = ov.ld_tok; p.out_ld_mid = ov.ld_mid; p.out_features = ov.features;
     }
     int stages = 0;
     // (fp16 outputs: one 2 KB image per warp, read back by the warp itself - nothing asynchronous to wait for)
-    for (int i = p.out_bf16 ? 2 : g_staging_first; i < 3; ++i) {
+    for (int i = p.out_f16 ? 2 : 0; i < 3; ++i) {
       const int st_i = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * cand[i][0] * cand[i][1]) / stage_bytes;
-      if (st_i > stages && (stages < g_min_stages || stages == 0)) { stages = st_i; p.stg_bytes = cand[i][0]; p.stg_bufs = cand[i][1]; }
+      if (st_i > stages && (stages < kMinStages || stages == 0)) { stages = st_i; p.stg_bytes = cand[i][0]; p.stg_bufs = cand[i][1]; }
     }
     const int xch_bytes = GEMM_EPI_WARPS * p.stg_bytes * p.stg_bufs;
     if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
     if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "GEMM stage does not fit shared memory");
-    p.stages = stages; p.flags = g_flags;
-    p.w_pre = g_w_pre < stages ? g_w_pre : stages;
-    if (g_trace) { p.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * 32; g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {cat, grid}; ++g_trace_n; }
+    p.stages = stages; p.flags = sctx.flags;
+    p.w_pre = kWeightStagesBeforeWait < stages ? kWeightStagesBeforeWait : stages;
     CUtensorMap mw[3], mx;
     for (int i = 0; i < 3; ++i) {
       const int n_w = p.a_pair == 1 ? 2 : (p.a_pair == 2 ? 1 : p.n_parts);
@@ -452,17 +556,104 @@ static int launch_gemm(int cat, cudaStream_t st, GemmParams proto, const OutView
     const size_t smem = static_cast<size_t>(stages) * stage_bytes + xch_bytes + 1024;
     {
       ProfScope ps(cat, st);
-      g_launch_cluster = p.cluster;
-      auto kern = p.mma2 ? (p.out_bf16 ? gemm_tcgen05_kernel<true, true> : gemm_tcgen05_kernel<true, false>)
-                         : (p.out_bf16 ? gemm_tcgen05_kernel<false, true> : gemm_tcgen05_kernel<false, false>);
-      cudaError_t e = launch_k(kern, dim3(grid), dim3(GEMM_THREADS), smem, st, mw[0], mw[1], mw[2], mx, mo, mp, p);
-      g_launch_cluster = 1;
+      auto kern = p.mma2 ? (p.out_f16 ? gemm_tcgen05_kernel<true, true> : gemm_tcgen05_kernel<true, false>)
+                         : (p.out_f16 ? gemm_tcgen05_kernel<false, true> : gemm_tcgen05_kernel<false, false>);
+      cudaError_t e = launch_k(kern, dim3(grid), dim3(GEMM_THREADS), smem, st, p.cluster, mw[0], mw[1], mw[2], mx, mo, mp, p);
       if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gemm_tcgen05_kernel failed: %s", cudaGetErrorString(e));
     }
     rc = check_launch("gemm_tcgen05_kernel");
     if (rc) return rc;
   }
   return AF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ layer chain (chain.cuh)
+// Host side of layer_chain_kernel: phases are appended to a ChainArgs (tensor maps deduplicated), then one launch.
+struct ChainBuilder {
+  ChainArgs a;
+  int n_maps = 0;
+  DevCtx* ctx = nullptr;
+  int max_rows = 0;          // row capacity of the workspace buffers the activation maps cover
+  ChainBuilder() { memset(&a, 0, sizeof a); }
+  int add_map(const CUtensorMap& m) {
+    for (int i = 0; i < n_maps; ++i)
+      if (memcmp(&a.maps[i], &m, sizeof m) == 0) return i;
+    if (n_maps == CH_MAX_MAPS) return -1;
+    a.maps[n_maps] = m;
+    return n_maps++;
+  }
+  ChainPhase* next() { return a.n_phases < CH_MAX_PHASES ? &a.ph[a.n_phases++] : nullptr; }
+};
+
+// One projection phase: y = x W^T over n_parts weight matrices stacked along the feature axis (a_pair = 2: gate | up
+// interleaved by af_prepare_gate_up).  split: SPLIT_K / SPLIT_SLABS (EPI_STORE, slabs) or SPLIT_STREAMK (EPI_SWIGLU).
+static int chain_add_gemm(ChainBuilder& b, const void* const* w, int n_parts, int part_rows, int a_pair, int K, int split, int max_slabs,
+                          int epi, const void* x, act_t* out, long long out_ld_tok, long long out_ld_slab, int out_features,
+                          const int** pair_slabs_out, int* n_slabs_out) {
+  ChainPhase* P = b.next();
+  if (!P) return fail(AF_ERR_UNSUPPORTED, "chain: too many phases");
+  P->kind = CH_GEMM;
+  const int n_tiles = a_pair ? (part_rows + 63) / 64 : n_parts * ((part_rows + GEMM_BM - 1) / GEMM_BM);
+  P->part_rows = part_rows; P->tiles_per_part = (part_rows + GEMM_BM - 1) / GEMM_BM; P->a_pair = a_pair;
+  P->n_tiles = n_tiles; P->num_kb = (K + GEMM_BK - 1) / GEMM_BK; P->epi = epi;
+  const int n_pairs = (n_tiles + 1) / 2;
+  int splits = max_slabs;
+  if (split == SPLIT_K) splits = gemm_split_count(b.ctx, n_tiles, K);
+  Sched sc;
+  int rc = build_schedule(b.ctx, split, n_pairs, P->num_kb, b.ctx->max_clusters, split == SPLIT_STREAMK ? 1 : splits, &sc);
+  if (rc) return rc;
+  P->sched = sc.dev;
+  if (pair_slabs_out) *pair_slabs_out = sc.pair_slabs;
+  if (n_slabs_out) *n_slabs_out = sc.max_slabs;
+  for (int i = 0; i < 3; ++i) {
+    CUtensorMap m;
+    const int n_w = a_pair ? 1 : n_parts;
+    if ((rc = get_map(w[i < n_w ? i : 0], a_pair ? n_tiles * GEMM_BM : part_rows, K, GEMM_BM, &m))) return rc;
+    if ((P->w_map[i] = b.add_map(m)) < 0) return fail(AF_ERR_UNSUPPORTED, "chain: too many tensor maps");
+  }
+  CUtensorMap mx;
+  if ((rc = get_map(x, b.max_rows, K, b.a.n1 / 2, &mx))) return rc;
+  if ((P->x_map = b.add_map(mx)) < 0) return fail(AF_ERR_UNSUPPORTED, "chain: too many tensor maps");
+  if (out_features % 8 || out_ld_tok % 8 || out_ld_slab % 8 || (reinterpret_cast<uintptr_t>(out) & 15))
+    return fail(AF_ERR_ARG, "chain: fp16 GEMM output needs 16-byte aligned rows");
+  P->out = out; P->out_ld_tok = out_ld_tok; P->out_ld_slab = out_ld_slab; P->out_features = out_features;
+  return AF_OK;
+}
+
+static int chain_add_rows(ChainBuilder& b, const void* src, int embed, int n_slabs, long long slab_stride, const void* gain, act_t* xn) {
+  ChainPhase* P = b.next();
+  if (!P) return fail(AF_ERR_UNSUPPORTED, "chain: too many phases");
+  P->kind = CH_ROWS; P->src = src; P->embed = embed; P->n_slabs = n_slabs; P->slab_stride = slab_stride;
+  P->gain = reinterpret_cast<const __nv_bfloat16*>(gain); P->xn = xn;
+  return AF_OK;
+}
+
+static int chain_add_rope(ChainBuilder& b, const act_t* qkv_slabs, long long slab_stride, const int* pair_slabs, act_t* q_out, act_t* kv_layer) {
+  ChainPhase* P = b.next();
+  if (!P) return fail(AF_ERR_UNSUPPORTED, "chain: too many phases");
+  P->kind = CH_ROPE; P->src = qkv_slabs; P->slab_stride = slab_stride; P->pair_slabs = pair_slabs; P->q_out = q_out; P->kv_layer = kv_layer;
+  return AF_OK;
+}
+
+static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
+  const int n_pad = b.a.n1 + b.a.n2;
+  const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2;
+  int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * 2048) / stage_bytes;
+  if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
+  if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "chain: a stage does not fit shared memory");
+  b.a.stages = stages;
+  const int grid = 2 * b.ctx->max_clusters;
+  b.a.trace = nullptr;
+  if (g_trace && grid <= GEMM_MAX_GRID) {
+    b.a.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * CH_TRACE_SLOTS;
+    g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {b.a.n_phases, grid};
+    ++g_trace_n;
+  }
+  const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_EPI_WARPS * 2048 + 1024;
+  cudaError_t e;
+  { ProfScope ps(cat, st); e = launch_k(layer_chain_kernel, dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
+  if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of layer_chain_kernel failed: %s", cudaGetErrorString(e));
+  return check_launch("layer_chain_kernel");
 }
 
 // ------------------------------------------------------------------------------------------------ ring handle
@@ -501,8 +692,8 @@ extern "C" size_t af_ring_bytes(const af_model_cfg* c, const af_ring_cfg* r) {
 // workspace = fixed part (stream-K partials) + per-row part; the carve depends only on (pointer, bytes)
 static size_t ws_per_row(const af_model_cfg* c) {
   const size_t D = c->d_model, F = c->ffn;
-  // xn, qkv, q_rot, attn, h (bf16) + split-K partial slabs of the O / down projections (fp32)
-  return align_up((D + 3 * D + D + D + F) * 2 + GEMM_MAX_SPLITS * D * 4, 256);
+  // xn, qkv (QKV_MAX_SLABS slabs), q_rot, attn, h (fp16) + split-K slabs of the O / down projections
+  return align_up((D + QKV_MAX_SLABS * 3 * D + D + D + F) * 2 + GEMM_MAX_SPLITS * D * 4, 256);
 }
 static size_t ws_fixed() { return align_up(gemm_partial_bytes(), 256) + 8 * 256; }
 
@@ -516,7 +707,7 @@ extern "C" size_t af_workspace_bytes(const af_model_cfg* c, int32_t max_rows, in
 struct Workspace {
   float* partial;        // stream-K partials [grid][n_pad][128]
   float* split;          // split-K slabs [GEMM_MAX_SPLITS][max_rows][D]
-  act_t *xn, *qkv, *q_rot, *attn, *h;   // fp16 activations
+  act_t *xn, *qkv, *q_rot, *attn, *h;   // fp16 activations (qkv: QKV_MAX_SLABS slabs of [max_rows][3D]; the per-stage path uses the first)
   int max_rows;
 };
 static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, Workspace* o) {
@@ -533,7 +724,7 @@ static int carve(const af_model_cfg* c, void* ws, size_t bytes, int need_rows, W
   o->partial = reinterpret_cast<float*>(take(gemm_partial_bytes()));
   o->split = reinterpret_cast<float*>(take(GEMM_MAX_SPLITS * rows * D * 4));
   o->xn = reinterpret_cast<act_t*>(take(rows * D * 2));
-  o->qkv = reinterpret_cast<act_t*>(take(rows * 3 * D * 2));
+  o->qkv = reinterpret_cast<act_t*>(take(QKV_MAX_SLABS * rows * 3 * D * 2));
   o->q_rot = reinterpret_cast<act_t*>(take(rows * D * 2));
   o->attn = reinterpret_cast<act_t*>(take(rows * D * 2));
   o->h = reinterpret_cast<act_t*>(take(rows * F * 2));
@@ -548,8 +739,8 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   if (r->n_regions <= 0 || r->capacity <= 0) return fail(AF_ERR_ARG, "ring needs n_regions > 0 and capacity > 0");
   if (reinterpret_cast<uintptr_t>(kv_mem) & 255) return fail(AF_ERR_ARG, "kv_mem must be 256-byte aligned");
   if (kv_bytes < af_ring_bytes(c, r)) return fail(AF_ERR_WORKSPACE, "kv_mem of %zu bytes < af_ring_bytes %zu", kv_bytes, af_ring_bytes(c, r));
-  rc = gemm_global_init();
-  if (rc) return rc;
+  DevCtx* ctx = nullptr;
+  if ((rc = get_ctx(&ctx))) return rc;
   af_ring* g = new af_ring();
   g->cfg = *c; g->rc = *r; g->kv = reinterpret_cast<act_t*>(kv_mem);
   g->base.assign(r->n_regions, 0); g->len.assign(r->n_regions, 0);
@@ -768,6 +959,9 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const int D = c.d_model, F = c.ffn, H = c.n_heads, hd = c.head_dim;
+  DevCtx* ctx = nullptr;
+  if ((rc = get_ctx(&ctx))) return rc;
+  if ((rc = serialise_on(ctx, st))) return rc;
   SegTableArg sta{};
   sta.n_segs = n_segs; sta.R = R; sta.C = C;
   int n_items = 0;
@@ -779,7 +973,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   cudaError_t le;
 #define AF_LAUNCH(cat, name, ...)                                                                              \
   do {                                                                                                         \
-    { ProfScope ps_(cat, st); le = launch_k(__VA_ARGS__); }                                                    \
+    { ProfScope ps_(cat, st); le = launch_k1(__VA_ARGS__); }                                                   \
     if (le != cudaSuccess) return fail(AF_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(le)); \
     if ((rc = check_launch(name))) return rc;                                                                  \
   } while (0)
@@ -788,6 +982,75 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   else rowmap_kernel<<<1, 256, 0, st>>>(sta, g->tb, g->n_items_dev);
   }
   if ((rc = check_launch("rowmap_kernel"))) return rc;
+  const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
+  const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
+  auto launch_attention = [&](int l) -> int {   // a4: segment-masked causal attention over the ring
+    act_t* kvl = g->kv + layer_elems * l;
+    auto att = hd == 128 ? (g->window > 0 ? attention_kernel<128, true> : attention_kernel<128, false>)
+                         : (g->window > 0 ? attention_kernel<64, true> : attention_kernel<64, false>);
+    AF_LAUNCH(PC_ATTENTION, "attention_kernel", att, dim3(H, n_items), dim3(ATT_THREADS), att_smem_bytes(hd), st,
+              static_cast<const act_t*>(ws.q_rot), static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2,
+              g->window);
+    return AF_OK;
+  };
+  // ---- the layer chain (chain.cuh): per layer ONE persistent launch for every projection and row stage + attention ----
+  const bool use_chain = w->weight_format == AF_WEIGHTS_FP16_GU && T <= GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
+                         ctx->max_clusters >= 2 && !g_prof_stages;
+  if (use_chain) {
+    StreamCtx sctx;
+    if ((rc = get_stream_ctx(ctx, st, &sctx))) return rc;
+    const long long split_stride = static_cast<long long>(ws.max_rows) * D;
+    const long long qkv_stride = static_cast<long long>(ws.max_rows) * 3 * D;
+    auto begin = [&](ChainBuilder& b) {
+      b.ctx = ctx; b.max_rows = ws.max_rows;
+      int n_pad = (T + 15) / 16 * 16;
+      if (n_pad <= 256) { b.a.n1 = n_pad; b.a.n2 = 0; }
+      else { b.a.n1 = ((T + 1) / 2 + 15) / 16 * 16; b.a.n2 = b.a.n1; }
+      b.a.T = T; b.a.D = D; b.a.eps = c.rms_eps; b.a.x = hidden_out; b.a.bar = sctx.bar; b.a.flags = sctx.flags;
+      b.a.partial = reinterpret_cast<uint8_t*>(ws.partial); b.a.tb = g->tb; b.a.rope_tab = g->rope_tab;
+      b.a.H = H; b.a.hd = hd; b.a.R = R; b.a.C = C;
+    };
+    auto add_qkv_rope = [&](ChainBuilder& b, int l) -> int {
+      const af_layer_weights& L = w->layers[l];
+      const void* wqkv[3] = {L.wq, L.wk, L.wv};
+      const int* pair_slabs = nullptr;
+      int r = chain_add_gemm(b, wqkv, 3, D, 0, D, SPLIT_SLABS, QKV_MAX_SLABS, EPI_STORE, ws.xn, ws.qkv, 3LL * D, qkv_stride, D, &pair_slabs, nullptr);
+      if (r) return r;
+      return chain_add_rope(b, ws.qkv, qkv_stride, pair_slabs, ws.q_rot, g->kv + layer_elems * l);
+    };
+    {   // launch 0: x = embeds; xn = RMSNorm(x; g_attn[0]) | QKV of layer 0 | RoPE + ring append
+      ChainBuilder b;
+      begin(b);
+      if ((rc = chain_add_rows(b, packed_embeds, 1, 0, 0, w->layers[0].g_attn, ws.xn))) return rc;
+      if ((rc = add_qkv_rope(b, 0))) return rc;
+      if ((rc = chain_launch(b, st, PC_CHAIN))) return rc;
+    }
+    for (int l = 0; l < c.n_layers; ++l) {
+      if ((rc = launch_attention(l))) return rc;
+      const af_layer_weights& L = w->layers[l];
+      ChainBuilder b;
+      begin(b);
+      int n_slabs = 0;
+      const void* wo[3] = {L.wo, nullptr, nullptr};
+      if ((rc = chain_add_gemm(b, wo, 1, D, 0, D, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.attn, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
+      if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, L.g_mlp, ws.xn))) return rc;
+      const void* wgu[3] = {L.w_gate, nullptr, nullptr};
+      if ((rc = chain_add_gemm(b, wgu, 2, F, 2, D, SPLIT_STREAMK, 1, EPI_SWIGLU, ws.xn, ws.h, F, 0, F, nullptr, nullptr))) return rc;
+      const void* wd[3] = {L.w_down, nullptr, nullptr};
+      if ((rc = chain_add_gemm(b, wd, 1, D, 0, F, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.h, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
+      if (l + 1 < c.n_layers) {
+        if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, w->layers[l + 1].g_attn, ws.xn))) return rc;
+        if ((rc = add_qkv_rope(b, l + 1))) return rc;
+      } else {
+        if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, nullptr, nullptr))) return rc;   // hidden_out: no final norm
+      }
+      if ((rc = chain_launch(b, st, PC_CHAIN))) return rc;
+    }
+    for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;   // a9 ring commit
+    g->last_T = T;
+    return serialise_done(ctx, st);
+  }
+  // ---- the per-stage path (bf16 / unpacked weights, T > 512, or per-stage profiling): one kernel per stage ----
   {
     const size_t n = static_cast<size_t>(T) * D;
     AF_LAUNCH(PC_OTHER, "embed_to_residual_kernel", embed_to_residual_kernel,
@@ -797,11 +1060,9 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   const int row_threads = row_threads_for(D);
   const int wfmt = w->weight_format == AF_WEIGHTS_FP16 || w->weight_format == AF_WEIGHTS_FP16_GU;
   const bool gu_packed = w->weight_format == AF_WEIGHTS_FP16_GU;
-  const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
-  const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   const long long split_stride = static_cast<long long>(ws.max_rows) * D;
   int prev_splits = 0;   // split-K slabs of the previous projection still to be added to the residual stream
-  auto split_count = [&](int n_tiles, int K) { return gemm_split_count(n_tiles, K); };
+  auto split_count = [&](int n_tiles, int K) { return gemm_split_count(ctx, n_tiles, K); };
   const int d_tiles = (D + GEMM_BM - 1) / GEMM_BM;
   for (int l = 0; l < c.n_layers; ++l) {
     const af_layer_weights& L = w->layers[l];
@@ -810,7 +1071,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     AF_LAUNCH(PC_RMSNORM, "residual_norm_kernel", residual_norm_kernel, dim3(T), dim3(row_threads), 0, st, hidden_out,
               reinterpret_cast<const act_t*>(ws.split), prev_splits, split_stride,
               reinterpret_cast<const __nv_bfloat16*>(L.g_attn), ws.xn, D, c.rms_eps);
-    // a2 + a3: QKV projection with the fused RoPE + ring-append epilogue
+    // a2: QKV projection (stream-K with fix-up, fp16 q|k|v rows)
     {
       GemmParams gp{};
       gp.part_f16 = 1; gp.w_fp16 = wfmt; gp.n_parts = 3; gp.part_rows = D; gp.a_pair = 0; gp.K = D; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
@@ -823,14 +1084,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     AF_LAUNCH(PC_ROPE_APPEND, "rope_append_kernel", rope_append_kernel, dim3(T), dim3(row_threads), 0, st,
               static_cast<const act_t*>(ws.qkv), ws.q_rot, kvl, static_cast<const float2*>(g->rope_tab), g->tb,
               H, hd, R, C);
-    // a4: segment-masked causal attention over the ring
-    {
-      auto att = hd == 128 ? (g->window > 0 ? attention_kernel<128, true> : attention_kernel<128, false>)
-                           : (g->window > 0 ? attention_kernel<64, true> : attention_kernel<64, false>);
-      AF_LAUNCH(PC_ATTENTION, "attention_kernel", att, dim3(H, n_items), dim3(ATT_THREADS), att_smem_bytes(hd), st,
-                static_cast<const act_t*>(ws.q_rot), static_cast<const act_t*>(kvl), ws.attn, g->tb, H, R, C, scale_log2,
-                g->window);
-    }
+    if ((rc = launch_attention(l))) return rc;
     // a5: O projection, split-K slabs (added to the residual by the next kernel)
     {
       GemmParams gp{};
@@ -871,7 +1125,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   // ---- a9 ring commit: a relabelling, zero bytes moved (replaces InPlaceShiftKV) ----
   for (int s = 0; s < n_segs; ++s) g->len[segs[s].req_id] = segs[s].start_pos + segs[s].len;
   g->last_T = T;
-  return AF_OK;
+  return serialise_done(ctx, st);
 }
 
 extern "C" int af_packed_forward(const af_weights* w, const void* packed_embeds, const af_segment* segs, int32_t n_segs,
@@ -897,7 +1151,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   for (int i = 0; i < n_rows; ++i) rl.rows[i] = rows[i];
   {
     ProfScope ps_(PC_RMSNORM, st);
-    cudaError_t le = launch_k(gather_norm_kernel, dim3(n_rows), dim3(row_threads_for(c.d_model)), 0, st, rl, hidden,
+    cudaError_t le = launch_k1(gather_norm_kernel, dim3(n_rows), dim3(row_threads_for(c.d_model)), 0, st, rl, hidden,
                               reinterpret_cast<const __nv_bfloat16*>(w->g_final), ws.xn, c.d_model, c.rms_eps);
     if (le != cudaSuccess) return fail(AF_ERR_CUDA, "launch of gather_norm_kernel failed: %s", cudaGetErrorString(le));
   }

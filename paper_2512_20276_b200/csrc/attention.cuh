@@ -54,10 +54,6 @@ __device__ __forceinline__ void mma_f16_16816(float* c, const uint32_t* a, uint3
       : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&h);
-}
 
 // byte offset of 16-byte chunk `chunk` of row `row` in a [rows][HD] 16-bit tile with XOR swizzle
 template <int HD>

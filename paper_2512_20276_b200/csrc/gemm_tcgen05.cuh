@@ -102,19 +102,19 @@ struct GemmParams {
   int split;           // GemmSplit
   int splits;          // SPLIT_K: pieces per tile
   const GemmPiece* sched;  // device: [clusters][GEMM_MAX_PIECES] pieces, ended by pair = -1
+  int n_cl;            // clusters of the launch (= rows of sched in use)
   int stages;
   int w_pre;           // weight tiles (pipeline stages) requested before griddepcontrol.wait
   int stg_bytes, stg_bufs;  // epilogue staging per warp: stg_bufs buffers of stg_bytes (2 x 4096, or 1 x 2048 to fit a stage more)
   int epi;             // GemmEpilogue
   int w_fp16;          // 1: the weight matrices already hold fp16 (af_convert_bf16_to_fp16); 0: bf16, converted per tile
-  int out_bf16;        // 0 = fp32 output (TMA stores through map_out), 2 = fp16 (16-byte global stores, fields below)
+  int out_f16;        // 0 = fp32 output (TMA stores through map_out), 2 = fp16 (16-byte global stores, fields below)
   void* out;           // fp16 output: element (feature f, middle m, token t) at out + t * out_ld_tok + m * out_ld_mid + f
   long long out_ld_tok, out_ld_mid;
   int out_features;    // features per middle index (multiple of 8): clips a ragged last tile
   void* partial;       // stream-K partials: fp32 [slot][512 tokens][128 features] written through map_part, or
   int part_f16;        // (part_f16, with fp16 outputs) raw fp16 staging images [slot][32-token chunk][lane quadrant][2 KB]
-  int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner
-  long long* trace;    // debug: [grid][32] globaltimer stamps, or nullptr
+  int* flags;          // [grid] 0/1: set by the contributor, cleared by the owner (per stream: af_lib.cu StreamCtx)
 };
 
 #define AF_EPI_BAR_STR2(n) "bar.sync 1, " #n ";\n"

@@ -29,10 +29,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
   // 2-CTA cluster: both CTAs sweep the same k-blocks of two neighbouring weight tiles and each loads one half of the
   // activation k-block, multicast into both (halves the L2 -> SM traffic of the operand every CTA needs in full)
   const int crank = p.cluster > 1 ? static_cast<int>(cluster_ctarank()) : 0;
-  const int cl = cta / p.cluster;   // work is split over clusters; a cluster's unit = (tile pair, k-block)
-  long long* trace = p.trace ? p.trace + static_cast<size_t>(cta) * 32 : nullptr;
-#define AF_TRACE(slot) do { if (trace) trace[slot] = static_cast<long long>(globaltimer_ns()); } while (0)
-  if (trace && threadIdx.x == 0) AF_TRACE(0);
+  // Work is split over clusters (unit = (tile pair, k-block)).  Schedule row n_cl - 1 - (launch order): a stream-K
+  // owner waits for contributor pieces of HIGHER schedule rows, i.e. of clusters that were dispatched EARLIER, so a
+  // waiting CTA never depends on one that is not yet resident (no deadlock when the grid is only partly resident).
+  const int cl = p.n_cl - 1 - cta / p.cluster;
 
   // the first use of this cluster's piece list (a dependent global load in front of the first TMA request) would cost
   // ~0.8 us after the cluster barrier: pull its line into L1 now
@@ -154,9 +154,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         advance();
         ++n_pre;
       }
-      AF_TRACE(24);
       pdl_wait();
-      AF_TRACE(25);
       for (int i = 0; i < n_pre; ++i) load_x(kb_pre[i], i);
       int stage = n_pre == p.stages ? 0 : n_pre;
       uint32_t phase = n_pre == p.stages ? 1 : 0;
@@ -169,13 +167,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         advance();
         if (++stage == p.stages) { stage = 0; phase ^= 1; }
       }
-      AF_TRACE(26);
     }
   } else if (warp == GEMM_EPI_WARPS + 1) {
     // ================================ MMA issuer (one thread) ================================
     if (lane == 0 && !(mma2 && crank != 0)) {   // mma2: only the pair's leader issues
-      const uint32_t idesc1 = umma_idesc_bf16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n1);
-      const uint32_t idesc2 = umma_idesc_bf16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n2 > 0 ? p.n2 : 16);
+      const uint32_t idesc1 = umma_idesc_f16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n1);
+      const uint32_t idesc2 = umma_idesc_f16(mma2 ? 2 * GEMM_BM : GEMM_BM, p.n2 > 0 ? p.n2 : 16);
       int stage = 0;
       uint32_t phase = 0, acc_phase = 0;
       for (int pi = 0; pi < GEMM_MAX_PIECES; ++pi) {
@@ -202,8 +199,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
               umma_f16_cg2(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
               if (p.n2 > 0) umma_f16_cg2(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
             } else {
-            umma_bf16(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
-            if (p.n2 > 0) umma_bf16(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
+            umma_f16_cg1(tmem_base, da + 2 * k, db1 + 2 * k, idesc1, accum);
+            if (p.n2 > 0) umma_f16_cg1(tmem_base + p.n1, da + 2 * k, db2 + 2 * k, idesc2, accum);
             }
           }
           // frees the smem slot when these MMAs have read it (in a cluster: in both CTAs, the peer multicasts into it)
@@ -229,7 +226,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
     // 16-bit outputs (every GEMM of the forward) are drained in the mma fragment layout: tcgen05.ld.16x256b gives thread
     // t (feature t/4 [+8], tokens 2(t%4), +1 of every 8), which is what stmatrix.trans writes as [token][feature] rows.
     // Byte offset of this lane's row address inside a staging image (token group 0; the others are + 512 bytes):
-    constexpr bool frag = kFrag;   // == (p.out_bf16 != 0), a template parameter so that each variant holds one epilogue
+    constexpr bool frag = kFrag;   // == (p.out_f16 != 0), a template parameter so that each variant holds one epilogue
     const uint32_t frag_off64 = (lane & 7) * 64 + (((lane >> 3) ^ ((lane & 7) >> 1)) << 4);   // 64-byte rows, SWIZZLE_64B
     const uint32_t frag_off32 = ((lane >> 4) * 8 + (lane & 7)) * 32 + ((((lane >> 3) & 1) ^ ((lane & 7) >> 2)) << 4);  // 32-byte rows, SWIZZLE_32B
     // ... and of the 16-byte piece this lane reads back and stores: token lane/4 (+ 8 per group), features 8(lane%4).. for
@@ -255,7 +252,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       ++n_st;
     };
     pdl_wait();
-    if (etid == 0) AF_TRACE(1);
     int piece = 0;
     const int stage_area = p.stages * static_cast<int>(stage_bytes);
     uint32_t acc_phase = 0, fix_phase = 0, cphase = 0;
@@ -299,7 +295,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         }
         AF_EPI_BAR();
       }
-      if (etid == 0 && piece < 4) AF_TRACE(2 + 4 * piece);
       store_ok = tile_valid;
       // ---- tile-uniform store coordinates: (feature, middle, token) of map_out ----
       int f0, mid;
@@ -440,7 +435,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           for (int j = 0; j < 16; j += 2) {
             const float g0 = v[j], g1 = v[j + 1];
             const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * v[16 + j], h1 = __fdividef(g1, 1.f + __expf(-g1)) * v[17 + j];
-            h[j >> 1] = pack_act(fminf(fmaxf(h0, -65504.f), 65504.f), fminf(fmaxf(h1, -65504.f), 65504.f));
+            h[j >> 1] = pack_act(h0, h1);   // (saturating conversion)
           }
           __syncwarp();
           const uint32_t sa = smem_u32(stg_base);
@@ -479,7 +474,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
       // (everything above is address arithmetic: done while the MMAs of this piece are still running)
       if (has_mma) mbar_wait(&tmem_full_bar, acc_phase);
       tc_fence_after();
-      if (etid == 0 && piece < 4) AF_TRACE(3 + 4 * piece);
       for (int b0 = 0; b0 < n_pad && b0 < p.T; b0 += blk_cols) {
         const int b1 = min(b0 + blk_cols, n_pad);
         float v[32];
@@ -489,7 +483,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           float vb[32];
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
-            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
           }
           auto issue = [&](int c0, float* w) {
             if (has_mma) {
@@ -520,7 +513,6 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         } else if (n_groups <= 1) {
           if (n_groups == 1) {
             load_group(0, n_contrib, b0, b1);
-            if (etid == 0 && piece < 4) AF_TRACE(4 + 4 * piece);
           }
           for (int c0 = b0 + 32 * par; c0 < b1 && c0 < p.T; c0 += GEMM_BLK) {
             const int cw = min(32, b1 - c0);
@@ -554,13 +546,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
           atomicExch(p.flags + my_slot, 1);
         }
       }
-      if (etid == 0 && piece < 4) AF_TRACE(5 + 4 * piece);
       ++piece;
       if (has_mma) acc_phase ^= 1;
     }
     if (lane == 0) bulk_wait<0>();  // all output stores are complete before the CTA exits
   }
-#undef AF_TRACE
 #undef stg
 
   tc_fence_before();

@@ -9,12 +9,16 @@
 namespace af {
 
 // Activations (normed rows, q/k/v, the KV ring, attention probabilities and outputs, the SwiGLU product) are fp16:
-// same bytes as bf16 with 3 more mantissa bits.  Weights are bf16 in global memory and are converted to fp16 (exactly)
-// tile by tile in shared memory; every accumulation is fp32.
+// same bytes as bf16 with 3 more mantissa bits.  The bf16-valued weights are fp16 too by the time the MMA reads them:
+// rewritten once at load time (af_convert_bf16_to_fp16 / af_prepare_gate_up, the default), or per tile in shared memory
+// (AF_WEIGHTS_BF16).  Every accumulation is fp32.
 using act_t = __half;
+// two fp32 -> packed fp16, round to nearest, SATURATING: a finite value beyond +-65504 becomes +-65504, never inf
+// (NaN stays NaN), so an outlier activation degrades one element instead of poisoning the residual stream.
 __device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
-  __half2 h = __floats2half2_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&h);
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;\n" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
 }
 __device__ __forceinline__ float act2f(act_t v) { return __half2float(v); }
 
@@ -22,16 +26,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
-
-__device__ __forceinline__ bool elect_one() {
-  uint32_t pred;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "elect.sync _|p, 0xffffffff;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}\n"
-      : "=r"(pred));
-  return pred != 0;
-}
 
 // ------------------------------------------------------------------------------------------------ mbarrier
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -95,28 +89,11 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, const void* s
                "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2)
                : "memory");
 }
-// shared -> global 1D bulk copy (bulk async-group completion), 16-byte aligned
-__device__ __forceinline__ void bulk_store_1d(void* gmem_dst, const void* smem_src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gmem_dst), "r"(smem_u32(smem_src)),
-               "r"(bytes)
-               : "memory");
-}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;\n" ::"n"(N) : "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;\n" ::"n"(N) : "memory"); }
-// L2 prefetch of a contiguous global range (size a multiple of 16).
-__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(reinterpret_cast<uint64_t>(gmem_src)), "r"(bytes)
-               : "memory");
-}
-// L2 prefetch of the box a later tma_load_2d will fetch (no shared memory, no barrier).
-__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* m, int32_t c0, int32_t c1) {
-  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];\n" ::"l"(reinterpret_cast<uint64_t>(m)),
-               "r"(c0), "r"(c1)
-               : "memory");
-}
 // As tma_load_2d, multicast to the CTAs of `cta_mask` in this cluster: the box lands at the same shared-memory offset
 // in every destination CTA and completes on the mbarrier at the same offset there.
 __device__ __forceinline__ void tma_load_2d_mc(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int32_t c0,
@@ -176,8 +153,8 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {  
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
 
-// D[tmem] (+)= A[smem] * B[smem]^T, bf16 x bf16 -> fp32, issued by ONE thread.
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+// D[tmem] (+)= A[smem] * B[smem]^T, fp16 x fp16 -> fp32 (cta_group::1), issued by ONE thread.
+__device__ __forceinline__ void umma_f16_cg1(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
                                           uint32_t accumulate) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
@@ -271,7 +248,7 @@ __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t smem_addr, uint32_t& 
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
-// Shared-memory matrix descriptor of a K-major bf16 tile stored as rows of 128 bytes with the 128-byte swizzle
+// Shared-memory matrix descriptor of a K-major 16-bit tile stored as rows of 128 bytes with the 128-byte swizzle
 // (what TMA writes for CU_TENSOR_MAP_SWIZZLE_128B with a 64-element inner box): start address, LBO = 1 (unused),
 // SBO = 1024 B between 8-row groups, descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.
 __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr) {
@@ -285,8 +262,8 @@ __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr) {
 }
 // Instruction descriptor, kind::f16: D = fp32 (bits 4-5 = 1), A = B = fp16 (format 0 in bits 7-9 and 10-12; bf16
 // would be 1), both K-major, M x N tile.  A and B must share one format: a bf16 x fp16 mix raises an
-// illegal-instruction fault on sm_100a, which is why the bf16 weight tiles are converted to fp16 in shared memory.
-__device__ __forceinline__ uint32_t umma_idesc_bf16(uint32_t M, uint32_t N) {
+// illegal-instruction fault on sm_100a, which is why bf16 weights are rewritten as fp16 (at load time, or per tile).
+__device__ __forceinline__ uint32_t umma_idesc_f16(uint32_t M, uint32_t N) {
   return (1u << 4) | (0u << 7) | (0u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 // two packed bf16 -> two packed fp16 (round to nearest; exact for finite |x| in [2^-14, 65504])
