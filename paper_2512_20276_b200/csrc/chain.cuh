@@ -195,40 +195,51 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
     const int req = gslot / C, slot = gslot - req * C;
     const act_t* src = qkv + static_cast<size_t>(i) * 3 * D;
     const float2* tab = rope_tab + static_cast<size_t>(pos) * half;
-    for (int w = gl; w < n_qk; w += 128) {
-      const int which = w / (H * per_head);           // 0 = q, 1 = k
-      const int rem = w - which * H * per_head;
-      const int h = rem / per_head, c = (rem - h * per_head) * 8;
-      const int col = which * D + h * hd + c;
-      uint4 rlo[QKV_MAX_SLABS_K], rhi[QKV_MAX_SLABS_K];
+    const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
+    for (int w0 = gl; w0 < n_qk; w0 += 256) {           // q, k: two (head, 8-element) items per lane at a time
+      uint4 rlo[2][QKV_MAX_SLABS_K], rhi[2][QKV_MAX_SLABS_K];
+      float4 cs[2][4];
+      int colv[2], hv[2], cv[2];
 #pragma unroll
-      for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) {   // (all QKV_MAX_SLABS_K slab buffers exist; slabs >= ns are not added)
-        rlo[sl] = __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + col));
-        rhi[sl] = __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + col + half));
+      for (int u = 0; u < 2; ++u) {
+        const int w = w0 + 128 * u < n_qk ? w0 + 128 * u : w0;
+        const int which = w / (H * per_head);           // 0 = q, 1 = k
+        const int rem = w - which * H * per_head;
+        hv[u] = rem / per_head; cv[u] = (rem - hv[u] * per_head) * 8;
+        colv[u] = which * D + hv[u] * hd + cv[u];
+        const int ns = s_pair_slabs[colv[u] / (2 * GEMM_BM)];   // (col and col + half lie in the same 128-feature tile)
+#pragma unroll
+        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) {
+          rlo[u][sl] = sl < ns ? __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + colv[u])) : zero4;
+          rhi[u][sl] = sl < ns ? __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + colv[u] + half)) : zero4;
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) cs[u][e] = __ldg(reinterpret_cast<const float4*>(tab + cv[u]) + e);   // (cos, sin) of 2 elements each
       }
-      float4 cs[4];
 #pragma unroll
-      for (int e = 0; e < 4; ++e) cs[e] = __ldg(reinterpret_cast<const float4*>(tab + c) + e);   // (cos, sin) of 2 elements each
-      const int ns = s_pair_slabs[col / (2 * GEMM_BM)];   // (col and col + half lie in the same 128-feature tile)
-      float lo[8], hi[8];
+      for (int u = 0; u < 2; ++u) {
+        float lo[8], hi[8];
 #pragma unroll
-      for (int m = 0; m < 8; ++m) { lo[m] = 0.f; hi[m] = 0.f; }
+        for (int m = 0; m < 8; ++m) { lo[m] = 0.f; hi[m] = 0.f; }
 #pragma unroll
-      for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) { add_h8(rlo[sl], sl < ns, lo); add_h8(rhi[sl], sl < ns, hi); }
-      uint4 out_lo, out_hi;
-      uint32_t* ol = reinterpret_cast<uint32_t*>(&out_lo);
-      uint32_t* oh = reinterpret_cast<uint32_t*>(&out_hi);
+        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) { add_h8(rlo[u][sl], true, lo); add_h8(rhi[u][sl], true, hi); }
+        uint4 out_lo, out_hi;
+        uint32_t* ol = reinterpret_cast<uint32_t*>(&out_lo);
+        uint32_t* oh = reinterpret_cast<uint32_t*>(&out_hi);
 #pragma unroll
-      for (int e = 0; e < 8; e += 2) {
-        const float4 t4 = cs[e >> 1];                   // cos(e), sin(e), cos(e + 1), sin(e + 1)
-        ol[e >> 1] = pack_act(lo[e] * t4.x - hi[e] * t4.y, lo[e + 1] * t4.z - hi[e + 1] * t4.w);
-        oh[e >> 1] = pack_act(hi[e] * t4.x + lo[e] * t4.y, hi[e + 1] * t4.z + lo[e + 1] * t4.w);
+        for (int e = 0; e < 8; e += 2) {
+          const float4 t4 = cs[u][e >> 1];                // cos(e), sin(e), cos(e + 1), sin(e + 1)
+          ol[e >> 1] = pack_act(lo[e] * t4.x - hi[e] * t4.y, lo[e + 1] * t4.z - hi[e + 1] * t4.w);
+          oh[e >> 1] = pack_act(hi[e] * t4.x + lo[e] * t4.y, hi[e + 1] * t4.z + lo[e + 1] * t4.w);
+        }
+        const bool is_q = colv[u] < D;
+        act_t* dst = is_q ? q_out + static_cast<size_t>(i) * D + hv[u] * hd + cv[u]
+                          : kv_layer + ((static_cast<size_t>(0 * R + req) * H + hv[u]) * C + slot) * hd + cv[u];
+        if (w0 + 128 * u < n_qk) {
+          *reinterpret_cast<uint4*>(dst) = out_lo;
+          *reinterpret_cast<uint4*>(dst + half) = out_hi;
+        }
       }
-      act_t* dst = (which == 0)
-          ? q_out + static_cast<size_t>(i) * D + h * hd + c
-          : kv_layer + ((static_cast<size_t>(0 * R + req) * H + h) * C + slot) * hd + c;
-      *reinterpret_cast<uint4*>(dst) = out_lo;
-      *reinterpret_cast<uint4*>(dst + half) = out_hi;
     }
     for (int w0 = gl; w0 < n_v; w0 += 256) {          // v: two 8-element items per lane at a time
       uint4 rv[2][QKV_MAX_SLABS_K];
@@ -236,17 +247,19 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
       for (int u = 0; u < 2; ++u) {
         const int w = w0 + 128 * u < n_v ? w0 + 128 * u : w0;
 #pragma unroll
-        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) rv[u][sl] = __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + 2 * D + w * 8));
+        const int ns = s_pair_slabs[(2 * D + w * 8) / (2 * GEMM_BM)];
+#pragma unroll
+        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl)
+          rv[u][sl] = sl < ns ? __ldcg(reinterpret_cast<const uint4*>(src + sl * slab_stride + 2 * D + w * 8)) : zero4;
       }
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int w = w0 + 128 * u;
-        const int ns = s_pair_slabs[(2 * D + (w < n_v ? w : w0) * 8) / (2 * GEMM_BM)];
         float o[8];
 #pragma unroll
         for (int m = 0; m < 8; ++m) o[m] = 0.f;
 #pragma unroll
-        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) add_h8(rv[u][sl], sl < ns, o);
+        for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl) add_h8(rv[u][sl], true, o);
         const int h = (w * 8) / hd, c = (w * 8) - h * hd;
         uint4 v;
         v.x = pack_act(o[0], o[1]); v.y = pack_act(o[2], o[3]); v.z = pack_act(o[4], o[5]); v.w = pack_act(o[6], o[7]);
