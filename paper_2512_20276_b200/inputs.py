@@ -126,3 +126,65 @@ def prediction_rows(segs):
 
 def total_rows(segs) -> int:
     return sum(s[3] for s in segs)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# f4 ("orthogonal to ... quantization"): weight-only FP8 storage.  Input preparation,
+# not part of the method: a projection matrix W [out, in] is stored as one E4M3 code per element plus one fp32 scale
+# per OUTPUT channel, scale_f = max_k |W_fk| / 448 (1 for an all-zero row), code_fk = E4M3(round-to-nearest-even of
+# W_fk / scale_f, clamped to +-448).  Both sides consume the SAME dequantised values  W'_fk = value(code_fk) * scale_f:
+# the oracle as fp32 matrices (fp8_dequantize), the CUDA library as the codes and the scales (it widens the codes to
+# fp16 exactly and applies the scale to the fp32 accumulator).  E4M3 ("fn"): 1 sign, 4 exponent (bias 7), 3 mantissa
+# bits, no infinities, 0x7f / 0xff = NaN, largest finite 448, subnormals m/8 * 2^-6.
+# ---------------------------------------------------------------------------------------------------------
+FP8_MAX = 448.0
+_FP8_MATRICES = ("wq", "wk", "wv", "wo", "w_gate", "w_up", "w_down")
+
+
+def fp8_decode(codes: torch.Tensor) -> torch.Tensor:
+    """uint8 E4M3 codes -> fp32 values, by the format's definition (not by a library cast)."""
+    c = codes.to(torch.int32)
+    sign = torch.where((c & 0x80) != 0, -1.0, 1.0).to(torch.float32)
+    e = ((c >> 3) & 0xF).to(torch.float32)
+    m = (c & 0x7).to(torch.float32)
+    normal = torch.pow(torch.tensor(2.0), e - 7.0) * (1.0 + m / 8.0)
+    sub = (m / 8.0) * 2.0 ** -6
+    v = torch.where(e > 0, normal, sub)
+    v = torch.where((c & 0x7F) == 0x7F, torch.tensor(float("nan")), v)
+    return sign * v
+
+
+def fp8_quantize(w: torch.Tensor):
+    """[out, in] matrix (any float dtype) -> (codes uint8 [out, in], scale fp32 [out])."""
+    wf = w.to(torch.float32)
+    amax = wf.abs().amax(dim=1)
+    scale = torch.where(amax > 0, amax / FP8_MAX, torch.ones_like(amax))
+    q = (wf / scale[:, None]).clamp(-FP8_MAX, FP8_MAX)
+    codes = q.to(torch.float8_e4m3fn).view(torch.uint8)       # round to nearest even (library primitive, pinned in tests)
+    return codes.contiguous(), scale.contiguous()
+
+
+def fp8_dequantize(codes: torch.Tensor, scale: torch.Tensor) -> torch.Tensor:
+    """The values both sides compute with: fp32 value(code) * scale of the row."""
+    return fp8_decode(codes) * scale[:, None]
+
+
+def quantize_weights_fp8(weights: dict) -> dict:
+    """{'layers': [{name: (codes, scale)} for the seven projection matrices + the bf16 gains], 'dequant': a weights dict
+    in make_weights' shape whose projection matrices are the fp32 dequantised values (for the oracle); g_final / w_lm
+    are passed through (the LM head stays 16-bit)."""
+    out = {"layers": [], "dequant": {"layers": [], "g_final": weights["g_final"], "w_lm": weights["w_lm"]},
+           "g_final": weights["g_final"], "w_lm": weights["w_lm"]}
+    for L in weights["layers"]:
+        q, d = {}, {}
+        for name, t in L.items():
+            if name in _FP8_MATRICES:
+                codes, scale = fp8_quantize(t)
+                q[name] = (codes, scale)
+                d[name] = fp8_dequantize(codes, scale)
+            else:
+                q[name] = t
+                d[name] = t
+        out["layers"].append(q)
+        out["dequant"]["layers"].append(d)
+    return out
