@@ -85,12 +85,28 @@ typedef struct {                 /* all device bf16 */
 #define AF_WEIGHTS_FP16_GU 2      /* as AF_WEIGHTS_FP16, and w_gate of every layer holds gate AND up, interleaved by
                                    * af_prepare_gate_up (w_up is ignored): one TMA box per weight tile instead of eight */
 
+#define AF_WEIGHTS_FP8 3          /* f4, weight-only FP8 storage: wq..w_down hold one E4M3 code per element
+                                   * (uint8, [out, in] row-major), w_gate holds gate AND up interleaved by
+                                   * af_prepare_gate_up_fp8 (w_up is ignored), af_weights.scales holds one fp32 scale per
+                                   * OUTPUT channel; the matrix the library multiplies by is value(code) * scale[out].
+                                   * The codes are widened to fp16 (exactly) tile by tile in shared memory and the scale
+                                   * is applied to the fp32 accumulator, so HBM carries half the bytes of the 16-bit
+                                   * formats.  w_lm stays a prepared fp16 matrix.  Packed steps of more than 512 rows
+                                   * return AF_ERR_UNSUPPORTED in this format. */
+
+typedef struct {                  /* AF_WEIGHTS_FP8: device fp32 [out_features] per matrix */
+  const float *sq, *sk, *sv, *so; /* [d_model] */
+  const float *s_gate, *s_up;     /* [ffn] */
+  const float *s_down;            /* [d_model] */
+} af_layer_scales;
+
 typedef struct {
   af_model_cfg cfg;
   const af_layer_weights* layers; /* HOST array [n_layers] of device pointers */
   const void* g_final;            /* device bf16 [d_model] */
   const void* w_lm;               /* device bf16 (or prepared fp16) [vocab, d_model] */
-  int32_t weight_format;          /* AF_WEIGHTS_BF16, AF_WEIGHTS_FP16 or AF_WEIGHTS_FP16_GU: format of wq..w_down and w_lm (gains stay bf16) */
+  int32_t weight_format;          /* AF_WEIGHTS_BF16, _FP16, _FP16_GU or _FP8: format of wq..w_down (and, except for _FP8, of w_lm); gains stay bf16 */
+  const af_layer_scales* scales;  /* HOST array [n_layers] of device pointers; read only when weight_format == AF_WEIGHTS_FP8 */
 } af_weights;
 
 /* Load-time weight preparation: dst[i] = fp16(src[i]) for n_elems bf16 values (n_elems % 8 == 0,
@@ -107,6 +123,12 @@ int af_convert_bf16_to_fp16(const void* src_bf16, void* dst_fp16, size_t n_elems
 size_t af_gate_up_rows(int32_t ffn);
 int af_prepare_gate_up(const void* gate_bf16, const void* up_bf16, void* dst_fp16, int32_t ffn, int32_t d_model,
                        void* cuda_stream);
+
+/* AF_WEIGHTS_FP8: the same row order for E4M3 codes (one byte per element; copied, not converted).  gate / up are
+ * [ffn, d_model] uint8, dst is af_gate_up_rows(ffn) x d_model uint8, rows of features >= ffn are zero codes; all device,
+ * 16-byte aligned, d_model % 16 == 0.  Enqueued on cuda_stream. */
+int af_prepare_gate_up_fp8(const void* gate_codes, const void* up_codes, void* dst_codes, int32_t ffn, int32_t d_model,
+                           void* cuda_stream);
 
 /* Bytes of kv_mem needed for (cfg, ring): 2 * n_layers * R * n_heads * C * head_dim * 2. */
 size_t af_ring_bytes(const af_model_cfg* cfg, const af_ring_cfg* ring);

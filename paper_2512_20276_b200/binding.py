@@ -43,12 +43,16 @@ class af_layer_weights(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("wq", "wk", "wv", "wo", "w_gate", "w_up", "w_down", "g_attn", "g_mlp")]
 
 
+class af_layer_scales(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("sq", "sk", "sv", "so", "s_gate", "s_up", "s_down")]
+
+
 class af_weights(C.Structure):
     _fields_ = [("cfg", af_model_cfg), ("layers", C.POINTER(af_layer_weights)), ("g_final", C.c_void_p),
-                ("w_lm", C.c_void_p), ("weight_format", C.c_int32)]
+                ("w_lm", C.c_void_p), ("weight_format", C.c_int32), ("scales", C.POINTER(af_layer_scales))]
 
 
-EXPORTS = ["af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
+EXPORTS = ["af_prepare_gate_up_fp8", "af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
            "af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
@@ -83,6 +87,8 @@ def load_library():
     L.af_gate_up_rows.restype = C.c_size_t
     L.af_prepare_gate_up.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp]
     L.af_prepare_gate_up.restype = C.c_int
+    L.af_prepare_gate_up_fp8.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp]
+    L.af_prepare_gate_up_fp8.restype = C.c_int
     L.af_ring_create.argtypes = [C.POINTER(af_model_cfg), C.POINTER(af_ring_cfg), vp, sz, C.POINTER(vp)]
     L.af_ring_reset_slot.argtypes = [vp, i32, i32]
     L.af_ring_set_window.argtypes = [vp, i32, i32]
@@ -164,7 +170,7 @@ class Weights:
         self.w_lm = self._prep(host_weights["w_lm"].to(torch.bfloat16).contiguous().to(device), True)
         torch.cuda.synchronize()
         self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr(),
-                                 2 if prepared is True else (1 if prepared else 0))
+                                 2 if prepared is True else (1 if prepared else 0), None)
 
     def _prep(self, t: torch.Tensor, is_matrix: bool) -> torch.Tensor:
         if not (self.prepared and is_matrix):
@@ -172,6 +178,50 @@ class Weights:
         out = torch.empty(t.shape, dtype=torch.float16, device=t.device)
         _check(load_library().af_convert_bf16_to_fp16(t.data_ptr(), out.data_ptr(), t.numel(), _stream_ptr()))
         return out
+
+
+class WeightsFP8:
+    """f4: AF_WEIGHTS_FP8.  `quantized` is inputs.quantize_weights_fp8(host_weights): per projection matrix (E4M3 codes
+    uint8 [out, in], fp32 scale [out]).  The codes go to the device as they are (gate | up interleaved by
+    af_prepare_gate_up_fp8, a byte permutation), the scales as fp32 vectors; gains stay bf16 and the LM head a prepared
+    fp16 matrix."""
+
+    _SCALE_OF = {"wq": "sq", "wk": "sk", "wv": "sv", "wo": "so", "w_gate": "s_gate", "w_up": "s_up", "w_down": "s_down"}
+
+    def __init__(self, cfg, quantized: dict, device="cuda"):
+        lib = load_library()
+        self.cfg = cfg
+        self.tensors = []
+        self._layers = (af_layer_weights * cfg.n_layers)()
+        self._scales = (af_layer_scales * cfg.n_layers)()
+        for l, L in enumerate(quantized["layers"]):
+            for name, sname in self._SCALE_OF.items():
+                codes, scale = L[name]
+                sc = scale.to(torch.float32).contiguous().to(device)
+                self.tensors.append(sc)
+                setattr(self._scales[l], sname, sc.data_ptr())
+                if name in ("w_gate", "w_up"):
+                    continue
+                cd = codes.contiguous().to(device)
+                self.tensors.append(cd)
+                setattr(self._layers[l], name, cd.data_ptr())
+            gate, up = L["w_gate"][0].contiguous().to(device), L["w_up"][0].contiguous().to(device)
+            gu = torch.empty(lib.af_gate_up_rows(cfg.ffn), cfg.d_model, dtype=torch.uint8, device=device)
+            _check(lib.af_prepare_gate_up_fp8(gate.data_ptr(), up.data_ptr(), gu.data_ptr(), cfg.ffn, cfg.d_model, _stream_ptr()))
+            torch.cuda.synchronize()
+            self.tensors.append(gu)
+            self._layers[l].w_gate = gu.data_ptr()
+            self._layers[l].w_up = gu.data_ptr()
+            for name in ("g_attn", "g_mlp"):
+                t = L[name].to(torch.bfloat16).contiguous().to(device)
+                self.tensors.append(t)
+                setattr(self._layers[l], name, t.data_ptr())
+        self.g_final = quantized["g_final"].to(torch.bfloat16).contiguous().to(device)
+        lm = quantized["w_lm"].to(torch.bfloat16).contiguous().to(device)
+        self.w_lm = torch.empty(lm.shape, dtype=torch.float16, device=device)
+        _check(lib.af_convert_bf16_to_fp16(lm.data_ptr(), self.w_lm.data_ptr(), lm.numel(), _stream_ptr()))
+        torch.cuda.synchronize()
+        self.struct = af_weights(_cfg_struct(cfg), self._layers, self.g_final.data_ptr(), self.w_lm.data_ptr(), 3, self._scales)
 
 
 class Ring:

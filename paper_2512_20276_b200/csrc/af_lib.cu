@@ -90,7 +90,7 @@ struct MapKey {
 static std::map<MapKey, CUtensorMap> g_maps;
 
 // Cached cuTensorMapEncodeTiled.  dims / box innermost first; strides (bytes) of dims 1..rank-1.
-static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 2 = bf16, -2 = fp16, 4 = fp32 */ const unsigned long long* dims,
+static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 2 = bf16, -2 = fp16, 4 = fp32, 1 = uint8 (E4M3 codes) */ const unsigned long long* dims,
                       const unsigned long long* strides, const unsigned* box, int swizzle /* 0 none, 128, 64 or 32 bytes */, CUtensorMap* out) {
   std::lock_guard<std::mutex> lk(g_mu);
   MapKey key;
@@ -116,7 +116,8 @@ static int get_map_nd(const void* ptr, int elem_bytes, int rank, /* elem_bytes: 
   for (int i = 0; i < rank; ++i) { d[i] = dims[i]; bx[i] = box[i]; }
   for (int i = 0; i + 1 < rank; ++i) st[i] = strides[i];
   const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
-                                 : (elem_bytes == -2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32);
+                                 : (elem_bytes == -2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16
+                                 : (elem_bytes == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32));
   CUresult r = g_encode(&m, dt, rank, const_cast<void*>(ptr), d, st, bx, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                         swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
                         : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
@@ -136,6 +137,16 @@ static int get_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
   const unsigned long long strides[1] = {static_cast<unsigned long long>(cols) * 2};
   const unsigned box[2] = {static_cast<unsigned>(GEMM_BK), static_cast<unsigned>(box_rows)};
   return get_map_nd(ptr, fp16 ? -2 : 2, 2, dims, strides, box, 128, out);
+}
+
+// E4M3 weight matrix [rows, cols] (one byte per element), box = [128 rows, 64 codes], no swizzle (the tile is widened to
+// the fp16 UMMA layout by the kernel), zero fill out of bounds.
+static int get_map_fp8(const void* ptr, int rows, int cols, CUtensorMap* out) {
+  if (cols % 16) return fail(AF_ERR_ARG, "FP8 matrix %p [%d,%d] needs a 16-byte row pitch", ptr, rows, cols);
+  const unsigned long long dims[2] = {static_cast<unsigned long long>(cols), static_cast<unsigned long long>(rows)};
+  const unsigned long long strides[1] = {static_cast<unsigned long long>(cols)};
+  const unsigned box[2] = {static_cast<unsigned>(GEMM_BK), static_cast<unsigned>(GEMM_BM)};
+  return get_map_nd(ptr, 1, 2, dims, strides, box, 0, out);
 }
 
 // Output view of a GEMM (see GemmParams): element (feature f, middle m, token t) at ptr + t*ld_tok + m*ld_mid + f.
@@ -222,7 +233,8 @@ static int get_ctx(DevCtx** out) {
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
-  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
@@ -241,7 +253,7 @@ static int get_ctx(DevCtx** out) {
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    if (cudaOccupancyMaxActiveClusters(&max_cl, layer_chain_kernel, &cfg) != cudaSuccess || max_cl < 1) { cudaGetLastError(); max_cl = c->num_sms / 2; }
+    if (cudaOccupancyMaxActiveClusters(&max_cl, layer_chain_kernel<false>, &cfg) != cudaSuccess || max_cl < 1) { cudaGetLastError(); max_cl = c->num_sms / 2; }
   }
   c->max_clusters = max_cl < c->num_sms / 2 ? max_cl : c->num_sms / 2;
   if (c->max_clusters < 1) c->max_clusters = 1;
@@ -574,6 +586,7 @@ struct ChainBuilder {
   int n_maps = 0;
   DevCtx* ctx = nullptr;
   int max_rows = 0;          // row capacity of the workspace buffers the activation maps cover
+  bool fp8 = false;          // AF_WEIGHTS_FP8: weight matrices are E4M3 codes + per-output-channel scales
   ChainBuilder() { memset(&a, 0, sizeof a); }
   int add_map(const CUtensorMap& m) {
     for (int i = 0; i < n_maps; ++i)
@@ -587,9 +600,9 @@ struct ChainBuilder {
 
 // One projection phase: y = x W^T over n_parts weight matrices stacked along the feature axis (a_pair = 2: gate | up
 // interleaved by af_prepare_gate_up).  split: SPLIT_K / SPLIT_SLABS (EPI_STORE, slabs) or SPLIT_STREAMK (EPI_SWIGLU).
-static int chain_add_gemm(ChainBuilder& b, const void* const* w, int n_parts, int part_rows, int a_pair, int K, int split, int max_slabs,
-                          int epi, const void* x, act_t* out, long long out_ld_tok, long long out_ld_slab, int out_features,
-                          const int** pair_slabs_out, int* n_slabs_out) {
+static int chain_add_gemm(ChainBuilder& b, const void* const* w, const float* const* scales, int n_parts, int part_rows, int a_pair, int K,
+                          int split, int max_slabs, int epi, const void* x, act_t* out, long long out_ld_tok, long long out_ld_slab,
+                          int out_features, const int** pair_slabs_out, int* n_slabs_out) {
   ChainPhase* P = b.next();
   if (!P) return fail(AF_ERR_UNSUPPORTED, "chain: too many phases");
   P->kind = CH_GEMM;
@@ -608,8 +621,11 @@ static int chain_add_gemm(ChainBuilder& b, const void* const* w, int n_parts, in
   for (int i = 0; i < 3; ++i) {
     CUtensorMap m;
     const int n_w = a_pair ? 1 : n_parts;
-    if ((rc = get_map(w[i < n_w ? i : 0], a_pair ? n_tiles * GEMM_BM : part_rows, K, GEMM_BM, &m))) return rc;
+    const int w_rows = a_pair ? n_tiles * GEMM_BM : part_rows;
+    if ((rc = b.fp8 ? get_map_fp8(w[i < n_w ? i : 0], w_rows, K, &m) : get_map(w[i < n_w ? i : 0], w_rows, K, GEMM_BM, &m))) return rc;
     if ((P->w_map[i] = b.add_map(m)) < 0) return fail(AF_ERR_UNSUPPORTED, "chain: too many tensor maps");
+    P->scale[i] = (b.fp8 && scales) ? scales[i < (a_pair ? 2 : n_parts) ? i : 0] : nullptr;
+    if (b.fp8 && !P->scale[i]) return fail(AF_ERR_ARG, "AF_WEIGHTS_FP8 needs af_weights.scales");
   }
   CUtensorMap mx;
   if ((rc = get_map(x, b.max_rows, K, b.a.n1 / 2, &mx))) return rc;
@@ -637,7 +653,7 @@ static int chain_add_rope(ChainBuilder& b, const act_t* qkv_slabs, long long sla
 
 static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   const int n_pad = b.a.n1 + b.a.n2;
-  const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2;
+  const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2 + (b.fp8 ? static_cast<int>(CH_RAW_BYTES) : 0);
   int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * 2048) / stage_bytes;
   if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
   if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "chain: a stage does not fit shared memory");
@@ -651,7 +667,7 @@ static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   }
   const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_EPI_WARPS * 2048 + 1024;
   cudaError_t e;
-  { ProfScope ps(cat, st); e = launch_k(layer_chain_kernel, dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
+  { ProfScope ps(cat, st); e = launch_k(b.fp8 ? layer_chain_kernel<true> : layer_chain_kernel<false>, dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
   if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of layer_chain_kernel failed: %s", cudaGetErrorString(e));
   return check_launch("layer_chain_kernel");
 }
@@ -875,6 +891,17 @@ extern "C" int af_prepare_gate_up(const void* gate, const void* up, void* dst, i
   return check_launch("interleave_gate_up_kernel");
 }
 
+extern "C" int af_prepare_gate_up_fp8(const void* gate, const void* up, void* dst, int32_t ffn, int32_t d_model, void* cuda_stream) {
+  if (!gate || !up || !dst || ffn <= 0 || d_model <= 0 || (d_model % 16)) return fail(AF_ERR_ARG, "null pointer, or d_model not a multiple of 16");
+  if ((reinterpret_cast<uintptr_t>(gate) | reinterpret_cast<uintptr_t>(up) | reinterpret_cast<uintptr_t>(dst)) & 15)
+    return fail(AF_ERR_ARG, "pointers must be 16-byte aligned");
+  const int vec_per_row = d_model / 16;
+  const size_t n_vec = af_gate_up_rows(ffn) * vec_per_row;
+  interleave_gate_up_bytes_kernel<<<static_cast<unsigned>((n_vec + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(
+      reinterpret_cast<const uint4*>(gate), reinterpret_cast<const uint4*>(up), reinterpret_cast<uint4*>(dst), ffn, vec_per_row, n_vec);
+  return check_launch("interleave_gate_up_bytes_kernel");
+}
+
 extern "C" int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters,
                                       int32_t splits, int32_t* pieces, int32_t max_clusters_out) {
   if (!pieces) return fail(AF_ERR_ARG, "null output");
@@ -901,8 +928,16 @@ static int check_weights(const af_weights* w, bool need_lm) {
       return fail(AF_ERR_ARG, "null weight pointer in layer %d", l);
   }
   if (need_lm && (!w->g_final || !w->w_lm)) return fail(AF_ERR_ARG, "null g_final / w_lm");
-  if (w->weight_format != AF_WEIGHTS_BF16 && w->weight_format != AF_WEIGHTS_FP16 && w->weight_format != AF_WEIGHTS_FP16_GU)
-    return fail(AF_ERR_ARG, "weight_format %d is not AF_WEIGHTS_BF16, AF_WEIGHTS_FP16 or AF_WEIGHTS_FP16_GU", w->weight_format);
+  if (w->weight_format != AF_WEIGHTS_BF16 && w->weight_format != AF_WEIGHTS_FP16 && w->weight_format != AF_WEIGHTS_FP16_GU &&
+      w->weight_format != AF_WEIGHTS_FP8)
+    return fail(AF_ERR_ARG, "weight_format %d is not AF_WEIGHTS_BF16, AF_WEIGHTS_FP16, AF_WEIGHTS_FP16_GU or AF_WEIGHTS_FP8", w->weight_format);
+  if (w->weight_format == AF_WEIGHTS_FP8) {
+    if (!w->scales) return fail(AF_ERR_ARG, "AF_WEIGHTS_FP8 needs af_weights.scales");
+    for (int l = 0; l < w->cfg.n_layers; ++l) {
+      const af_layer_scales& S = w->scales[l];
+      if (!S.sq || !S.sk || !S.sv || !S.so || !S.s_gate || !S.s_up || !S.s_down) return fail(AF_ERR_ARG, "null scale pointer in layer %d", l);
+    }
+  }
   return AF_OK;
 }
 
@@ -994,7 +1029,10 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     return AF_OK;
   };
   // ---- the layer chain (chain.cuh): per layer ONE persistent launch for every projection and row stage + attention ----
-  const bool use_chain = w->weight_format == AF_WEIGHTS_FP16_GU && T <= GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
+  const bool fp8 = w->weight_format == AF_WEIGHTS_FP8;
+  if (fp8 && (T > GEMM_MAX_TOK || D > 4096 || D % 256 != 0 || F < 128 || ctx->max_clusters < 2 || g_prof_stages))
+    return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8 runs on the layer chain only: T <= %d packed rows, d_model <= 4096 and a multiple of 256", GEMM_MAX_TOK);
+  const bool use_chain = (w->weight_format == AF_WEIGHTS_FP16_GU || fp8) && T <= GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
                          ctx->max_clusters >= 2 && !g_prof_stages;
   if (use_chain) {
     StreamCtx sctx;
@@ -1002,7 +1040,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     const long long split_stride = static_cast<long long>(ws.max_rows) * D;
     const long long qkv_stride = static_cast<long long>(ws.max_rows) * 3 * D;
     auto begin = [&](ChainBuilder& b) {
-      b.ctx = ctx; b.max_rows = ws.max_rows;
+      b.ctx = ctx; b.max_rows = ws.max_rows; b.fp8 = fp8;
       int n_pad = (T + 15) / 16 * 16;
       if (n_pad <= 256) { b.a.n1 = n_pad; b.a.n2 = 0; }
       else { b.a.n1 = ((T + 1) / 2 + 15) / 16 * 16; b.a.n2 = b.a.n1; }
@@ -1013,8 +1051,9 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     auto add_qkv_rope = [&](ChainBuilder& b, int l) -> int {
       const af_layer_weights& L = w->layers[l];
       const void* wqkv[3] = {L.wq, L.wk, L.wv};
+      const float* sqkv[3] = {fp8 ? w->scales[l].sq : nullptr, fp8 ? w->scales[l].sk : nullptr, fp8 ? w->scales[l].sv : nullptr};
       const int* pair_slabs = nullptr;
-      int r = chain_add_gemm(b, wqkv, 3, D, 0, D, SPLIT_SLABS, QKV_MAX_SLABS, EPI_STORE, ws.xn, ws.qkv, 3LL * D, qkv_stride, D, &pair_slabs, nullptr);
+      int r = chain_add_gemm(b, wqkv, sqkv, 3, D, 0, D, SPLIT_SLABS, QKV_MAX_SLABS, EPI_STORE, ws.xn, ws.qkv, 3LL * D, qkv_stride, D, &pair_slabs, nullptr);
       if (r) return r;
       return chain_add_rope(b, ws.qkv, qkv_stride, pair_slabs, ws.q_rot, g->kv + layer_elems * l);
     };
@@ -1032,12 +1071,15 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
       begin(b);
       int n_slabs = 0;
       const void* wo[3] = {L.wo, nullptr, nullptr};
-      if ((rc = chain_add_gemm(b, wo, 1, D, 0, D, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.attn, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
+      const float* so[3] = {fp8 ? w->scales[l].so : nullptr, nullptr, nullptr};
+      const float* sgu[3] = {fp8 ? w->scales[l].s_gate : nullptr, fp8 ? w->scales[l].s_up : nullptr, nullptr};
+      const float* sd[3] = {fp8 ? w->scales[l].s_down : nullptr, nullptr, nullptr};
+      if ((rc = chain_add_gemm(b, wo, so, 1, D, 0, D, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.attn, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
       if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, L.g_mlp, ws.xn))) return rc;
       const void* wgu[3] = {L.w_gate, nullptr, nullptr};
-      if ((rc = chain_add_gemm(b, wgu, 2, F, 2, D, SPLIT_STREAMK, 1, EPI_SWIGLU, ws.xn, ws.h, F, 0, F, nullptr, nullptr))) return rc;
+      if ((rc = chain_add_gemm(b, wgu, sgu, 2, F, 2, D, SPLIT_STREAMK, 1, EPI_SWIGLU, ws.xn, ws.h, F, 0, F, nullptr, nullptr))) return rc;
       const void* wd[3] = {L.w_down, nullptr, nullptr};
-      if ((rc = chain_add_gemm(b, wd, 1, D, 0, F, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.h, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
+      if ((rc = chain_add_gemm(b, wd, sd, 1, D, 0, F, SPLIT_K, GEMM_MAX_SPLITS, EPI_STORE, ws.h, reinterpret_cast<act_t*>(ws.split), D, split_stride, D, nullptr, &n_slabs))) return rc;
       if (l + 1 < c.n_layers) {
         if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, w->layers[l + 1].g_attn, ws.xn))) return rc;
         if ((rc = add_qkv_rope(b, l + 1))) return rc;
@@ -1157,7 +1199,7 @@ extern "C" int af_logits_rows(const af_weights* w, const float* hidden, const in
   }
   if ((rc = check_launch("gather_norm_kernel"))) return rc;
   GemmParams gp{};
-  gp.w_fp16 = w->weight_format != AF_WEIGHTS_BF16;
+  gp.w_fp16 = w->weight_format != AF_WEIGHTS_BF16;   // (AF_WEIGHTS_FP8: the LM head stays a prepared fp16 matrix)
   gp.n_parts = 1; gp.part_rows = c.vocab; gp.K = c.d_model; gp.split = SPLIT_STREAMK; gp.epi = EPI_STORE;
   gp.partial = ws.partial;
   if (c.vocab % 4) return fail(AF_ERR_UNSUPPORTED, "vocab must be a multiple of 4 (16-byte logits rows)");

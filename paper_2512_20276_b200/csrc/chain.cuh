@@ -40,6 +40,7 @@ struct ChainPhase {
   act_t* out;               // element (token t, slab s, part p, feature f) at out + s * out_ld_slab + t * out_ld_tok + p * part_rows + f
   long long out_ld_tok, out_ld_slab;
   int out_features;         // features per part (multiple of 8): clips a ragged last tile
+  const float* scale[3];    // FP8 weights: per-output-channel fp32 scales of the parts (a_pair: [0] = gate, [1] = up)
   // ---- CH_ROWS: x[i,:] (= embeds[i,:] | += sum of slabs[s][i,:]);  xn[i,:] = fp16(RMSNorm(x[i,:]; gain)) unless gain == nullptr ----
   const void* src;          // nullptr: nothing to add; embed != 0: bf16 [T, D] embeddings; else fp16 slabs [n_slabs][.][D]
   int embed, n_slabs;
@@ -69,6 +70,27 @@ struct ChainArgs {
   int H, hd, R, C;
   long long* trace;         // debug: [grid][CH_TRACE_SLOTS] globaltimer stamps, or nullptr
 };
+
+// FP8 weights (f4): a stage also holds the raw 8 KB E4M3 tile, which the epilogue warps widen to the fp16 UMMA tile
+constexpr uint32_t CH_RAW_BYTES = GEMM_BM * GEMM_BK;
+__device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t two_codes) {   // exact: every E4M3 value is an fp16 value
+  uint32_t r;
+  asm("cvt.rn.f16x2.e4m3x2 %0, %1;\n" : "=r"(r) : "h"(static_cast<unsigned short>(two_codes)));
+  return r;
+}
+__device__ __forceinline__ void mbar_arrive_leader_release(uint64_t* bar) {   // publishes this thread's (fenced) shared-memory writes to the pair's leader
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(leader_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {   // acquire at cluster scope
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  }
+}
 
 // Grid barrier = one 64-bit arrival counter that only ever grows (it never wraps in practice and is a multiple of the
 // grid size whenever no launch is in flight): barrier k of a launch is passed when count >= base + (k + 1) * grid.
@@ -269,6 +291,7 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
   }
 }
 
+template <bool kFp8>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -276,10 +299,13 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   const int n_pad = a.n1 + a.n2;
   constexpr uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
   const uint32_t b_bytes = static_cast<uint32_t>(n_pad / 2) * GEMM_BK * 2;   // this CTA's half of the activation rows
-  const uint32_t stage_bytes = a_bytes + b_bytes;
+  const uint32_t stage_bytes = a_bytes + b_bytes + (kFp8 ? CH_RAW_BYTES : 0u);   // [fp16 weight tile][activation boxes][raw FP8 tile]
   uint8_t* xch = tiles + static_cast<size_t>(a.stages) * stage_bytes;         // 8 x 2 KB epilogue staging
 
+  // full_bar: the stage's TMA loads have landed (FP8: the activation boxes only; the raw weight tile lands on this CTA's
+  // own wfull_bar and conv_bar, on the pair's leader, counts the epilogue warps of BOTH CTAs that have widened their tile)
   __shared__ uint64_t full_bar[GEMM_MAX_STAGES], empty_bar[GEMM_MAX_STAGES], tmem_full_bar, tmem_empty_bar;
+  __shared__ uint64_t wfull_bar[GEMM_MAX_STAGES], conv_bar[GEMM_MAX_STAGES];
   __shared__ uint32_t tmem_base_smem;
   __shared__ int deps_done;                         // grid barriers this CTA has passed (published to the producer)
   __shared__ float row_red[CH_ROW_GROUPS][4];
@@ -292,7 +318,10 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   long long* trace = a.trace ? a.trace + static_cast<size_t>(cta) * CH_TRACE_SLOTS : nullptr;
 
   if (warp == GEMM_EPI_WARPS && lane == 0) {
-    for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    for (int s = 0; s < a.stages; ++s) {
+      mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1);
+      mbar_init(&wfull_bar[s], 1); mbar_init(&conv_bar[s], 2 * GEMM_EPI_WARPS);
+    }
     mbar_init(&tmem_full_bar, 1);
     mbar_init(&tmem_empty_bar, 2 * GEMM_EPI_WARPS);   // the leader waits for both CTAs' drains
     fence_barrier_init();
@@ -350,8 +379,14 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
       auto advance = [&](Cursor& c) { if (++c.kb == c.kb1) next_piece(c); };
       const int h1 = a.n1 / 2;
       auto load_w = [&](const Cursor& c, int stage) {
-        if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
-        tma_load_2d_cg2(tiles + static_cast<size_t>(stage) * stage_bytes, c.wmap, &full_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
+        if (kFp8) {   // raw E4M3 tile -> this CTA's own barrier (its epilogue warps widen it); activations -> the leader's
+          if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * b_bytes);
+          mbar_arrive_expect_tx(&wfull_bar[stage], CH_RAW_BYTES);
+          tma_load_2d(tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes + b_bytes, c.wmap, &wfull_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
+        } else {
+          if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
+          tma_load_2d_cg2(tiles + static_cast<size_t>(stage) * stage_bytes, c.wmap, &full_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
+        }
       };
       auto load_x = [&](const Cursor& c, int stage) {
         uint8_t* sb = tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes;
@@ -424,6 +459,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           tc_fence_after();
           for (int kb = pc.kb0; kb < pc.kb1; ++kb) {
             mbar_wait(&full_bar[stage], phase);
+            if (kFp8) mbar_wait_cluster(&conv_bar[stage], phase);   // both CTAs' weight tiles have been widened to fp16
             tc_fence_after();
             const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
             const uint32_t sb = sa + a_bytes;
@@ -464,8 +500,8 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
       if (a.ph[ph].kind == CH_ROPE)
         for (int i = etid; i < 3 * a.D / (2 * GEMM_BM) && i < 64; i += GEMM_EPI_WARPS * 32) s_pair_slabs[i] = __ldg(a.ph[ph].pair_slabs + i);
     AF_EPI_BAR();
-    uint32_t acc_phase = 0;
-    int n_bar = 0;
+    uint32_t acc_phase = 0, cphase = 0;
+    int n_bar = 0, cstage = 0;
 
     for (int ph = 0; ph < a.n_phases; ++ph) {
       const ChainPhase& P = a.ph[ph];
@@ -477,6 +513,29 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           const bool has_mma = pc.kb1 > pc.kb0;
           const int tile = pc.pair * 2 + crank;
           const bool tile_valid = tile < P.n_tiles;
+          if (kFp8) {
+            // ---- widen this piece's raw E4M3 weight tiles to the fp16 UMMA tile (K-major, 128-byte swizzle), stage by stage
+            //      as they land: thread (row r, half h) rewrites codes [32h, 32h + 32) of row r as four 16-byte chunks ----
+            const int r = etid >> 1, hsel = etid & 1;
+            for (int kb = pc.kb0; kb < pc.kb1; ++kb) {
+              mbar_wait(&wfull_bar[cstage], cphase);
+              uint8_t* sbase = tiles + static_cast<size_t>(cstage) * stage_bytes;
+              const uint4* raw = reinterpret_cast<const uint4*>(sbase + a_bytes + b_bytes + r * GEMM_BK + hsel * 32);
+              const uint4 c0 = raw[0], c1 = raw[1];
+              const uint32_t w8[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                uint4 o;
+                o.x = e4m3x2_to_f16x2(w8[2 * j]); o.y = e4m3x2_to_f16x2(w8[2 * j] >> 16);
+                o.z = e4m3x2_to_f16x2(w8[2 * j + 1]); o.w = e4m3x2_to_f16x2(w8[2 * j + 1] >> 16);
+                *reinterpret_cast<uint4*>(sbase + r * 128 + (((hsel * 4 + j) ^ (r & 7)) << 4)) = o;
+              }
+              fence_proxy_async();
+              __syncwarp();
+              if (lane == 0) mbar_arrive_leader_release(&conv_bar[cstage]);
+              if (++cstage == a.stages) { cstage = 0; cphase ^= 1; }
+            }
+          }
           const bool contributor = pc.kind == PK_CONTRIB;
           const int my_slot = pc.slot * 2 + crank;
           int n_contrib = 0, c_first = 0;
@@ -502,6 +561,28 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           // partial exchange (stream-K): thread-private 64 bytes per 32-token chunk, in the epilogue's register layout
           auto part_ptr = [&](int slot, int c0) {
             return a.partial + (static_cast<size_t>(slot) * (GEMM_MAX_TOK / 32) * 4 + (c0 >> 5) * 4 + quad) * 2048 + lane * 16;
+          };
+          // FP8: per-output-channel scales of this thread's four accumulator rows (TMEM lanes lane/4, +8, +16, +24 of the quadrant)
+          float sc4[4] = {1.f, 1.f, 1.f, 1.f};
+          if (kFp8) {
+            if (P.a_pair) {   // lanes [0,16) = gate rows, [16,32) = up rows of features tile * 64 + quad * 16 + ..
+              const int f = tile * 64 + quad * 16 + (lane >> 2);
+              sc4[0] = f < P.out_features ? __ldg(P.scale[0] + f) : 0.f;     sc4[1] = f + 8 < P.out_features ? __ldg(P.scale[0] + f + 8) : 0.f;
+              sc4[2] = f < P.out_features ? __ldg(P.scale[1] + f) : 0.f;     sc4[3] = f + 8 < P.out_features ? __ldg(P.scale[1] + f + 8) : 0.f;
+            } else {
+              const int fl = f0 + (lane >> 2);
+#pragma unroll
+              for (int j = 0; j < 4; ++j) sc4[j] = (tile_valid && fl + 8 * j < P.out_features) ? __ldg(P.scale[part] + fl + 8 * j) : 0.f;
+            }
+          }
+          auto apply_scale = [&](float* w) {
+            if (kFp8) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g) {
+                w[4 * g] *= sc4[0]; w[4 * g + 1] *= sc4[0]; w[4 * g + 2] *= sc4[1]; w[4 * g + 3] *= sc4[1];
+                w[16 + 4 * g] *= sc4[2]; w[16 + 4 * g + 1] *= sc4[2]; w[16 + 4 * g + 2] *= sc4[3]; w[16 + 4 * g + 3] *= sc4[3];
+              }
+            }
           };
           if (has_mma) mbar_wait(&tmem_full_bar, acc_phase);
           tc_fence_after();
@@ -585,6 +666,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
             auto in_range = [&](int c0) { return c0 < n_pad && c0 < a.T; };
             auto step = [&](int c0, float* cur, float* nxt) {
               tmem_ld_wait();
+              apply_scale(cur);     // (before the fix-up adds and every store: partials and slabs carry scaled sums)
               if (n_contrib > 0) {
                 fix_add(q, cur);
                 for (int c = 1; c < n_contrib; ++c) { uint4 q2[4]; fix_load(c, c0, q2); fix_add(q2, cur); }

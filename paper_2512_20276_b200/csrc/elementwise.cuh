@@ -286,6 +286,16 @@ __global__ void interleave_gate_up_kernel(const uint4* __restrict__ gate, const 
   dst[i] = v;
 }
 
+// The same row order for one-byte elements (af_prepare_gate_up_fp8: E4M3 codes are copied, not converted): 16 codes per thread.
+__global__ void interleave_gate_up_bytes_kernel(const uint4* __restrict__ gate, const uint4* __restrict__ up, uint4* __restrict__ dst,
+                                                int F, int vec_per_row, size_t n_vec) {
+  const size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n_vec) return;
+  const int row = static_cast<int>(i / vec_per_row), c = static_cast<int>(i - static_cast<size_t>(row) * vec_per_row);
+  const int t = row >> 7, q = (row >> 5) & 3, half = (row >> 4) & 1, f = t * 64 + q * 16 + (row & 15);
+  dst[i] = f < F ? (half ? up : gate)[static_cast<size_t>(f) * vec_per_row + c] : make_uint4(0u, 0u, 0u, 0u);
+}
+
 // f1: ArgMax over one logits row per block (Alg. 1 l.5/l.8).  (value, index) pairs are reduced with "greater value, or
 // equal value and lower index, wins", which is associative and commutative, so the result does not depend on the
 // reduction order: the lowest index of the maximum.  NaNs lose every comparison.
