@@ -653,7 +653,7 @@ static int chain_add_rope(ChainBuilder& b, const act_t* qkv_slabs, long long sla
 
 static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   const int n_pad = b.a.n1 + b.a.n2;
-  const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2 + (b.fp8 ? static_cast<int>(CH_RAW_BYTES) : 0);
+  const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2;   // (FP8: the raw tile lands inside the fp16 tile's slot)
   int stages = (GEMM_SMEM_BUDGET - 1024 - GEMM_EPI_WARPS * 2048) / stage_bytes;
   if (stages > GEMM_MAX_STAGES) stages = GEMM_MAX_STAGES;
   if (stages < 2) return fail(AF_ERR_UNSUPPORTED, "chain: a stage does not fit shared memory");

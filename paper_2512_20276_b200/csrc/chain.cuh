@@ -268,7 +268,6 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int w = w0 + 128 * u < n_v ? w0 + 128 * u : w0;
-#pragma unroll
         const int ns = s_pair_slabs[(2 * D + w * 8) / (2 * GEMM_BM)];
 #pragma unroll
         for (int sl = 0; sl < QKV_MAX_SLABS_K; ++sl)
@@ -299,7 +298,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   const int n_pad = a.n1 + a.n2;
   constexpr uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
   const uint32_t b_bytes = static_cast<uint32_t>(n_pad / 2) * GEMM_BK * 2;   // this CTA's half of the activation rows
-  const uint32_t stage_bytes = a_bytes + b_bytes + (kFp8 ? CH_RAW_BYTES : 0u);   // [fp16 weight tile][activation boxes][raw FP8 tile]
+  const uint32_t stage_bytes = a_bytes + b_bytes;   // [fp16 weight tile (FP8: the raw 8 KB tile lands in its upper half)][activation boxes]
   uint8_t* xch = tiles + static_cast<size_t>(a.stages) * stage_bytes;         // 8 x 2 KB epilogue staging
 
   // full_bar: the stage's TMA loads have landed (FP8: the activation boxes only; the raw weight tile lands on this CTA's
@@ -320,7 +319,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   if (warp == GEMM_EPI_WARPS && lane == 0) {
     for (int s = 0; s < a.stages; ++s) {
       mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1);
-      mbar_init(&wfull_bar[s], 1); mbar_init(&conv_bar[s], 2 * GEMM_EPI_WARPS);
+      mbar_init(&wfull_bar[s], 1); mbar_init(&conv_bar[s], GEMM_EPI_WARPS);   // 4 warps of each CTA of the pair
     }
     mbar_init(&tmem_full_bar, 1);
     mbar_init(&tmem_empty_bar, 2 * GEMM_EPI_WARPS);   // the leader waits for both CTAs' drains
@@ -382,7 +381,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         if (kFp8) {   // raw E4M3 tile -> this CTA's own barrier (its epilogue warps widen it); activations -> the leader's
           if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * b_bytes);
           mbar_arrive_expect_tx(&wfull_bar[stage], CH_RAW_BYTES);
-          tma_load_2d(tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes + b_bytes, c.wmap, &wfull_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
+          tma_load_2d(tiles + static_cast<size_t>(stage) * stage_bytes + CH_RAW_BYTES, c.wmap, &wfull_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
         } else {
           if (crank == 0) mbar_arrive_expect_tx(&full_bar[stage], 2 * stage_bytes);
           tma_load_2d_cg2(tiles + static_cast<size_t>(stage) * stage_bytes, c.wmap, &full_bar[stage], c.kb * GEMM_BK, c.row, pol_w);
@@ -459,7 +458,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           tc_fence_after();
           for (int kb = pc.kb0; kb < pc.kb1; ++kb) {
             mbar_wait(&full_bar[stage], phase);
-            if (kFp8) mbar_wait_cluster(&conv_bar[stage], phase);   // both CTAs' weight tiles have been widened to fp16
+            if (kFp8) mbar_wait(&conv_bar[stage], phase);   // both CTAs' weight tiles have been widened to fp16
             tc_fence_after();
             const uint32_t sa = smem_u32(tiles + static_cast<size_t>(stage) * stage_bytes);
             const uint32_t sb = sa + a_bytes;
@@ -501,7 +500,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         for (int i = etid; i < 3 * a.D / (2 * GEMM_BM) && i < 64; i += GEMM_EPI_WARPS * 32) s_pair_slabs[i] = __ldg(a.ph[ph].pair_slabs + i);
     AF_EPI_BAR();
     uint32_t acc_phase = 0, cphase = 0;
-    int n_bar = 0, cstage = 0;
+    int n_bar = 0, cstage = 0, cunit = 0;
 
     for (int ph = 0; ph < a.n_phases; ++ph) {
       const ChainPhase& P = a.ph[ph];
@@ -515,24 +514,39 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           const bool tile_valid = tile < P.n_tiles;
           if (kFp8) {
             // ---- widen this piece's raw E4M3 weight tiles to the fp16 UMMA tile (K-major, 128-byte swizzle), stage by stage
-            //      as they land: thread (row r, half h) rewrites codes [32h, 32h + 32) of row r as four 16-byte chunks ----
-            const int r = etid >> 1, hsel = etid & 1;
+            //      as they land.  The two groups of 4 warps take alternate stages (two conversions in flight). ----
+            const int cg = warp >> 2, ct = (warp & 3) * 32 + lane;   // thread 0..127 of its group
             for (int kb = pc.kb0; kb < pc.kb1; ++kb) {
-              mbar_wait(&wfull_bar[cstage], cphase);
-              uint8_t* sbase = tiles + static_cast<size_t>(cstage) * stage_bytes;
-              const uint4* raw = reinterpret_cast<const uint4*>(sbase + a_bytes + b_bytes + r * GEMM_BK + hsel * 32);
-              const uint4 c0 = raw[0], c1 = raw[1];
-              const uint32_t w8[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+              if ((cunit & 1) == cg) {
+                mbar_wait(&wfull_bar[cstage], cphase);
+                uint8_t* sbase = tiles + static_cast<size_t>(cstage) * stage_bytes;
+                const uint4* raw = reinterpret_cast<const uint4*>(sbase + CH_RAW_BYTES);   // upper half of the 16 KB fp16 tile
+                // 16-byte chunk id = i * 128 + ct (a warp reads 512 contiguous bytes: no bank conflicts) = 16 codes of row
+                // id / 4, which become fp16 chunks 2 (id % 4) and 2 (id % 4) + 1 of that row in the swizzled tile
+                uint4 c4[4];
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                uint4 o;
-                o.x = e4m3x2_to_f16x2(w8[2 * j]); o.y = e4m3x2_to_f16x2(w8[2 * j] >> 16);
-                o.z = e4m3x2_to_f16x2(w8[2 * j + 1]); o.w = e4m3x2_to_f16x2(w8[2 * j + 1] >> 16);
-                *reinterpret_cast<uint4*>(sbase + r * 128 + (((hsel * 4 + j) ^ (r & 7)) << 4)) = o;
+                for (int i = 0; i < 4; ++i) c4[i] = raw[i * 128 + ct];
+                AF_ROWGRP_BAR(cg);   // in-place expansion: every raw chunk is in registers before the first fp16 chunk is written
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  const int id = i * 128 + ct, r = id >> 2, cc = (id & 3) * 2;
+                  uint4 o0, o1;
+                  o0.x = e4m3x2_to_f16x2(c4[i].x); o0.y = e4m3x2_to_f16x2(c4[i].x >> 16);
+                  o0.z = e4m3x2_to_f16x2(c4[i].y); o0.w = e4m3x2_to_f16x2(c4[i].y >> 16);
+                  o1.x = e4m3x2_to_f16x2(c4[i].z); o1.y = e4m3x2_to_f16x2(c4[i].z >> 16);
+                  o1.z = e4m3x2_to_f16x2(c4[i].w); o1.w = e4m3x2_to_f16x2(c4[i].w >> 16);
+                  *reinterpret_cast<uint4*>(sbase + r * 128 + ((cc ^ (r & 7)) << 4)) = o0;
+                  *reinterpret_cast<uint4*>(sbase + r * 128 + (((cc + 1) ^ (r & 7)) << 4)) = o1;
+                }
+                // Generic-proxy writes -> the tensor core's (async-proxy) reads, possibly issued from the peer CTA: the proxy
+                // fence completes this thread's shared-memory writes towards the async proxy before the arrive is issued; the
+                // arrive itself is relaxed (a cluster-scope release costs ~1000 cycles per stage here - measured: 2x the
+                // whole step), the leader's wait acquires at cluster scope.
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_leader(&conv_bar[cstage]);
               }
-              fence_proxy_async();
-              __syncwarp();
-              if (lane == 0) mbar_arrive_leader_release(&conv_bar[cstage]);
+              ++cunit;
               if (++cstage == a.stages) { cstage = 0; cphase ^= 1; }
             }
           }
