@@ -22,10 +22,21 @@
  *     weights are [out_features, in_features] row-major (y = x W^T).  The KV ring holds fp16 (same bytes as bf16, 3 more
  *     mantissa bits: DESIGN.md "Precision"); all accumulation and the residual stream are fp32.
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t cast to void*) and return without host synchronisation
- *     (the af_debug_* and af_ring_read_* calls synchronise; they are test/bench helpers, not the hot path).
+ *     (the af_debug_* calls of af_debug.h synchronise; they are test/bench helpers, not the hot path).
+ *   - Devices and streams.  The library keeps nothing process-global that kernels synchronise through: its schedule
+ *     tables are per device, its stream-K flags and the layer-chain kernel's grid barrier per (device, stream).  Its
+ *     persistent kernels wait inside themselves (stream-K owners for contributors of their own launch, the chain for its
+ *     own grid barrier), so they need their whole grid resident: grids are sized with the occupancy API for the current
+ *     device, and a step enqueued on one stream is ordered (cudaStreamWaitEvent) behind the library work last enqueued on
+ *     another stream of the same device - two rings driven from two streams are correct, but never overlap.  Other
+ *     work of the caller that occupies SMs while a step runs only delays it (a stream-K owner waits for CTAs dispatched
+ *     before it, never after); it must not itself wait for the step.
+ *   - fp16 range.  Values stored as fp16 (q, k, v, attention output, the SwiGLU product, the partial sums exchanged
+ *     between CTAs) are converted with saturation: a finite value beyond +-65504 becomes +-65504, never inf.
  *   - Return value: 0 on success, a negative AF_ERR_* otherwise.  On any error raised by argument validation
  *     no kernel has been launched and the ring bookkeeping is unchanged.  af_last_error() gives a message.
- *   - One af_ring is not thread-safe; the caller serialises calls on it.
+ *   - One af_ring is not thread-safe; the caller serialises calls on it (different rings may be driven from different
+ *     host threads and streams).
  *   - There is no CPU fallback anywhere in this library.
  *
  * Ring geometry (reading A6).  One allocation `kv_mem` holds, for every layer, all R = n_regions
@@ -220,42 +231,8 @@ int af_loop_destroy(af_loop* loop);
 
 int af_ring_destroy(af_ring* ring); /* frees the handle and its own metadata; never frees caller memory */
 
-/* ---- introspection for bit-exact bookkeeping parity; these synchronise, they are not hot path ---- */
-int af_ring_get_state(const af_ring* ring, int32_t req_id, int32_t* base, int32_t* len);
-/* Row map of the LAST af_packed_forward, copied back from the DEVICE tables the kernels used.
- * Each output is a HOST int32 [n] array (n <= T of that step) or NULL. */
-int af_debug_row_map(const af_ring* ring, int32_t* row_req, int32_t* row_pos, int32_t* row_slot, int32_t n);
-/* Bench/test only: rewind (or set) the bookkeeping length of a region; moves no data. */
-int af_debug_set_len(af_ring* ring, int32_t req_id, int32_t len);
-/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
-int64_t af_debug_launch_count(void);
-/* Plain C = A B^T through the same tcgen05 GEMM kernel the forward uses (unit tests / roofline probes).
- * a: device fp16 [n_tok, k] (activations), w: device bf16 [n_out, k]; out: device fp32 [n_tok, n_out], n_out % 4 == 0. */
-int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32_t n_out, int32_t k,
-                  void* workspace, size_t ws_bytes, void* cuda_stream);
-
-/* Per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline leg; adds event records
- * between kernels, so it is switched on only for a separate profiling pass).  Classes, in order: gemm_qkv, gemm_o,
- * gemm_gateup, gemm_down, gemm_lm, attention, rope_append, rmsnorm, silu_mul, other (10 slots).
- * af_debug_profile_read synchronises, returns summed milliseconds and launch counts since the last read, and clears. */
-int af_debug_profile(int enable);
-int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
-
-/* The work lists of the GEMM kernel (pure host logic, needs no GPU): for `n_tile_pairs` pairs of 128-row weight tiles and
- * `n_kblocks` 64-wide k-blocks on at most `max_clusters` 2-CTA clusters, either split-K (split_k != 0: `splits` slabs per
- * tile pair) or stream-K ranges.  pieces = HOST int32 [max_clusters_out][16][8]; piece = {pair, kb0, kb1, kind (0 plain,
- * 1 contributor, 2 owner), slot, n_contrib, slab, 0}, a cluster's list ends at pair = -1.  Returns the number of
- * clusters used, or a negative AF_ERR_*. */
-int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters, int32_t splits,
-                           int32_t* pieces, int32_t max_clusters_out);
-
-/* Debug timeline of the GEMM kernel: while enabled every gemm_tcgen05_kernel launch records %globaltimer / clock stamps
- * per CTA (kernel start, PDL wait, per piece: accumulator ready / fix-up loaded / drained, producer and MMA-thread
- * counters) into a library-owned device buffer that keeps the last 16 launches.  af_debug_trace_read synchronises and
- * copies them out: stamps = HOST int64 [16][160][32], meta = HOST int32 [16][2] (kernel class as in af_debug_profile,
- * grid size); returns the number of launches recorded since af_debug_trace(1), or a negative AF_ERR_*. */
-int af_debug_trace(int enable);
-int af_debug_trace_read(long long* stamps, int* meta);
+/* Introspection (row map, bookkeeping), per-kernel timing, the GEMM work lists and the chain kernel's timeline are test /
+ * bench helpers, not the product path: they are declared in include/af_debug.h (same library). */
 
 const char* af_last_error(void); /* thread-local message of the last failing call */
 

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "af_lib.cu")
 OUT = os.path.join(HERE, "libaf_b200.so")
 DEPS = [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))] + \
-       [os.path.join(os.path.dirname(HERE), "include", "af.h")]
+       [os.path.join(os.path.dirname(HERE), "include", "af.h"), os.path.join(os.path.dirname(HERE), "include", "af_debug.h")]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -12,7 +12,7 @@
 #include <tuple>
 #include <vector>
 
-#include "../../include/af.h"
+#include "../../include/af_debug.h"
 
 namespace af { constexpr int AF_MAX_SEGS_K = AF_MAX_SEGS; }
 #include "gemm_tcgen05.cuh"
@@ -907,7 +907,7 @@ extern "C" int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int
   if (!pieces) return fail(AF_ERR_ARG, "null output");
   std::vector<GemmPiece> flat;
   int n_cl = 0;
-  const int rc = make_schedule(split_k ? SPLIT_K : SPLIT_STREAMK, n_tile_pairs, n_kblocks, max_clusters, splits, &flat, &n_cl);
+  const int rc = make_schedule(split_k == 2 ? SPLIT_SLABS : (split_k ? SPLIT_K : SPLIT_STREAMK), n_tile_pairs, n_kblocks, max_clusters, splits, &flat, &n_cl);
   if (rc) return rc;
   if (n_cl > max_clusters_out) return fail(AF_ERR_ARG, "%d clusters do not fit the output (%d)", n_cl, max_clusters_out);
   memcpy(pieces, flat.data(), flat.size() * sizeof(GemmPiece));
@@ -1030,10 +1030,22 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   };
   // ---- the layer chain (chain.cuh): per layer ONE persistent launch for every projection and row stage + attention ----
   const bool fp8 = w->weight_format == AF_WEIGHTS_FP8;
+  // every work list of the chain is built (and cached) BEFORE the first launch: a shape it cannot schedule falls back to the
+  // per-stage path (FP8: AF_ERR_UNSUPPORTED) with nothing enqueued
+  auto chain_schedulable = [&]() {
+    const int kd = (D + GEMM_BK - 1) / GEMM_BK, kf = (F + GEMM_BK - 1) / GEMM_BK;
+    const int d_pairs = ((D + GEMM_BM - 1) / GEMM_BM + 1) / 2, gu_pairs = ((F + 63) / 64 + 1) / 2;
+    Sched sc;
+    return build_schedule(ctx, SPLIT_SLABS, (3 * ((D + GEMM_BM - 1) / GEMM_BM) + 1) / 2, kd, ctx->max_clusters, QKV_MAX_SLABS, &sc) == AF_OK &&
+           build_schedule(ctx, SPLIT_K, d_pairs, kd, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, D), &sc) == AF_OK &&
+           build_schedule(ctx, SPLIT_K, d_pairs, kf, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, F), &sc) == AF_OK &&
+           build_schedule(ctx, SPLIT_STREAMK, gu_pairs, kd, ctx->max_clusters, 1, &sc) == AF_OK;
+  };
   if (fp8 && (T > GEMM_MAX_TOK || D > 4096 || D % 256 != 0 || F < 128 || ctx->max_clusters < 2 || g_prof_stages))
     return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8 runs on the layer chain only: T <= %d packed rows, d_model <= 4096 and a multiple of 256", GEMM_MAX_TOK);
+  if (fp8 && !chain_schedulable()) return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8: this shape has no layer-chain schedule on this device");
   const bool use_chain = (w->weight_format == AF_WEIGHTS_FP16_GU || fp8) && T <= GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
-                         ctx->max_clusters >= 2 && !g_prof_stages;
+                         ctx->max_clusters >= 2 && !g_prof_stages && chain_schedulable();
   if (use_chain) {
     StreamCtx sctx;
     if ((rc = get_stream_ctx(ctx, st, &sctx))) return rc;

@@ -8,10 +8,17 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared_functions():
-    src = open(os.path.join(ROOT, "include", "af.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"\b(af_[a-z0-9_]+)\s*\(", src)
+    names = []
+    for hdr in ("af.h", "af_debug.h"):          # the C ABI proper + the test / bench helpers of the same library
+        src = open(os.path.join(ROOT, "include", hdr)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names += re.findall(r"\b(af_[a-z0-9_]+)\s*\(", src)
     return sorted(set(names))
+
+
+def test_debug_helpers_live_in_their_own_header():
+    src = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "af.h")).read(), flags=re.S)
+    assert "af_debug_" not in src
 
 
 def test_header_declares_the_north_star_calls():

@@ -112,3 +112,47 @@ def test_splitk_schedules(n_pairs, nkb, splits):
         assert (p["pair"], p["mid"]) not in slabs
         slabs.add((p["pair"], p["mid"]))
     assert (cover == 1).all() and len(slabs) == n_pairs * splits
+
+
+def check_slabs(n_pairs, nkb, max_cl, splits):
+    """Layer-chain slab ranges (split_k = 2): every (tile pair, k-block) exactly once, every piece plain, a pair's pieces
+    carry slab ordinals 0, 1, 2, .. in k order (the row stage adds them in that order), never more than `splits`."""
+    try:
+        cl = schedule(2, n_pairs, nkb, max_cl, splits)
+    except AssertionError as e:
+        # a range that touches more than 15 tile pairs does not fit a cluster's piece list: refused (AF_ERR_UNSUPPORTED),
+        # never truncated - only possible when the device exposes very few clusters
+        assert "pieces in one cluster" in str(e) and -(-n_pairs * nkb // max_cl) > 13 * nkb
+        return None, None
+    assert 1 <= len(cl) <= max(max_cl, 1)
+    cover = np.zeros((n_pairs, nkb), dtype=np.int32)
+    by_pair = {}
+    for pieces in cl:
+        assert pieces
+        for p in pieces:
+            assert p["kind"] == PLAIN and 0 <= p["kb0"] < p["kb1"] <= nkb
+            cover[p["pair"], p["kb0"]:p["kb1"]] += 1
+            by_pair.setdefault(p["pair"], []).append(p)
+    assert (cover == 1).all()
+    for pair, ps in by_pair.items():
+        ps.sort(key=lambda q: q["kb0"])
+        assert [q["mid"] for q in ps] == list(range(len(ps))) and len(ps) <= splits
+    units = [sum(p["kb1"] - p["kb0"] for p in pieces) for pieces in cl]
+    return cl, units
+
+
+@pytest.mark.parametrize("n_pairs,nkb,max_cl,splits", [
+    (48, 64, 74, 4),     # QKV at 7B: 74 ranges of 42 units, at most 3 slabs per pair
+    (2, 4, 74, 4), (6, 4, 74, 4), (1, 1, 74, 4), (16, 64, 74, 4), (16, 172, 74, 4), (48, 64, 8, 4), (5, 7, 3, 2), (9, 5, 74, 1),
+])
+def test_slab_schedules(n_pairs, nkb, max_cl, splits):
+    cl, units = check_slabs(n_pairs, nkb, max_cl, splits)
+    assert cl is not None
+    if (n_pairs, nkb, max_cl) == (48, 64, 74):
+        assert len(cl) == 74 and max(units) == 42 and max(len(p) for p in cl) == 2
+
+
+@settings(max_examples=60, deadline=None)
+@given(st.integers(1, 60), st.integers(1, 40), st.integers(1, 80), st.integers(1, 4))
+def test_slab_schedules_random_shapes(n_pairs, nkb, max_cl, splits):
+    check_slabs(n_pairs, nkb, max_cl, splits)
