@@ -26,7 +26,7 @@ from paper_2512_20276_b200.measure import (ClockSampler, L_P, K_STAGES, R_REGION
 
 # DRAM bytes per layer_chain_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum of the 7-phase launches of a steady
 # step, ncu, cold caches): profiles/launches_r2.md.  Algorithmic weight bytes per launch: 404.8 MB (one layer).
-CHAIN_TRAFFIC_BYTES_PER_LAUNCH = None
+CHAIN_TRAFFIC_BYTES_PER_LAUNCH = 426.8e6
 WORKLOAD = "cfg3: 32-layer Llama-2-7B shape, steady pipelined step = 276-row prefill + 6 decodes (ctx 277..282) + LM head on 7 rows"
 
 
