@@ -9,13 +9,13 @@
 
 namespace af {
 
-constexpr int ATT_BQ = 64;
+constexpr int ATT_BQ = 32;       // query rows per work item: two 16-row strips, each taken by TWO warps on alternate KV tiles
 constexpr int ATT_BKV = 32;
 #ifndef AF_ATT_STAGES
 #define AF_ATT_STAGES 3
 #endif
 constexpr int ATT_STAGES = AF_ATT_STAGES;   // K/V tiles in flight (cp.async groups)
-constexpr int att_smem_bytes(int hd) { return (ATT_BQ + 2 * ATT_STAGES * ATT_BKV) * hd * 2; }
+__host__ __device__ constexpr int att_smem_bytes(int hd) { return (ATT_BQ + 2 * ATT_STAGES * ATT_BKV) * hd * 2; }
 constexpr int ATT_THREADS = 128;
 
 struct StepTables {      // device arrays written by rowmap_kernel (elementwise.cuh), one set per ring
@@ -61,6 +61,13 @@ __device__ __forceinline__ uint32_t sw_off(int row, int chunk) {
   return static_cast<uint32_t>(row * (HD * 2) + ((chunk ^ (row & 7)) << 4));
 }
 
+// A segment of ONE row (every decode row of the paper's schedule) is not MMA-shaped: on the m16n8k16 path it fills 1 of 16
+// accumulator rows and one of the CTA's four warps walks its 8-9 KV tiles alone (the legacy HMMA pipe issues one m16n8k16
+// per ~13 cycles per scheduler, so these rows cost 40 % of the kernel's tensor time for 0.1 % of its FLOPs).  Such a
+// (segment, head) unit keeps the kernel's cp.async K/V tile pipeline but computes each tile on plain FMAs with all 128
+// threads: QK with 4 threads per position (HD / 4 dims each, q in registers) and a 2-step shuffle, the 32 scores of the
+// tile through shared memory, then an online-softmax update in which thread t owns output columns [t * HD / 128, ..).
+// Tiles are walked in LOGICAL position order (result independent of base_r), every reduction order is fixed.
 // WIN (f3): rows see only the last `window` positions, max(0, p - window + 1)..p; positions may exceed C, slot
 // (base + j) mod C then holds the newest position congruent to j (af.h: af_ring_set_window).  WIN = false is the v1 kernel.
 template <int HD, bool WIN = false>
@@ -95,6 +102,9 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   const act_t* kbase = kv + (static_cast<size_t>(0 * R + req) * H + h) * head_stride;
   const act_t* vbase = kv + (static_cast<size_t>(1 * R + req) * H + h) * head_stride;
 
+  const bool fma_row = !WIN && len == 1;   // a one-row segment: the FMA tile path below (block-uniform)
+  __shared__ float s_scores[ATT_BKV];
+
   // ---- async loads: Q tile, then KV tile 0 ----
   for (int i = tid; i < ATT_BQ * CH; i += ATT_THREADS) {
     const int r = i / CH, c = i % CH;
@@ -128,9 +138,12 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
   uint32_t qf[HD / 16][4];
 
-  const bool warp_active = warp * 16 < nq;
-  const int p_lo = start + q0 + warp * 16 + g;   // position of this thread's first row (second = +8)
-  const int warp_pmin = start + q0 + warp * 16, warp_pmax = warp_pmin + 15;
+  // warp -> (16-row strip, KV part): the two warps of a strip take alternate KV tiles and their partial (max, sum, O) are
+  // merged at the end in part order - a strip's serial chain is half as long as with one warp per strip
+  const int strip = warp & 1, part = warp >> 1;
+  const bool warp_active = strip * 16 < nq;
+  const int p_lo = start + q0 + strip * 16 + g;   // position of this thread's first row (second = +8)
+  const int warp_pmin = start + q0 + strip * 16, warp_pmax = warp_pmin + 15;
 
   for (int tile = tile_lo; tile < n_tiles; ++tile) {
     const int stage = (tile - tile_lo) % ATT_STAGES;
@@ -142,13 +155,61 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
     if (tile == tile_lo) {
 #pragma unroll
       for (int kk = 0; kk < HD / 16; ++kk) {
-        const int r = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const int r = strip * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
         const int c = kk * 2 + (lane >> 4);
         ldsm_x4(smem_u32(sQ + sw_off<HD>(r, c)), qf[kk][0], qf[kk][1], qf[kk][2], qf[kk][3]);
       }
     }
     const int j0 = tile * ATT_BKV;
-    if (warp_active && j0 <= warp_pmax && (!WIN || j0 + ATT_BKV - 1 > warp_pmin - W)) {
+    if (fma_row) {
+      // ---- one query row on FMAs: thread (jj = tid / 4, part = tid % 4) scores position j0 + jj over HD / 4 dims ----
+      const uint8_t* cK = sK + stage * TILE_BYTES;
+      const uint8_t* cV = sV + stage * TILE_BYTES;
+      constexpr int CPT = CH / 4;                       // 16-byte chunks of a K row per thread
+      const int jj = tid >> 2, prt = tid & 3;
+      if (tile == tile_lo) {                            // q (row 0 of the Q tile) -> registers, this thread's HD / 4 dims
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) {
+          const uint4 v = *reinterpret_cast<const uint4*>(sQ + sw_off<HD>(0, prt * CPT + c));
+          qf[c][0] = v.x; qf[c][1] = v.y; qf[c][2] = v.z; qf[c][3] = v.w;
+        }
+      }
+      float sdot = 0.f;
+#pragma unroll
+      for (int c = 0; c < CPT; ++c) {
+        const uint4 kk = *reinterpret_cast<const uint4*>(cK + sw_off<HD>(jj, prt * CPT + c));
+        const uint32_t b4[4] = {kk.x, kk.y, kk.z, kk.w};
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+          const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&qf[c][m]));
+          const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&b4[m]));
+          sdot = fmaf(a.x, b.x, sdot); sdot = fmaf(a.y, b.y, sdot);
+        }
+      }
+      sdot += __shfl_xor_sync(0xffffffffu, sdot, 1);
+      sdot += __shfl_xor_sync(0xffffffffu, sdot, 2);
+      if (prt == 0) s_scores[jj] = (j0 + jj < kv_end) ? sdot * scale_log2 : -INFINITY;
+      __syncthreads();
+      // online softmax: every thread scans the tile's 32 scores (broadcast reads) and updates its own output column(s)
+      float mt = -INFINITY;
+#pragma unroll
+      for (int j = 0; j < ATT_BKV; ++j) mt = fmaxf(mt, s_scores[j]);
+      const float m_new = fmaxf(m_run[0], mt);          // finite: position j0 <= own position is always visible
+      const float alpha = exp2f(m_run[0] - m_new);
+      m_run[0] = m_new;
+      float rs = 0.f, a0 = o_acc[0][0] * alpha, a1 = o_acc[0][1] * alpha;
+      const int col = (2 * tid) % HD;                   // this thread's two output columns (HD = 64: the upper half of the CTA repeats them)
+#pragma unroll
+      for (int j = 0; j < ATT_BKV; ++j) {
+        const float pj = exp2f(s_scores[j] - m_new);
+        rs += pj;
+        const float2 vv = __half22float2(*reinterpret_cast<const __half2*>(cV + sw_off<HD>(j, col >> 3) + (col & 7) * 2));
+        a0 = fmaf(pj, vv.x, a0); a1 = fmaf(pj, vv.y, a1);
+      }
+      l_run[0] = l_run[0] * alpha + rs;
+      o_acc[0][0] = a0; o_acc[0][1] = a1;
+    } else
+    if (warp_active && ((tile - tile_lo) & 1) == part && j0 <= warp_pmax && (!WIN || j0 + ATT_BKV - 1 > warp_pmin - W)) {
       const uint8_t* cK = sK + stage * TILE_BYTES;
       const uint8_t* cV = sV + stage * TILE_BYTES;
       float s[ATT_BKV / 8][4];
@@ -243,23 +304,48 @@ attention_kernel(const act_t* __restrict__ q,     // [T, H*HD] rotated queries
   }
   cp_async_wait<0>();
 
-  if (warp_active) {
-#pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 1);
-      l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 2);
+  if (fma_row) {
+    if (2 * tid < HD) {
+      const float inv = 1.f / l_run[0];
+      *reinterpret_cast<uint32_t*>(out + static_cast<size_t>(row0) * (H * HD) + h * HD + 2 * tid) = pack_act(o_acc[0][0] * inv, o_acc[0][1] * inv);
     }
+    return;
+  }
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 1);
+    l_run[r] += __shfl_xor_sync(0xffffffffu, l_run[r], 2);
+  }
+  // ---- merge the two KV parts of every strip through the (now idle) K/V stages: part 1 publishes, part 0 combines ----
+  float* mo = reinterpret_cast<float*>(sK) + static_cast<size_t>(strip) * (16 * HD + 32);   // O [16][HD], then m[16], l[16]
+  if (part == 1 && warp_active) {
+#pragma unroll
+    for (int db = 0; db < HD / 8; ++db) {
+      *reinterpret_cast<float2*>(mo + g * HD + db * 8 + 2 * t) = make_float2(o_acc[db][0], o_acc[db][1]);
+      *reinterpret_cast<float2*>(mo + (g + 8) * HD + db * 8 + 2 * t) = make_float2(o_acc[db][2], o_acc[db][3]);
+    }
+    if (t == 0) {
+      mo[16 * HD + g] = m_run[0]; mo[16 * HD + g + 8] = m_run[1];
+      mo[16 * HD + 16 + g] = l_run[0]; mo[16 * HD + 24 + g] = l_run[1];
+    }
+  }
+  __syncthreads();
+  if (part == 0 && warp_active) {
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
-      const int qi = warp * 16 + g + r * 8;
-      if (qi < nq) {
-        const float inv = 1.f / l_run[r];
-        act_t* dst = out + static_cast<size_t>(row0 + q0 + qi) * (H * HD) + h * HD;
+      const float m_o = mo[16 * HD + g + 8 * r], l_o = mo[16 * HD + 16 + g + 8 * r];
+      const float m_new = fmaxf(m_run[r], m_o);
+      const float a_s = (m_new == -INFINITY) ? 1.f : exp2f(m_run[r] - m_new);
+      const float a_o = (m_new == -INFINITY) ? 0.f : exp2f(m_o - m_new);
+      l_run[r] = l_run[r] * a_s + l_o * a_o;
+      const int qi = strip * 16 + g + r * 8;
+      const float inv = 1.f / l_run[r];
+      act_t* dst = out + static_cast<size_t>(row0 + q0 + (qi < nq ? qi : 0)) * (H * HD) + h * HD;
 #pragma unroll
-        for (int db = 0; db < HD / 8; ++db) {
-          *reinterpret_cast<uint32_t*>(dst + db * 8 + 2 * t) =
-              pack_act(o_acc[db][2 * r] * inv, o_acc[db][2 * r + 1] * inv);
-        }
+      for (int db = 0; db < HD / 8; ++db) {
+        const float2 ov = *reinterpret_cast<const float2*>(mo + (g + 8 * r) * HD + db * 8 + 2 * t);
+        const float x0 = (o_acc[db][2 * r] * a_s + ov.x * a_o) * inv, x1 = (o_acc[db][2 * r + 1] * a_s + ov.y * a_o) * inv;
+        if (qi < nq) *reinterpret_cast<uint32_t*>(dst + db * 8 + 2 * t) = pack_act(x0, x1);
       }
     }
   }
