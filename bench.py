@@ -235,6 +235,36 @@ def main():
         step(e_dev[tau[0] % n_buf])
     prof = binding.profile_read()
     binding.profile(False)
+    # ---- one more step with the chain kernel's per-phase stamps on: where a whole-layer launch spends its time ----
+    chain_phases = None
+    if rank == 0:
+        binding.chain_trace(True)
+        step(e_dev[tau[0] % n_buf])
+        torch.cuda.synchronize()
+        st_, meta_, n_tr = binding.chain_trace_read()
+        binding.chain_trace(False)
+        full = [i for i in range(min(n_tr, 16)) if int(meta_[i][0]) == 7]       # whole-layer launches among the last 16
+        if full:
+            import numpy as np
+            names = ["o_proj", "rows_mlp_norm", "gate_up_swiglu", "down_proj", "rows_attn_norm", "qkv_proj", "rope_append"]
+            acc = np.zeros(7)
+            for i in full:
+                g_ = int(meta_[i][1])
+                s_ = st_[i, :g_].astype(np.float64)
+                t0_, prev_ = s_[:, 0].min(), 0.0
+                for ph in range(7):
+                    end_ = (s_[:, 2 + 2 * ph].max() if ph < 6 else s_[:, 1 + 2 * ph].max()) - t0_
+                    acc[ph] += (end_ - prev_) / 1e3
+                    prev_ = end_
+            acc /= len(full)
+            proj_us = float(acc[0] + acc[2] + acc[3] + acc[5])
+            layer_flops = 2.0 * T * (4 * cfg.d_model ** 2 + 3 * cfg.d_model * cfg.ffn)
+            chain_phases = {"what": "layer_chain_kernel, whole-layer launches of one step in this run (af_debug_trace, %globaltimer; "
+                                    "a phase runs from the previous grid barrier's release to its own, max over the 148 CTAs)",
+                            "launches": len(full), "us": {n_: float(v_) for n_, v_ in zip(names, acc)},
+                            "launch_us": float(acc.sum()), "projection_phases_us": proj_us,
+                            "projection_phases_tflops": layer_flops / proj_us / 1e6,
+                            "projection_phases_weight_gbs": 2.0 * (4 * cfg.d_model ** 2 + 3 * cfg.d_model * cfg.ffn) / proj_us / 1e3}
     # ---- extra leg: the same steady step with AF_WEIGHTS_FP8 (E4M3 codes + per-output-channel scales,
     #      half the weight bytes in HBM); the headline stays the 16-bit line ----
     ms_fp8 = None
@@ -302,6 +332,7 @@ def main():
                      "share_of_step": gemm_ms / all_ms,
                      "weight_stream_gbs": work["weight_bytes"] / (gemm_ms / 1e3) / 1e9},
         "kernel_ms_per_step": {k: v[0] / n_prof for k, v in prof.items()},
+        "chain_phases": chain_phases,
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": T * cfg.d_model * 2,
                 "d2h_bytes_per_step": K_STAGES * cfg.vocab * 4},
         "e2e_device_loop": {"value": replicas.whole_job_throughput(args.steps, ms_loop), "unit": "frames/s",

@@ -326,6 +326,25 @@ def profile_read() -> dict:
     return {k: (ms[i], cnt[i]) for i, k in enumerate(PROFILE_CLASSES)}
 
 
+def chain_trace(enable: bool):
+    """af_debug_trace: switch the layer-chain kernel's per-phase %globaltimer stamps on / off (synchronises)."""
+    L = load_library()
+    L.af_debug_trace.argtypes, L.af_debug_trace.restype = [C.c_int], C.c_int
+    _check(L.af_debug_trace(1 if enable else 0))
+
+
+def chain_trace_read():
+    """(stamps int64 [16][160][18], meta int32 [16][2] = (phases, grid), launches recorded) of the last 16 chain launches."""
+    import numpy as np
+    L = load_library()
+    L.af_debug_trace_read.argtypes, L.af_debug_trace_read.restype = [C.c_void_p, C.c_void_p], C.c_int
+    st, meta = np.zeros((16, 160, 18), dtype=np.int64), np.zeros((16, 2), dtype=np.int32)
+    n = L.af_debug_trace_read(st.ctypes.data, meta.ctypes.data)
+    if n < 0:
+        _check(n)
+    return st, meta, n
+
+
 def argmax_rows(logits: torch.Tensor) -> torch.Tensor:
     """af_argmax_rows: int32 [n] = lowest index of the maximum of every row of fp32 logits [n, V] (device)."""
     assert logits.is_cuda and logits.dtype == torch.float32 and logits.dim() == 2 and logits.is_contiguous()
