@@ -557,8 +557,8 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
             c_first = pc.slot; n_contrib = pc.n_contrib;
             if (etid < n_contrib) {
               volatile int* f = a.flags + (c_first + etid) * 2 + crank;
-              while (*f == 0) {
-              }
+              SpinGuard sg;
+              while (*f == 0) sg.poll();
               *f = 0;   // one consumer per flag: ready for the next use (graph-replay safe)
               __threadfence();
             }
@@ -727,8 +727,8 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         if (etid == 0) {
           bar_target += static_cast<unsigned>(n_cta);
           red_release_gpu_add(a.bar, 1ull);       // (release: cumulative over what the CTA's threads wrote before bar.sync)
-          while (ld_acquire_gpu(a.bar) < bar_target) {
-          }
+          SpinGuard sg;
+          while (ld_acquire_gpu(a.bar) < bar_target) sg.poll();
           fence_proxy_async_all();
           st_release_cta_shared(&deps_done, ++n_bar);
           if (trace) trace[2 + 2 * ph] = static_cast<long long>(globaltimer_ns());

@@ -288,8 +288,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap map_w0, const __grid_con
         c_first = pc.slot; n_contrib = pc.n_contrib;
         if (etid < n_contrib) {
           volatile int* f = p.flags + (c_first + etid) * p.cluster + crank;
-          while (*f == 0) {
-          }
+          SpinGuard sg;
+          while (*f == 0) sg.poll();
           *f = 0;  // one consumer per flag: ready for the next launch (graph-replay safe)
           __threadfence();
         }

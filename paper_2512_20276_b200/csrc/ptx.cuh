@@ -279,6 +279,22 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   return t;
 }
 
+// Waits on another CTA of the same grid (stream-K flags, the layer chain's grid barrier) are bounded: if the awaited CTA can
+// never run (the grid is not co-resident after all - MPS / green-context limits below what the occupancy query saw, a
+// debugger, a preempted context) the kernel traps after ~4 s and the stream reports a launch failure instead of hanging
+// the GPU.  Checked once per 4096 polls, so the hot path pays nothing.
+struct SpinGuard {
+  unsigned long long t0 = 0;
+  unsigned polls = 0;
+  __device__ __forceinline__ void poll() {
+    if ((++polls & 4095u) == 0) {
+      const unsigned long long now = globaltimer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 4000000000ull) asm volatile("trap;\n");
+    }
+  }
+};
+
 // Programmatic dependent launch
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
