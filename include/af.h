@@ -30,7 +30,9 @@
  *     device, and a step enqueued on one stream is ordered (cudaStreamWaitEvent) behind the library work last enqueued on
  *     another stream of the same device - two rings driven from two streams are correct, but never overlap.  Other
  *     work of the caller that occupies SMs while a step runs only delays it (a stream-K owner waits for CTAs dispatched
- *     before it, never after); it must not itself wait for the step.
+ *     before it, never after); it must not itself wait for the step.  Every such wait is bounded: a CTA that waits ~4 s
+ *     for another CTA of its grid traps, and the stream reports a launch failure (AF_ERR_CUDA on the next call) instead
+ *     of hanging the device.
  *   - fp16 range.  Values stored as fp16 (q, k, v, attention output, the SwiGLU product, the partial sums exchanged
  *     between CTAs) are converted with saturation: a finite value beyond +-65504 becomes +-65504, never inf.
  *   - Return value: 0 on success, a negative AF_ERR_* otherwise.  On any error raised by argument validation

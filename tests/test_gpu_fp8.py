@@ -87,6 +87,29 @@ def test_fp8_cfg3_pipeline_steps(binding):
     print(f"fp8 cfg3: worst hidden {worst:.3e}, logits {relmax(lg, ref_lg):.3e}")
 
 
+def test_fp8_single_7b_layer_is_deterministic(binding):
+    """The widened weight tiles are handed from the epilogue warps (generic proxy) to the tensor core (async proxy) of the
+    pair's leader: a hand-over that let an MMA read a tile too early would show up as run-to-run differences.  Twelve
+    repetitions of the cfg2 step are bit-identical."""
+    cfg = I.CFG_7B_1L
+    qw = I.quantize_weights_fp8(I.make_weights(cfg, seed=1, threads=16))
+    W = binding.WeightsFP8(cfg, qw)
+    ring = binding.Ring(cfg, 8, 512, max_rows=288)
+    for s in range(1, 7):
+        ring.packed_forward(W, I.make_embeds(cfg, 1, s, 275 + s).cuda(), [(s, 0, 0, 275 + s)])
+    segs = [(0, 0, 0, 276)] + [(s, 1, 275 + s, 1) for s in range(1, 7)]
+    e = I.make_embeds(cfg, 1, 10, 282).cuda()
+    first = None
+    for rep in range(12):
+        ring.reset_slot(0, 0)
+        for s in range(1, 7):
+            ring.set_len(s, 275 + s)
+        hid = ring.packed_forward(W, e, segs).clone()
+        if first is None:
+            first = hid
+        assert torch.equal(hid, first), f"repetition {rep} differs"
+
+
 def test_fp8_rejects_wide_steps(binding):
     cfg = I.CFG_TINY
     qw = I.quantize_weights_fp8(I.make_weights(cfg, seed=0))
