@@ -205,7 +205,7 @@ constexpr int QKV_MAX_SLABS = QKV_MAX_SLABS_K;    // pieces per weight tile of t
 // their whole grid resident, so steps enqueued on different streams of one device are ordered behind each other with an
 // event (serialise_on): they never run concurrently, whatever the caller's streams allow.
 struct SchedKey {
-  int split, n_pairs, nkb, max_cl, splits;
+  int split, n_pairs, nkb, max_cl, splits, chunks;
   bool operator<(const SchedKey& o) const { return memcmp(this, &o, sizeof(SchedKey)) < 0; }
 };
 struct Sched { GemmPiece* dev; int n_cl; int* pair_slabs; int max_slabs; };
@@ -233,8 +233,10 @@ static int get_ctx(DevCtx** out) {
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(gemm_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
-  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
-  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
+  CUDA_TRY(cudaFuncSetAttribute(layer_chain_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BUDGET));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
@@ -253,7 +255,7 @@ static int get_ctx(DevCtx** out) {
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    if (cudaOccupancyMaxActiveClusters(&max_cl, layer_chain_kernel<false>, &cfg) != cudaSuccess || max_cl < 1) { cudaGetLastError(); max_cl = c->num_sms / 2; }
+    if (cudaOccupancyMaxActiveClusters(&max_cl, layer_chain_kernel<false, false>, &cfg) != cudaSuccess || max_cl < 1) { cudaGetLastError(); max_cl = c->num_sms / 2; }
   }
   c->max_clusters = max_cl < c->num_sms / 2 ? max_cl : c->num_sms / 2;
   if (c->max_clusters < 1) c->max_clusters = 1;
@@ -464,9 +466,11 @@ static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits
 
 // The device copy has at least max_cl rows (clusters beyond n_cl find an empty list), so that kernels whose grid is the
 // whole device (layer_chain_kernel) can index it with any cluster id.
-static int build_schedule(DevCtx* ctx, int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out) {
+// chunks = 2 (the chain with 512 < T <= 1024): every piece appears twice, for token chunk 0 and 1 (GemmPiece::pad), adjacent in
+// its cluster's list - the second pass re-reads the same weight k-range while it is still in L2.
+static int build_schedule(DevCtx* ctx, int split, int n_pairs, int nkb, int max_cl, int splits, Sched* out, int chunks = 1) {
   std::lock_guard<std::mutex> lk(g_ctx_mu);
-  const SchedKey key{split, n_pairs, nkb, max_cl, splits};
+  const SchedKey key{split, n_pairs, nkb, max_cl, splits, chunks};
   auto it = ctx->scheds.find(key);
   if (it != ctx->scheds.end()) { *out = it->second; return AF_OK; }
   std::vector<GemmPiece> flat;
@@ -474,6 +478,21 @@ static int build_schedule(DevCtx* ctx, int split, int n_pairs, int nkb, int max_
   int n_cl = 0;
   const int rc = make_schedule(split, n_pairs, nkb, max_cl, splits, &flat, &n_cl, &pair_slabs);
   if (rc) return rc;
+  if (chunks == 2) {
+    std::vector<GemmPiece> two(flat.size(), GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
+    for (int c = 0; c < n_cl; ++c) {
+      int n = 0;
+      for (int i = 0; i < GEMM_MAX_PIECES && flat[static_cast<size_t>(c) * GEMM_MAX_PIECES + i].pair >= 0; ++i) {
+        if (n + 2 > GEMM_MAX_PIECES - 1) return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: too many pieces in one cluster for two token chunks");
+        for (int ch = 0; ch < 2; ++ch) {
+          GemmPiece q = flat[static_cast<size_t>(c) * GEMM_MAX_PIECES + i];
+          q.pad = ch;
+          two[static_cast<size_t>(c) * GEMM_MAX_PIECES + n++] = q;
+        }
+      }
+    }
+    flat.swap(two);
+  }
   if (n_cl < max_cl) flat.resize(static_cast<size_t>(max_cl) * GEMM_MAX_PIECES, GemmPiece{-1, 0, 0, 0, 0, 0, 0, 0});
   Sched sc{nullptr, n_cl, nullptr, 0};
   for (int v : pair_slabs) sc.max_slabs = v > sc.max_slabs ? v : sc.max_slabs;
@@ -587,6 +606,7 @@ struct ChainBuilder {
   DevCtx* ctx = nullptr;
   int max_rows = 0;          // row capacity of the workspace buffers the activation maps cover
   bool fp8 = false;          // AF_WEIGHTS_FP8: weight matrices are E4M3 codes + per-output-channel scales
+  int chunks = 1;            // 2: 512 < T <= 1024, every piece once per token chunk
   ChainBuilder() { memset(&a, 0, sizeof a); }
   int add_map(const CUtensorMap& m) {
     for (int i = 0; i < n_maps; ++i)
@@ -613,7 +633,7 @@ static int chain_add_gemm(ChainBuilder& b, const void* const* w, const float* co
   int splits = max_slabs;
   if (split == SPLIT_K) splits = gemm_split_count(b.ctx, n_tiles, K);
   Sched sc;
-  int rc = build_schedule(b.ctx, split, n_pairs, P->num_kb, b.ctx->max_clusters, split == SPLIT_STREAMK ? 1 : splits, &sc);
+  int rc = build_schedule(b.ctx, split, n_pairs, P->num_kb, b.ctx->max_clusters, split == SPLIT_STREAMK ? 1 : splits, &sc, b.chunks);
   if (rc) return rc;
   P->sched = sc.dev;
   if (pair_slabs_out) *pair_slabs_out = sc.pair_slabs;
@@ -667,7 +687,8 @@ static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   }
   const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_EPI_WARPS * 2048 + 1024;
   cudaError_t e;
-  { ProfScope ps(cat, st); e = launch_k(b.fp8 ? layer_chain_kernel<true> : layer_chain_kernel<false>, dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
+  { ProfScope ps(cat, st); e = launch_k(b.chunks == 2 ? (b.fp8 ? layer_chain_kernel<true, true> : layer_chain_kernel<false, true>)
+                                                         : (b.fp8 ? layer_chain_kernel<true, false> : layer_chain_kernel<false, false>), dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
   if (e != cudaSuccess) return fail(AF_ERR_CUDA, "launch of layer_chain_kernel failed: %s", cudaGetErrorString(e));
   return check_launch("layer_chain_kernel");
 }
@@ -1032,19 +1053,20 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   const bool fp8 = w->weight_format == AF_WEIGHTS_FP8;
   // every work list of the chain is built (and cached) BEFORE the first launch: a shape it cannot schedule falls back to the
   // per-stage path (FP8: AF_ERR_UNSUPPORTED) with nothing enqueued
+  const int t_chunks = T > GEMM_MAX_TOK ? 2 : 1;
   auto chain_schedulable = [&]() {
     const int kd = (D + GEMM_BK - 1) / GEMM_BK, kf = (F + GEMM_BK - 1) / GEMM_BK;
     const int d_pairs = ((D + GEMM_BM - 1) / GEMM_BM + 1) / 2, gu_pairs = ((F + 63) / 64 + 1) / 2;
     Sched sc;
-    return build_schedule(ctx, SPLIT_SLABS, (3 * ((D + GEMM_BM - 1) / GEMM_BM) + 1) / 2, kd, ctx->max_clusters, QKV_MAX_SLABS, &sc) == AF_OK &&
-           build_schedule(ctx, SPLIT_K, d_pairs, kd, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, D), &sc) == AF_OK &&
-           build_schedule(ctx, SPLIT_K, d_pairs, kf, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, F), &sc) == AF_OK &&
-           build_schedule(ctx, SPLIT_STREAMK, gu_pairs, kd, ctx->max_clusters, 1, &sc) == AF_OK;
+    return build_schedule(ctx, SPLIT_SLABS, (3 * ((D + GEMM_BM - 1) / GEMM_BM) + 1) / 2, kd, ctx->max_clusters, QKV_MAX_SLABS, &sc, t_chunks) == AF_OK &&
+           build_schedule(ctx, SPLIT_K, d_pairs, kd, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, D), &sc, t_chunks) == AF_OK &&
+           build_schedule(ctx, SPLIT_K, d_pairs, kf, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, F), &sc, t_chunks) == AF_OK &&
+           build_schedule(ctx, SPLIT_STREAMK, gu_pairs, kd, ctx->max_clusters, 1, &sc, t_chunks) == AF_OK;
   };
-  if (fp8 && (T > GEMM_MAX_TOK || D > 4096 || D % 256 != 0 || F < 128 || ctx->max_clusters < 2 || g_prof_stages))
-    return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8 runs on the layer chain only: T <= %d packed rows, d_model <= 4096 and a multiple of 256", GEMM_MAX_TOK);
+  if (fp8 && (T > 2 * GEMM_MAX_TOK || D > 4096 || D % 256 != 0 || F < 128 || ctx->max_clusters < 2 || g_prof_stages))
+    return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8 runs on the layer chain only: T <= %d packed rows, d_model <= 4096 and a multiple of 256", 2 * GEMM_MAX_TOK);
   if (fp8 && !chain_schedulable()) return fail(AF_ERR_UNSUPPORTED, "AF_WEIGHTS_FP8: this shape has no layer-chain schedule on this device");
-  const bool use_chain = (w->weight_format == AF_WEIGHTS_FP16_GU || fp8) && T <= GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
+  const bool use_chain = (w->weight_format == AF_WEIGHTS_FP16_GU || fp8) && T <= 2 * GEMM_MAX_TOK && D <= 4096 && D % 256 == 0 && F >= 128 &&
                          ctx->max_clusters >= 2 && !g_prof_stages && chain_schedulable();
   if (use_chain) {
     StreamCtx sctx;
@@ -1053,9 +1075,12 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     const long long qkv_stride = static_cast<long long>(ws.max_rows) * 3 * D;
     auto begin = [&](ChainBuilder& b) {
       b.ctx = ctx; b.max_rows = ws.max_rows; b.fp8 = fp8;
-      int n_pad = (T + 15) / 16 * 16;
+      int Tc = T;                                               // rows of one token chunk
+      b.a.T0 = 0;
+      if (T > GEMM_MAX_TOK) { Tc = ((T + 1) / 2 + 15) / 16 * 16; b.a.T0 = Tc; b.chunks = 2; }
+      int n_pad = (Tc + 15) / 16 * 16;
       if (n_pad <= 256) { b.a.n1 = n_pad; b.a.n2 = 0; }
-      else { b.a.n1 = ((T + 1) / 2 + 15) / 16 * 16; b.a.n2 = b.a.n1; }
+      else { b.a.n1 = ((Tc + 1) / 2 + 15) / 16 * 16; b.a.n2 = b.a.n1; }
       b.a.T = T; b.a.D = D; b.a.eps = c.rms_eps; b.a.x = hidden_out; b.a.bar = sctx.bar; b.a.flags = sctx.flags;
       b.a.partial = reinterpret_cast<uint8_t*>(ws.partial); b.a.tb = g->tb; b.a.rope_tab = g->rope_tab;
       b.a.H = H; b.a.hd = hd; b.a.R = R; b.a.C = C;

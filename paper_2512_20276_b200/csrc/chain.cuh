@@ -58,6 +58,9 @@ struct ChainArgs {
   ChainPhase ph[CH_MAX_PHASES];
   int n_phases;
   int T, n1, n2;            // packed rows; UMMA N of the two token halves (n2 may be 0)
+  int T0;                   // 0: one token chunk (T <= 512).  Else 512 < T <= 1024: every piece exists twice (GemmPiece::pad = token
+                            // chunk 0 / 1, adjacent in its cluster's list, so the second pass re-reads its weight k-range from L2):
+                            // chunk 0 = rows [0, T0), chunk 1 = rows [T0, T); n1, n2 describe one chunk
   int stages;
   int D;
   float eps;
@@ -290,11 +293,14 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
   }
 }
 
-template <bool kFp8>
+// kTwo: 512 < T <= 1024, two token chunks per piece (ChainArgs::T0); a separate instantiation so that the one-chunk kernel
+// - the benchmark path - carries none of the chunk arithmetic (measured: 4 % of the step when it was a runtime branch).
+template <bool kFp8, bool kTwo>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  const int T0 = kTwo ? a.T0 : 0;
   const int n_pad = a.n1 + a.n2;
   constexpr uint32_t a_bytes = GEMM_BM * GEMM_BK * 2;
   const uint32_t b_bytes = static_cast<uint32_t>(n_pad / 2) * GEMM_BK * 2;   // this CTA's half of the activation rows
@@ -348,10 +354,10 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
     // stage ring allows; the ACTIVATION cursor follows and stops at a phase until that phase's input has been
     // published (deps_done, raised by this CTA's epilogue after the grid barrier; phase 0: griddepcontrol.wait).
     if (lane == 0) {
-      const uint64_t pol_w = policy_evict_first();
+      const uint64_t pol_w = T0 > 0 ? policy_evict_last() : policy_evict_first();   // (two token chunks: the second pass re-reads the k-range from L2)
       const uint64_t pol_x = policy_evict_last();
       // A cursor walks the (phase, piece, k-block) units of this cluster in order; all of its state is in registers.
-      struct Cursor { int ph, pi, kb, kb1, row; const CUtensorMap* wmap; const CUtensorMap* xmap; const GemmPiece* list; bool more; };
+      struct Cursor { int ph, pi, kb, kb1, row, tok0; const CUtensorMap* wmap; const CUtensorMap* xmap; const GemmPiece* list; bool more; };
       auto next_piece = [&](Cursor& c) {   // move to the next (phase, piece) that has k-blocks
         while (true) {
           if (c.ph >= 0 && c.pi + 1 < GEMM_MAX_PIECES) {
@@ -365,6 +371,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
               c.wmap = &a.maps[P.w_map[part]];
               c.row = P.a_pair ? tile * GEMM_BM : (tile - part * P.tiles_per_part) * GEMM_BM;
               c.kb = pc.kb0; c.kb1 = pc.kb1;
+              c.tok0 = kTwo ? pc.pad * T0 : 0;
               return;
             }
           }
@@ -389,11 +396,11 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
       };
       auto load_x = [&](const Cursor& c, int stage) {
         uint8_t* sb = tiles + static_cast<size_t>(stage) * stage_bytes + a_bytes;
-        tma_load_2d_cg2(sb, c.xmap, &full_bar[stage], c.kb * GEMM_BK, crank * h1, pol_x);
+        tma_load_2d_cg2(sb, c.xmap, &full_bar[stage], c.kb * GEMM_BK, c.tok0 + crank * h1, pol_x);
         if (a.n2 > 0)
-          tma_load_2d_cg2(sb + static_cast<size_t>(h1) * GEMM_BK * 2, c.xmap, &full_bar[stage], c.kb * GEMM_BK, a.n1 + crank * h1, pol_x);
+          tma_load_2d_cg2(sb + static_cast<size_t>(h1) * GEMM_BK * 2, c.xmap, &full_bar[stage], c.kb * GEMM_BK, c.tok0 + a.n1 + crank * h1, pol_x);
       };
-      Cursor w{-1, GEMM_MAX_PIECES, 0, 0, 0, nullptr, nullptr, nullptr, true};
+      Cursor w{-1, GEMM_MAX_PIECES, 0, 0, 0, 0, nullptr, nullptr, nullptr, true};
       next_piece(w);
       Cursor x = w;                      // the activation cursor: equal to w in lock step, behind it at a phase boundary
       int st_w = 0, st_x = 0, lag = 0;   // lag = stages that hold weights but not yet their activations
@@ -551,12 +558,15 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
             }
           }
           const bool contributor = pc.kind == PK_CONTRIB;
-          const int my_slot = pc.slot * 2 + crank;
+          const int chunk = kTwo ? pc.pad : 0, tok0 = chunk * T0;                      // token chunk of this piece (0 unless T > 512)
+          const int Tv = T0 > 0 ? (chunk ? a.T - T0 : T0) : a.T;        // its valid rows
+          const int nch = T0 > 0 ? 2 : 1;
+          const int my_slot = (pc.slot * nch + chunk) * 2 + crank;           // partial / flag slot: per (cluster, chunk, CTA of the pair)
           int n_contrib = 0, c_first = 0;
           if (pc.kind == PK_OWNER) {
             c_first = pc.slot; n_contrib = pc.n_contrib;
             if (etid < n_contrib) {
-              volatile int* f = a.flags + (c_first + etid) * 2 + crank;
+              volatile int* f = a.flags + ((c_first + etid) * nch + chunk) * 2 + crank;
               SpinGuard sg;
               while (*f == 0) sg.poll();
               *f = 0;   // one consumer per flag: ready for the next use (graph-replay safe)
@@ -571,7 +581,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           const int st_feat = f0 + 8 * (lane & ((1 << st_sh) - 1)), st_tok = lane >> st_sh;
           const bool st_ok = tile_valid && st_feat < P.out_features;
           act_t* const st_ptr = P.out + static_cast<size_t>(P.epi == EPI_SWIGLU ? 0 : pc.mid) * P.out_ld_slab +
-                                static_cast<size_t>(part) * P.part_rows + st_feat + static_cast<size_t>(st_tok) * P.out_ld_tok;
+                                static_cast<size_t>(part) * P.part_rows + st_feat + static_cast<size_t>(tok0 + st_tok) * P.out_ld_tok;
           // partial exchange (stream-K): thread-private 64 bytes per 32-token chunk, in the epilogue's register layout
           auto part_ptr = [&](int slot, int c0) {
             return a.partial + (static_cast<size_t>(slot) * (GEMM_MAX_TOK / 32) * 4 + (c0 >> 5) * 4 + quad) * 2048 + lane * 16;
@@ -612,7 +622,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
             }
           };
           auto fix_load = [&](int c, int c0, uint4* q) {   // contributor c's partial of this thread's chunk
-            const uint8_t* src = part_ptr((c_first + c) * 2 + crank, c0);
+            const uint8_t* src = part_ptr(((c_first + c) * nch + chunk) * 2 + crank, c0);
 #pragma unroll
             for (int g = 0; g < 4; ++g) q[g] = __ldcg(reinterpret_cast<const uint4*>(src + g * 512));
           };
@@ -646,7 +656,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
                                   pack_act(v[16 + 4 * g], v[16 + 4 * g + 1]), pack_act(v[16 + 4 * g + 2], v[16 + 4 * g + 3]));
               __syncwarp();
               act_t* dst = st_ptr + static_cast<size_t>(c0) * P.out_ld_tok;
-              const int n_ok = a.T - c0 - st_tok;
+              const int n_ok = Tv - c0 - st_tok;
 #pragma unroll
               for (int g = 0; g < 4; ++g)
                 if (st_ok && 8 * g < n_ok)
@@ -665,7 +675,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
               stmatrix_x4_trans(sa + frag_off32 + 512, h[4], h[5], h[6], h[7]);
               __syncwarp();
               act_t* dst = st_ptr + static_cast<size_t>(c0) * P.out_ld_tok;
-              const int n_ok = a.T - c0 - st_tok;
+              const int n_ok = Tv - c0 - st_tok;
 #pragma unroll
               for (int j = 0; j < 2; ++j)
                 if (st_ok && 16 * j < n_ok)
@@ -677,7 +687,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           {
             float v[32], vb[32];
             uint4 q[4];
-            auto in_range = [&](int c0) { return c0 < n_pad && c0 < a.T; };
+            auto in_range = [&](int c0) { return c0 < n_pad && c0 < Tv; };
             auto step = [&](int c0, float* cur, float* nxt) {
               tmem_ld_wait();
               apply_scale(cur);     // (before the fix-up adds and every store: partials and slabs carry scaled sums)

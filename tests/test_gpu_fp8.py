@@ -110,12 +110,24 @@ def test_fp8_single_7b_layer_is_deterministic(binding):
         assert torch.equal(hid, first), f"repetition {rep} differs"
 
 
+def test_fp8_two_token_chunks_tiny(binding):
+    """512 < T <= 1024 runs the layer chain with two token chunks per projection (FP8 weights): 700 packed rows."""
+    cfg = I.CFG_TINY
+    qw = I.quantize_weights_fp8(I.make_weights(cfg, seed=0))
+    W = binding.WeightsFP8(cfg, qw)
+    P = Pair(cfg, qw["dequant"], R=3, C=1024, max_rows=1024, dev_weights=W)
+    P.step([(1, 0, 0, 33)], I.make_embeds(cfg, 0, 0, 33))
+    hid, ref = P.step([(0, 0, 0, 650), (1, 1, 33, 1), (2, 0, 0, 49)], I.make_embeds(cfg, 0, 1, 700))
+    P.check_ring([0, 1, 2])
+    print(f"fp8, 700 rows: hidden {relmax(hid, ref):.3e}")
+
+
 def test_fp8_rejects_wide_steps(binding):
     cfg = I.CFG_TINY
     qw = I.quantize_weights_fp8(I.make_weights(cfg, seed=0))
     W = binding.WeightsFP8(cfg, qw)
-    ring = binding.Ring(cfg, 2, 1024, max_rows=1024)
+    ring = binding.Ring(cfg, 2, 2048, max_rows=2048)
     with pytest.raises(binding.AfError) as ei:
-        ring.packed_forward(W, I.make_embeds(cfg, 0, 0, 600).cuda(), [(0, 0, 0, 600)])
+        ring.packed_forward(W, I.make_embeds(cfg, 0, 0, 1100).cuda(), [(0, 0, 0, 1100)])
     assert ei.value.code == binding.AF_ERR_UNSUPPORTED
     assert ring.get_state(0) == (0, 0)

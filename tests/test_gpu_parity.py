@@ -229,15 +229,16 @@ def test_prepare_gate_up_layout(binding):
     assert torch.equal(out.cpu(), ref)
 
 
-@pytest.mark.parametrize("n_prefill", [257, 300, 513])
+@pytest.mark.parametrize("n_prefill", [257, 300, 509, 513, 800, 1021, 1100])
 def test_wide_packed_steps_tiny(binding, n_prefill):
-    """Packed steps wider than one UMMA N (two accumulator halves: 257, 300 rows) and wider than one GEMM launch (513
-    rows: two token chunks) on the tiny model, whose ffn = 688 leaves a ragged SwiGLU tile: a long prefill that wraps
-    its region, packed with decode rows of three other requests."""
+    """Packed steps wider than one UMMA N (two accumulator halves: 257, 300, 512 rows), wider than the 512 TMEM columns
+    (516 .. 1024 rows: the layer chain walks two token chunks per weight tile) and wider than that (1103 rows: the
+    per-stage path, three GEMM launches per projection) on the tiny model, whose ffn = 688 leaves a ragged SwiGLU tile: a
+    long prefill that wraps its region, packed with decode rows of three other requests."""
     cfg = I.CFG_TINY
     hw = I.make_weights(cfg, seed=5)
-    R, C = 4, 640
-    P = Pair(cfg, hw, R=R, C=C, max_rows=640, bases=[600, 0, 17, 639])
+    R, C = 4, 1280
+    P = Pair(cfg, hw, R=R, C=C, max_rows=1280, bases=[1200, 0, 17, 1279])
     for r in (1, 2, 3):
         P.step([(r, 0, 0, 20 + r)], I.make_embeds(cfg, 5, r, 20 + r))
     segs = [(0, 0, 0, n_prefill)] + [(r, 1, 20 + r, 1) for r in (1, 2, 3)]
