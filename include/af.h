@@ -104,7 +104,7 @@ typedef struct {                 /* all device bf16 */
                                    * OUTPUT channel; the matrix the library multiplies by is value(code) * scale[out].
                                    * The codes are widened to fp16 (exactly) tile by tile in shared memory and the scale
                                    * is applied to the fp32 accumulator, so HBM carries half the bytes of the 16-bit
-                                   * formats.  w_lm stays a prepared fp16 matrix.  Packed steps of more than 512 rows
+                                   * formats.  w_lm stays a prepared fp16 matrix.  Packed steps of more than 1024 rows
                                    * return AF_ERR_UNSUPPORTED in this format. */
 
 typedef struct {                  /* AF_WEIGHTS_FP8: device fp32 [out_features] per matrix */

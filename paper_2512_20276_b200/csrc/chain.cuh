@@ -14,7 +14,8 @@
 // layout: the owner thread reads back exactly the 64 bytes its counterpart wrote, no shared-memory staging).
 //
 // Restrictions (the host falls back to the one-kernel-per-stage path otherwise): prepared fp16 weights with gate|up
-// interleaved (AF_WEIGHTS_FP16_GU), T <= 512 packed rows, d_model <= 4096, at least two weight tiles per projection.
+// interleaved (AF_WEIGHTS_FP16_GU) or FP8 codes, T <= 1024 packed rows (above 512: two token chunks per piece, kTwo),
+// d_model <= 4096, at least two weight tiles per projection.
 #pragma once
 #include "gemm_tcgen05.cuh"
 #include "attention.cuh"   // StepTables
