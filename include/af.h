@@ -191,6 +191,18 @@ int af_logits_rows(const af_weights* w, const float* hidden, const int32_t* rows
  *   logits : device fp32 [n_rows, vocab] (row pitch = vocab);  tokens_out : device int32 [n_rows].  Enqueued. */
 int af_argmax_rows(const float* logits, int32_t n_rows, int32_t vocab, int32_t* tokens_out, void* cuda_stream);
 
+/* af_argmax_rows for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same result (the rule above is order-free, so the tokens are identical), no
+ * cudaMalloc / cudaFree / allocating library routine on any call, the first included.  Every row's vocabulary is split
+ * over up to 64 CTAs; their candidates and one arrival counter per row live in a static __device__ array inside the
+ * library (131 KB of device memory that every GPU which loads the library holds until exit).
+ *   n_rows <= AF_ARGMAX_STATIC_MAX_ROWS, else AF_ERR_UNSUPPORTED (nothing enqueued; use af_argmax_rows).
+ *   Every call on a device shares that array, which keeps the last call's contents; the call clears the counters it
+ *   uses (a memset enqueued before the kernel).  Calls that OVERLAP on the GPU (two streams, or two processes' worth of
+ *   threads on one device) race on it and return wrong tokens: order them on one stream or with events.  Enqueued. */
+#define AF_ARGMAX_STATIC_MAX_ROWS 256
+int af_argmax_rows_static(const float* logits, int32_t n_rows, int32_t vocab, int32_t* tokens_out, void* cuda_stream);
+
 /* embeds_out[i, :] = table[tokens[i], :]  (the token half of Alg. 1 l.2 "Embed(.., GetLastTokenEach(A_sequences))",
  * P:134): the rows a step's decode segments take as input.  A copy, bit-exact.
  *   table : device bf16 [vocab, d_model] (d_model % 8 == 0, 16-byte aligned);  tokens : device int32 [n_rows], each in

@@ -53,7 +53,7 @@ class af_weights(C.Structure):
 
 
 EXPORTS = ["af_prepare_gate_up_fp8", "af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
-           "af_argmax_rows", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
+           "af_argmax_rows", "af_argmax_rows_static", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
            "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
@@ -81,6 +81,8 @@ def load_library():
     L.af_convert_bf16_to_fp16.restype = C.c_int
     L.af_argmax_rows.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
     L.af_argmax_rows.restype = C.c_int
+    L.af_argmax_rows_static.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
+    L.af_argmax_rows_static.restype = C.c_int
     L.af_embed_rows.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int32, vp, vp]
     L.af_embed_rows.restype = C.c_int
     L.af_gate_up_rows.argtypes = [C.c_int32]
@@ -350,6 +352,15 @@ def argmax_rows(logits: torch.Tensor) -> torch.Tensor:
     assert logits.is_cuda and logits.dtype == torch.float32 and logits.dim() == 2 and logits.is_contiguous()
     out = torch.empty(logits.shape[0], dtype=torch.int32, device=logits.device)
     _check(load_library().af_argmax_rows(logits.data_ptr(), logits.shape[0], logits.shape[1], out.data_ptr(), _stream_ptr()))
+    return out
+
+
+def argmax_rows_static(logits: torch.Tensor, out: torch.Tensor) -> torch.Tensor:
+    """af_argmax_rows_static: af_argmax_rows without any allocation in the library (static device scratch, at most
+    AF_ARGMAX_STATIC_MAX_ROWS = 256 rows); `out` is the caller's int32 [n] device tensor."""
+    assert logits.is_cuda and logits.dtype == torch.float32 and logits.dim() == 2 and logits.is_contiguous()
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() >= logits.shape[0]
+    _check(load_library().af_argmax_rows_static(logits.data_ptr(), logits.shape[0], logits.shape[1], out.data_ptr(), _stream_ptr()))
     return out
 
 

@@ -1412,3 +1412,111 @@ extern "C" int af_loop_step(af_loop* lp, int32_t use_graph, void* cuda_stream) {
 }
 
 extern "C" int32_t af_loop_steps_done(const af_loop* lp) { return lp ? lp->t : -1; }
+
+// ------------------------------------------------------------------------------------------------ f1 without allocation
+// af_argmax_rows_static: the ArgMax of Alg. 1 l.5/l.8 for callers that cannot allocate (code under stream capture, tight
+// serving loops).  A variant of argmax_rows_kernel that splits every row's vocabulary over several CTAs (a decode step
+// has 1 + n_dec rows: one CTA per row leaves most of the 148 SMs idle) and therefore needs scratch: the per-chunk
+// (value, index) candidates and one arrival ticket per row.  That scratch is the file-scope array below - 131 KB that
+// every GPU which loads the library holds until exit - instead of caller or cudaMalloc memory.  In HOST code the array's
+// name is a host-side stand-in, not a device address: the launch takes the pointer cudaGetSymbolAddress returns, looked
+// up once per device with that device current.
+constexpr int ARGMAX_STATIC_MAX_ROWS = AF_ARGMAX_STATIC_MAX_ROWS;
+constexpr int ARGMAX_STATIC_MAX_CHUNKS = 64;       // CTAs per row at most
+constexpr int ARGMAX_STATIC_MIN_CHUNK = 2048;      // logits per CTA at least (8 per thread)
+constexpr int ARGMAX_STATIC_MAX_DEVICES = 64;
+struct ArgmaxScratch {
+  float v[ARGMAX_STATIC_MAX_ROWS][ARGMAX_STATIC_MAX_CHUNKS];
+  int i[ARGMAX_STATIC_MAX_ROWS][ARGMAX_STATIC_MAX_CHUNKS];
+  unsigned ticket[ARGMAX_STATIC_MAX_ROWS];         // chunks of the row that have published their candidate; 0 between calls
+};
+static __device__ __align__(256) unsigned char g_argmax_scratch[sizeof(ArgmaxScratch)];
+
+// grid (n_chunks, n_rows).  CTA (c, r) reduces logits[r, c*chunk .. (c+1)*chunk) with argmax_rows_kernel's order-free
+// rule ("greater value, or equal value and lower index, wins"; NaNs lose every comparison), publishes its candidate and
+// takes a ticket; the CTA that takes the row's last ticket reduces the candidates, stores the token and puts the ticket
+// back to 0.
+__global__ void __launch_bounds__(256)
+argmax_rows_split_kernel(const float* __restrict__ logits, int vocab, int chunk, int* __restrict__ tokens_out, ArgmaxScratch* sc) {
+  __shared__ float s_v[8];
+  __shared__ int s_i[8];
+  __shared__ bool s_last;
+  const int r = blockIdx.y, c = blockIdx.x, n_chunks = gridDim.x;
+  const float* row = logits + static_cast<size_t>(r) * vocab;
+  const int v0 = c * chunk, v1 = min(vocab, v0 + chunk);
+  auto better = [](float a, int ai, float b, int bi) { return a > b || (a == b && ai < bi); };
+  auto block_reduce = [&](float& best, int& best_i) {   // result in thread 0
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, best_i, o);
+      if (better(ov, oi, best, best_i)) { best = ov; best_i = oi; }
+    }
+    if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = best; s_i[threadIdx.x >> 5] = best_i; }
+    __syncthreads();
+    if (threadIdx.x == 0)
+      for (int w = 1; w < 8; ++w)
+        if (better(s_v[w], s_i[w], best, best_i)) { best = s_v[w]; best_i = s_i[w]; }
+  };
+  float best = -INFINITY;
+  int best_i = 0x7fffffff;
+  for (int v = v0 + threadIdx.x; v < v1; v += 256) {
+    const float x = row[v];
+    if (better(x, v, best, best_i)) { best = x; best_i = v; }
+  }
+  block_reduce(best, best_i);
+  if (threadIdx.x == 0) {
+    sc->v[r][c] = best;
+    sc->i[r][c] = best_i;
+    __threadfence();                                     // the candidate is visible before the ticket is
+    s_last = atomicAdd(&sc->ticket[r], 1u) == static_cast<unsigned>(n_chunks - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();                                       // the other chunks' candidates, published before their tickets
+  best = -INFINITY;
+  best_i = 0x7fffffff;
+  if (threadIdx.x < n_chunks) {
+    best = __ldcg(&sc->v[r][threadIdx.x]);
+    best_i = __ldcg(&sc->i[r][threadIdx.x]);
+  }
+  __syncthreads();                                       // s_v / s_i are reused
+  block_reduce(best, best_i);
+  if (threadIdx.x == 0) {
+    tokens_out[r] = best_i == 0x7fffffff ? 0 : best_i;
+    sc->ticket[r] = 0u;
+  }
+}
+
+static std::mutex g_argmax_static_mu;
+static ArgmaxScratch* g_argmax_static_ptr[ARGMAX_STATIC_MAX_DEVICES] = {};
+
+extern "C" int af_argmax_rows_static(const float* logits, int32_t n_rows, int32_t vocab, int32_t* tokens_out, void* cuda_stream) {
+  if (n_rows < 0 || vocab <= 0 || (n_rows > 0 && (!logits || !tokens_out))) return fail(AF_ERR_ARG, "af_argmax_rows_static: bad argument");
+  if (n_rows > ARGMAX_STATIC_MAX_ROWS)
+    return fail(AF_ERR_UNSUPPORTED, "af_argmax_rows_static: n_rows %d > %d, the rows its static scratch holds (use af_argmax_rows)", n_rows, ARGMAX_STATIC_MAX_ROWS);
+  if (n_rows == 0) return AF_OK;
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= ARGMAX_STATIC_MAX_DEVICES) return fail(AF_ERR_UNSUPPORTED, "af_argmax_rows_static: device %d outside [0,%d)", dev, ARGMAX_STATIC_MAX_DEVICES);
+  ArgmaxScratch* sc = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_argmax_static_mu);
+    if (!g_argmax_static_ptr[dev]) {                     // set-up, once per device, with that device current
+      void* p = nullptr;
+      CUDA_TRY(cudaGetSymbolAddress(&p, g_argmax_scratch));
+      g_argmax_static_ptr[dev] = static_cast<ArgmaxScratch*>(p);
+    }
+    sc = g_argmax_static_ptr[dev];
+  }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int n_chunks = (vocab + ARGMAX_STATIC_MIN_CHUNK - 1) / ARGMAX_STATIC_MIN_CHUNK;
+  if (n_chunks > ARGMAX_STATIC_MAX_CHUNKS) n_chunks = ARGMAX_STATIC_MAX_CHUNKS;
+  const int chunk = (vocab + n_chunks - 1) / n_chunks;
+  n_chunks = (vocab + chunk - 1) / chunk;                // no empty chunk
+  // the array keeps the last call's contents: tickets must start at 0 (they do after a call that ran to its end; a call
+  // that was aborted, or one that overlapped another, may have left some behind)
+  CUDA_TRY(cudaMemsetAsync(sc->ticket, 0, sizeof(unsigned) * n_rows, st));
+  argmax_rows_split_kernel<<<dim3(n_chunks, n_rows), 256, 0, st>>>(logits, vocab, chunk, tokens_out, sc);
+  return check_launch("argmax_rows_split_kernel");
+}
