@@ -55,7 +55,7 @@ class af_weights(C.Structure):
 EXPORTS = ["af_prepare_gate_up_fp8", "af_ring_set_window", "af_loop_create", "af_loop_buffers", "af_loop_step", "af_loop_steps_done", "af_loop_destroy",
            "af_argmax_rows", "af_argmax_rows_static", "af_embed_rows", "af_convert_bf16_to_fp16", "af_gate_up_rows", "af_prepare_gate_up", "af_ring_bytes", "af_workspace_bytes", "af_ring_create", "af_ring_reset_slot", "af_packed_forward",
            "af_logits_rows", "af_ring_destroy", "af_ring_get_state", "af_debug_row_map", "af_debug_set_len",
-           "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
+           "af_debug_launch_count", "af_debug_gemm", "af_debug_gemm_schedule", "af_debug_profile", "af_debug_attention", "af_debug_profile_read", "af_debug_trace", "af_debug_trace_read", "af_last_error"]
 
 PROFILE_CLASSES = ["gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm", "attention", "rope_append",
                    "rmsnorm", "chain", "other"]
@@ -320,6 +320,13 @@ def profile(enable: bool):
     _check(load_library().af_debug_profile(1 if enable else 0))
 
 
+def attention_mode(mode: int):
+    """af_debug_attention: 0 / 1 = attention_kernel (mma.sync), 2 = the tcgen05 units of attention_umma.cuh where they apply."""
+    L = load_library()
+    L.af_debug_attention.argtypes, L.af_debug_attention.restype = [C.c_int], C.c_int
+    _check(L.af_debug_attention(int(mode)))
+
+
 def profile_read() -> dict:
     """{class: (sum_ms, launches)} since the last read (CUDA events on the launching stream)."""
     n = len(PROFILE_CLASSES)
@@ -332,7 +339,7 @@ def chain_trace(enable: bool):
     """af_debug_trace: switch the layer-chain kernel's per-phase %globaltimer stamps on / off (synchronises)."""
     L = load_library()
     L.af_debug_trace.argtypes, L.af_debug_trace.restype = [C.c_int], C.c_int
-    _check(L.af_debug_trace(1 if enable else 0))
+    _check(L.af_debug_trace(int(enable)))   # 2: the attention_umma_kernel launches' stamps instead of the chain's
 
 
 def chain_trace_read():

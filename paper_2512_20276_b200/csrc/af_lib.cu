@@ -62,6 +62,12 @@ struct ProfScope {
   }
   ~ProfScope() { if (on) { cudaEventRecord(r.b, st); g_prof.push_back(r); } }
 };
+static int g_att_mode = 0;   // af_debug_attention: 0 / 1 attention_kernel (mma.sync); 2 the tcgen05 units of attention_umma.cuh where they apply
+extern "C" int af_debug_attention(int mode) {
+  if (mode < 0 || mode > 2) return fail(AF_ERR_ARG, "af_debug_attention: mode %d outside [0,2]", mode);
+  g_att_mode = mode;
+  return AF_OK;
+}
 extern "C" int af_debug_profile(int enable) { g_prof_on = enable != 0; g_prof_stages = enable == 2; return AF_OK; }
 extern "C" int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n) {
   if (!ms_sum || !counts || n < PC_COUNT) return fail(AF_ERR_ARG, "need %d slots", (int)PC_COUNT);
@@ -241,6 +247,7 @@ static int get_ctx(DevCtx** out) {
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(128)));
   CUDA_TRY(cudaFuncSetAttribute(attention_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem_bytes(64)));
+  CUDA_TRY(cudaFuncSetAttribute(attention_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AU_SMEM_BYTES));
   DevCtx* c = new DevCtx();
   c->dev = dev;
   c->num_sms = prop.multiProcessorCount < GEMM_MAX_GRID ? prop.multiProcessorCount : GEMM_MAX_GRID;
@@ -303,6 +310,7 @@ static int serialise_done(DevCtx* c, cudaStream_t st) {
 constexpr int TRACE_LAUNCHES = 16;
 static long long* g_trace = nullptr;
 static int g_trace_n = 0;
+static bool g_trace_att = false;
 struct TraceMeta { int n_phases, grid; };
 static TraceMeta g_trace_meta[TRACE_LAUNCHES];
 extern "C" int af_debug_trace(int enable) {
@@ -313,6 +321,7 @@ extern "C" int af_debug_trace(int enable) {
   }
   if (!enable && g_trace) { cudaFree(g_trace); g_trace = nullptr; }
   g_trace_n = 0;
+  g_trace_att = enable == 2;
   return AF_OK;
 }
 extern "C" int af_debug_trace_read(long long* out, int* meta) {
@@ -671,6 +680,16 @@ static int chain_add_rope(ChainBuilder& b, const act_t* qkv_slabs, long long sla
   return AF_OK;
 }
 
+static int chain_add_attn(ChainBuilder& b, const AuArgs& att) {   // must be the launch's last phase
+  if (b.a.n_phases >= CH_MAX_PHASES) return fail(AF_ERR_UNSUPPORTED, "chain: too many phases");
+  ChainPhase& P = b.a.ph[b.a.n_phases++];
+  P = ChainPhase{};
+  P.kind = CH_ATTN;
+  b.a.att = att;
+  b.a.att_on = 1;
+  return AF_OK;
+}
+
 static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   const int n_pad = b.a.n1 + b.a.n2;
   const int stage_bytes = GEMM_BM * GEMM_BK * 2 + (n_pad / 2) * GEMM_BK * 2;   // (FP8: the raw tile lands inside the fp16 tile's slot)
@@ -680,12 +699,18 @@ static int chain_launch(ChainBuilder& b, cudaStream_t st, int cat) {
   b.a.stages = stages;
   const int grid = 2 * b.ctx->max_clusters;
   b.a.trace = nullptr;
-  if (g_trace && grid <= GEMM_MAX_GRID) {
+  if (g_trace && !g_trace_att && grid <= GEMM_MAX_GRID) {
     b.a.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * CH_TRACE_SLOTS;
     g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {b.a.n_phases, grid};
     ++g_trace_n;
   }
-  const size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_EPI_WARPS * 2048 + 1024;
+  size_t smem = static_cast<size_t>(stages) * stage_bytes + GEMM_EPI_WARPS * 2048 + 1024;
+  if (b.a.att_on) {   // the attention units' tiles and state reuse the stage ring
+    if (b.a.ph[b.a.n_phases - 1].kind != CH_ATTN) return fail(AF_ERR_UNSUPPORTED, "chain: attention must be the last phase");
+    const size_t need = static_cast<size_t>(AU_TILE_BYTES) + sizeof(AuAux) + 1024;
+    if (need > static_cast<size_t>(GEMM_SMEM_BUDGET)) return fail(AF_ERR_UNSUPPORTED, "chain: attention tiles do not fit shared memory");
+    if (smem < need) smem = need;
+  }
   cudaError_t e;
   { ProfScope ps(cat, st); e = launch_k(b.chunks == 2 ? (b.fp8 ? layer_chain_kernel<true, true> : layer_chain_kernel<false, true>)
                                                          : (b.fp8 ? layer_chain_kernel<true, false> : layer_chain_kernel<false, false>), dim3(grid), dim3(GEMM_THREADS), smem, st, 2, b.a); }
@@ -702,6 +727,7 @@ struct af_ring {
   int* tables = nullptr;        // library-owned device ints backing StepTables
   StepTables tb{};
   int* n_items_dev = nullptr;
+  int* att_sched = nullptr;
   float2* rope_tab = nullptr;   // [C][hd/2]
   int max_rows = 0;
   int last_T = 0;
@@ -784,7 +810,7 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   g->max_pos = r->capacity;
   const long long cap_rows = static_cast<long long>(r->n_regions) * r->capacity;
   g->max_rows = static_cast<int>(cap_rows > 65536 ? 65536 : cap_rows);
-  const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 4 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1;
+  const size_t n_int = 5 * AF_MAX_SEGS + 3 * static_cast<size_t>(g->max_rows) + 4 * (g->max_rows / ATT_BQ + AF_MAX_SEGS) + 1 + 2;
   cudaError_t e = cudaMalloc(&g->tables, n_int * sizeof(int));
   if (e == cudaSuccess) e = cudaMalloc(&g->rope_tab, static_cast<size_t>(r->capacity) * (c->head_dim / 2) * sizeof(float2));
   if (e != cudaSuccess) { cudaFree(g->tables); delete g; return fail(AF_ERR_CUDA, "cudaMalloc: %s", cudaGetErrorString(e)); }
@@ -794,7 +820,9 @@ extern "C" int af_ring_create(const af_model_cfg* c, const af_ring_cfg* r, void*
   g->tb.row_req = p; p += g->max_rows; g->tb.row_pos = p; p += g->max_rows; g->tb.row_slot = p; p += g->max_rows;
   const int max_items = g->max_rows / ATT_BQ + AF_MAX_SEGS;
   g->tb.item_seg = p; p += max_items; g->tb.item_q0 = p; p += max_items; g->tb.item_tmp = p; p += 2 * max_items;
-  g->n_items_dev = p;
+  g->n_items_dev = p; ++p;
+  g->att_sched = p;   // attention_umma_kernel's unit counters: zero between launches
+  if (cudaMemset(g->att_sched, 0, 2 * sizeof(int)) != cudaSuccess) { cudaFree(g->tables); cudaFree(g->rope_tab); delete g; return fail(AF_ERR_CUDA, "cudaMemset failed"); }
   const int n = r->capacity * (c->head_dim / 2);
   rope_table_kernel<<<(n + 255) / 256, 256>>>(g->rope_tab, r->capacity, c->head_dim, static_cast<double>(c->rope_theta));
   rc = check_launch("rope_table_kernel");
@@ -1040,8 +1068,35 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   if ((rc = check_launch("rowmap_kernel"))) return rc;
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
+  // a4 on tcgen05 (attention_umma.cuh) when every segment's context fits one unit; attention_kernel otherwise
+  bool att_umma = g_att_mode == 2 && hd == AU_HD && g->window == 0;
+  int au_items = 0, au_rows = 0;
+  for (int s = 0; s < n_segs; ++s) {
+    if (segs[s].start_pos + segs[s].len > AU_KV_MAX) att_umma = false;
+    if (segs[s].len == 1) ++au_rows;
+    else au_items += (segs[s].len + AU_BQ - 1) / AU_BQ;
+  }
+  if (au_items > AU_MAX_ITEMS) att_umma = false;
+  const int au_units = (au_items + au_rows) * H;
+  auto attn_args = [&](int l) {
+    AuArgs aa{};
+    aa.q = ws.q_rot; aa.kv = g->kv + layer_elems * l; aa.out = ws.attn; aa.tb = g->tb; aa.n_segs = n_segs; aa.H = H; aa.R = R; aa.C = C;
+    aa.scale_log2 = scale_log2; aa.sched = g->att_sched;
+    if (g_trace && g_trace_att) {   // af_debug_trace(2): the attention units' stamps instead of the chain's
+      aa.trace = g_trace + static_cast<size_t>(g_trace_n % TRACE_LAUNCHES) * GEMM_MAX_GRID * CH_TRACE_SLOTS;
+      g_trace_meta[g_trace_n % TRACE_LAUNCHES] = {0, ctx->num_sms};
+      ++g_trace_n;
+    }
+    return aa;
+  };
   auto launch_attention = [&](int l) -> int {   // a4: segment-masked causal attention over the ring
     act_t* kvl = g->kv + layer_elems * l;
+    if (att_umma) {
+      const AuArgs aa = attn_args(l);
+      AF_LAUNCH(PC_ATTENTION, "attention_umma_kernel", attention_umma_kernel, dim3(au_units < ctx->num_sms ? au_units : ctx->num_sms),
+                dim3(AU_THREADS), static_cast<size_t>(AU_SMEM_BYTES), st, aa);
+      return AF_OK;
+    }
     auto att = hd == 128 ? (g->window > 0 ? attention_kernel<128, true> : attention_kernel<128, false>)
                          : (g->window > 0 ? attention_kernel<64, true> : attention_kernel<64, false>);
     AF_LAUNCH(PC_ATTENTION, "attention_kernel", att, dim3(H, n_items), dim3(ATT_THREADS), att_smem_bytes(hd), st,
@@ -1099,10 +1154,11 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
       begin(b);
       if ((rc = chain_add_rows(b, packed_embeds, 1, 0, 0, w->layers[0].g_attn, ws.xn))) return rc;
       if ((rc = add_qkv_rope(b, 0))) return rc;
+      if (att_umma && (rc = chain_add_attn(b, attn_args(0)))) return rc;
       if ((rc = chain_launch(b, st, PC_CHAIN))) return rc;
     }
     for (int l = 0; l < c.n_layers; ++l) {
-      if ((rc = launch_attention(l))) return rc;
+      if (!att_umma && (rc = launch_attention(l))) return rc;   // (else: the last phase of the previous launch)
       const af_layer_weights& L = w->layers[l];
       ChainBuilder b;
       begin(b);
@@ -1120,6 +1176,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
       if (l + 1 < c.n_layers) {
         if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, w->layers[l + 1].g_attn, ws.xn))) return rc;
         if ((rc = add_qkv_rope(b, l + 1))) return rc;
+        if (att_umma && (rc = chain_add_attn(b, attn_args(l + 1)))) return rc;
       } else {
         if ((rc = chain_add_rows(b, ws.split, 0, n_slabs, split_stride, nullptr, nullptr))) return rc;   // hidden_out: no final norm
       }

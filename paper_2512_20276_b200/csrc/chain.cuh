@@ -3,6 +3,7 @@
 //
 //   [O proj -> slabs] | [x += slabs; RMSNorm] | [gate|up + SiLU*mul] | [down -> slabs] | [x += slabs; RMSNorm]
 //                     | [QKV of the next layer -> slabs] | [slab reduce + RoPE + ring append  (FusedRoPEAndWriteKV)]
+//                     | [attention of the next layer (attention_umma.cuh: tcgen05 units on the stage ring's shared memory)]
 //
 // One CTA per SM (74 two-CTA clusters), the warp roles of gemm_tcgen05.cuh (8 epilogue warps, one TMA producer, one MMA
 // issuer), and one shared-memory stage ring that lives across the phases: the producer streams the WEIGHT tiles of the
@@ -18,7 +19,7 @@
 // d_model <= 4096, at least two weight tiles per projection.
 #pragma once
 #include "gemm_tcgen05.cuh"
-#include "attention.cuh"   // StepTables
+#include "attention_umma.cuh"   // StepTables; the attention units of the chain's last phase
 
 namespace af {
 
@@ -29,7 +30,7 @@ constexpr int CH_TRACE_SLOTS = 2 * CH_MAX_PHASES + 2;
 constexpr int GEMM_MAX_SLABS_K = 4;       // slabs a row stage adds at most (= GEMM_MAX_SPLITS of af_lib.cu)
 constexpr int QKV_MAX_SLABS_K = 4;        // slabs of the QKV projection (= QKV_MAX_SLABS of af_lib.cu; all are allocated)
 
-enum ChainKind : int { CH_GEMM = 0, CH_ROWS = 1, CH_ROPE = 2 };
+enum ChainKind : int { CH_GEMM = 0, CH_ROWS = 1, CH_ROPE = 2, CH_ATTN = 3 };
 
 struct ChainPhase {
   int kind;
@@ -73,6 +74,8 @@ struct ChainArgs {
   const float2* rope_tab;
   int H, hd, R, C;
   long long* trace;         // debug: [grid][CH_TRACE_SLOTS] globaltimer stamps, or nullptr
+  int att_on;               // the LAST phase is CH_ATTN: attention of the layer whose q / k / v this launch has just produced
+  AuArgs att;               // ... its arguments (attention_umma.cuh); the units' tiles reuse the stage ring
 };
 
 // FP8 weights (f4): a stage also holds the raw 8 KB E4M3 tile, which the epilogue warps widen to the fp16 UMMA tile
@@ -294,6 +297,16 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
   }
 }
 
+// CH_ATTN on the 8 epilogue warps (a function of its own: its register allocation is independent of the GEMM epilogue's)
+// (the shared-memory pointers are rebuilt from the dynamic allocation here, not passed in: through a call boundary they would
+// be generic pointers and every P store / table read a generic access; the arguments travel by value)
+__device__ __noinline__ void chain_attn_phase(uint32_t tmem, const AuArgs a, int cta, int n_cta, int tid) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  AuAux* x = reinterpret_cast<AuAux*>(tiles + AU_TILE_BYTES);
+  au_workers(*x, tiles, tmem, a, cta, n_cta, tid);
+}
+
 // kTwo: 512 < T <= 1024, two token chunks per piece (ChainArgs::T0); a separate instantiation so that the one-chunk kernel
 // - the benchmark path - carries none of the chunk arithmetic (measured: 4 % of the step when it was a runtime branch).
 template <bool kFp8, bool kTwo>
@@ -307,6 +320,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   const uint32_t b_bytes = static_cast<uint32_t>(n_pad / 2) * GEMM_BK * 2;   // this CTA's half of the activation rows
   const uint32_t stage_bytes = a_bytes + b_bytes;   // [fp16 weight tile (FP8: the raw 8 KB tile lands in its upper half)][activation boxes]
   uint8_t* xch = tiles + static_cast<size_t>(a.stages) * stage_bytes;         // 8 x 2 KB epilogue staging
+  AuAux* ax = reinterpret_cast<AuAux*>(tiles + AU_TILE_BYTES);                // CH_ATTN: the units' small state, behind their tiles
 
   // full_bar: the stage's TMA loads have landed (FP8: the activation boxes only; the raw weight tile lands on this CTA's
   // own wfull_bar and conv_bar, on the pair's leader, counts the epilogue warps of BOTH CTAs that have widened their tile)
@@ -486,6 +500,12 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           acc_phase ^= 1;
         }
       }
+    }
+    // CH_ATTN (always the last phase): every CTA issues its own units' MMAs (cta_group::1) - nothing below waits on it
+    // (its barriers live in the epilogue staging area: they are initialised at the grid barrier before the phase, see below)
+    if (lane == 0 && a.att_on) {
+      while (ld_acquire_cta_shared(&deps_done) < a.n_phases - 1) {}
+      au_mma_loop(*ax, tiles, tmem_base);
     }
   } else {
     // ================================ epilogue warps 0..7: drains, row stages, grid barriers ================================
@@ -727,9 +747,11 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         const int ns = (P.src && !P.embed) ? P.n_slabs : 0;
         if (P.embed) chain_rows_phase<true>(a.x, P.src, 0, 0, P.gain, P.xn, a.D, a.eps, a.T, row_red, cta, n_cta, warp, lane);
         else chain_rows_phase<false>(a.x, P.src ? P.src : a.x, ns, P.slab_stride, P.gain, P.xn, a.D, a.eps, a.T, row_red, cta, n_cta, warp, lane);
-      } else {
+      } else if (P.kind == CH_ROPE) {
         chain_rope_phase(reinterpret_cast<const act_t*>(P.src), P.slab_stride, P.q_out, P.kv_layer, a.tb.row_pos, a.tb.row_slot,
                          a.rope_tab, a.H, a.hd, a.R, a.C, a.D, a.T, s_pair_slabs, cta, n_cta, warp, lane);
+      } else {
+        chain_attn_phase(tmem_base, a.att, cta, n_cta, etid);
       }
       if (etid == 0 && trace) trace[1 + 2 * ph] = static_cast<long long>(globaltimer_ns());
       // ---- grid barrier: everything this phase wrote is visible to every CTA before the next phase reads it ----
@@ -741,6 +763,10 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
           SpinGuard sg;
           while (ld_acquire_gpu(a.bar) < bar_target) sg.poll();
           fence_proxy_async_all();
+          if (a.att_on && ph + 2 == a.n_phases) {   // the next phase is CH_ATTN: its mbarriers (the staging area is free from here on)
+            au_init_barriers(*ax);
+            fence_barrier_init();
+          }
           st_release_cta_shared(&deps_done, ++n_bar);
           if (trace) trace[2 + 2 * ph] = static_cast<long long>(globaltimer_ns());
         }
