@@ -109,13 +109,17 @@ __device__ __forceinline__ float ex2_approx(float x) {   // 2^x, one MUFU; 2^(-i
   return y;
 }
 
+// The step's segment table and unit lists in shared memory: they depend on the step only, so the layer chain builds them
+// at kernel start (static shared memory), off the attention phase's path.
+struct AuLists {
+  int seg_req[AF_MAX_SEGS_K], seg_start[AF_MAX_SEGS_K], seg_len[AF_MAX_SEGS_K], seg_row0[AF_MAX_SEGS_K], seg_base[AF_MAX_SEGS_K];
+  int it_seg[AU_MAX_ITEMS], it_q0[AU_MAX_ITEMS], dec_seg[AF_MAX_SEGS_K], cnt[2];
+};
 // Shared-memory state of a CTA's attention units besides the tiles: static in attention_umma_kernel, carved from the
 // dynamic allocation (behind the tiles) in layer_chain_kernel.
 struct AuAux {
   uint64_t bar_k[3], bar_v, bar_s, bar_p, bar_o;   // K chunks / V landed (256 arrivals), S done (commit), P written (256), O done (commit)
   int kvp[2];                                      // N extent of the tensor unit the MMA thread runs next, by barrier parity; 0 = no more units
-  int seg_req[AF_MAX_SEGS_K], seg_start[AF_MAX_SEGS_K], seg_len[AF_MAX_SEGS_K], seg_row0[AF_MAX_SEGS_K], seg_base[AF_MAX_SEGS_K];
-  int it_seg[AU_MAX_ITEMS], it_q0[AU_MAX_ITEMS], dec_seg[AF_MAX_SEGS_K], cnt[2];
   int next[2];                                     // the CTA's next unit (double-buffered across units)
   float sc[AU_KV_MAX];                             // row units: scores, then probabilities
   float mx[2][AU_BQ], sm[2][AU_BQ];                // tensor units: row maxima / sums of the two column halves
@@ -174,11 +178,31 @@ __device__ __forceinline__ void au_mma_loop(AuAux& x, uint8_t* tiles, uint32_t t
   }
 }
 
+// Look-ahead between units.  A unit publishes the CTA's next unit (thread 0 knows it: static stride or the counter pop made at
+// the unit's start) at one of its block barriers, and once its own K (tensor unit: everything) is dead it starts the q + K
+// loads of a following ROW unit - one cp.async group that stays in flight across the unit boundary.
+struct AuNext {
+  int u_t0;       // thread 0: the next unit (other threads: ignored)
+  int slot;       // x.next[slot] carries it to the block
+  int n_mm, n_units;
+};
+__device__ __forceinline__ void au_row_issue_qk(AuAux& x, const AuLists& L, uint8_t* tiles, const AuArgs& a, int u, const AuNext& nx, int tid) {
+  if (u >= nx.n_mm && u < nx.n_units) {
+    const int k = (u - nx.n_mm) / a.H, h = (u - nx.n_mm) - k * a.H;
+    const int seg = L.dec_seg[k];
+    const int n = L.seg_start[seg] + 1;
+    const act_t* kbase = a.kv + (static_cast<size_t>(0 * a.R + L.seg_req[seg]) * a.H + h) * (static_cast<size_t>(a.C) * AU_HD);
+    if (tid < 16) cp_async16(x.q + tid * 16, a.q + static_cast<size_t>(L.seg_row0[seg]) * (a.H * AU_HD) + h * AU_HD + tid * 8, true);
+    au_load_rows_plain(tiles, kbase, L.seg_base[seg], a.C, (n + 15) & ~15, n, tid);
+  }
+  cp_async_commit();   // (an empty group when nothing follows: the waits below count groups)
+}
+
 // ---- tensor unit, the 8 worker warps: (segment seg, query rows q0 .. q0 + 127, head h) ----
-__device__ __forceinline__ void au_tile_unit(AuAux& x, uint8_t* tiles, uint32_t tmem, const AuArgs& a, int seg, int q0, int h,
-                                             uint32_t par, int tid, long long* trace, int ts) {
+__device__ __forceinline__ int au_tile_unit(AuAux& x, const AuLists& L, uint8_t* tiles, uint32_t tmem, const AuArgs& a, int seg, int q0, int h,
+                                            uint32_t par, const AuNext& nx, int tid, long long* trace, int ts) {
   const int warp = tid >> 5, lane = tid & 31;
-  const int req = x.seg_req[seg], start = x.seg_start[seg], len = x.seg_len[seg], row0 = x.seg_row0[seg], base = x.seg_base[seg];
+  const int req = L.seg_req[seg], start = L.seg_start[seg], len = L.seg_len[seg], row0 = L.seg_row0[seg], base = L.seg_base[seg];
   const int nq = min(AU_BQ, len - q0);
   const int kv_end = start + q0 + nq;          // positions [0, kv_end) are visible to the tile's last row
   const int kvp = (kv_end + 15) & ~15;         // N extent of S = K extent of P V
@@ -235,7 +259,9 @@ __device__ __forceinline__ void au_tile_unit(AuAux& x, uint8_t* tiles, uint32_t 
     for (int e = 0; e < 32; ++e) mx = fmaxf(mx, (j0 + e <= p) ? v[e] : -INFINITY);
   }
   x.mx[hf][r] = mx;
+  if (tid == 0) x.next[nx.slot] = nx.u_t0;
   AU_WORKER_BAR();
+  const int u_next = x.next[nx.slot];
   AU_STAMP(ts + 4);
   const float m = fmaxf(x.mx[0][r], x.mx[1][r]) * a.scale_log2;     // finite for a valid row: position 0 is always visible
   float sum = 0.f;
@@ -274,6 +300,7 @@ __device__ __forceinline__ void au_tile_unit(AuAux& x, uint8_t* tiles, uint32_t 
   mbar_wait(&x.bar_o, par);
   tc_fence_after();
   AU_STAMP(ts + 6);
+  au_row_issue_qk(x, L, tiles, a, u_next, nx, tid);   // Q, K, P and V are dead: a following row unit's loads fly during the epilogue
   act_t* dst = a.out + static_cast<size_t>(row0 + q0 + (row_ok ? r : 0)) * ldq + h * AU_HD + hf * 64;
 #pragma unroll
   for (int cc = 0; cc < 2; ++cc) {
@@ -289,12 +316,14 @@ __device__ __forceinline__ void au_tile_unit(AuAux& x, uint8_t* tiles, uint32_t 
   }
   tc_fence_before();
   AU_STAMP(ts + 7);
+  return u_next;
 }
 
 // ---- row unit, the 8 worker warps: (one-row segment seg, head h) - a decode row against its whole context ----
-__device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuArgs& a, int seg, int h, int tid, long long* trace, int ts) {
+__device__ __forceinline__ int au_row_unit(AuAux& x, const AuLists& L, uint8_t* tiles, const AuArgs& a, int seg, int h, bool qk_in_flight,
+                                           const AuNext& nx, int tid, long long* trace, int ts) {
   const int warp = tid >> 5, lane = tid & 31;
-  const int req = x.seg_req[seg], start = x.seg_start[seg], row0 = x.seg_row0[seg], base = x.seg_base[seg];
+  const int req = L.seg_req[seg], start = L.seg_start[seg], row0 = L.seg_row0[seg], base = L.seg_base[seg];
   const int n = start + 1;                      // the row sees positions [0, start]
   const int n16 = (n + 15) & ~15;
   const int ldq = a.H * AU_HD;
@@ -303,9 +332,11 @@ __device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuAr
   const act_t* vbase = a.kv + (static_cast<size_t>(1 * a.R + req) * a.H + h) * head_stride;
   uint8_t* sK = tiles;
   uint8_t* sV = tiles + AU_KV_MAX * (AU_HD * 2);
-  if (tid < 16) cp_async16(x.q + tid * 16, a.q + static_cast<size_t>(row0) * ldq + h * AU_HD + tid * 8, true);
-  au_load_rows_plain(sK, kbase, base, a.C, n16, n, tid);
-  cp_async_commit();
+  if (!qk_in_flight) {     // (else: the previous unit started them, one group)
+    if (tid < 16) cp_async16(x.q + tid * 16, a.q + static_cast<size_t>(row0) * ldq + h * AU_HD + tid * 8, true);
+    au_load_rows_plain(sK, kbase, base, a.C, n16, n, tid);
+    cp_async_commit();
+  }
   au_load_rows_plain(sV, vbase, base, a.C, n, n, tid);
   cp_async_commit();
   AU_STAMP(ts + 0);
@@ -322,28 +353,43 @@ __device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuAr
       qa[kk][2] = g == 0 ? *reinterpret_cast<const uint32_t*>(x.q + (kk * 16 + 8 + 2 * t) * 2) : 0u;
       qa[kk][1] = 0u; qa[kk][3] = 0u;
     }
-    for (int j0 = warp * 16; j0 < n16; j0 += 8 * 16) {
-      float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+    // the warp's (up to) three groups in one pass: three independent accumulator chains instead of three serial ones
+    float s0[3][4], s1[3][4];
 #pragma unroll
-      for (int kk = 0; kk < AU_HD / 16; ++kk) {
-        uint32_t b0, b1, b2, b3;
-        const int r = j0 + (lane & 7) + (lane >> 4) * 8;
-        const int c = kk * 2 + ((lane >> 3) & 1);
-        ldsm_x4(smem_u32(sK + sw_off<AU_HD>(r, c)), b0, b1, b2, b3);
-        mma_f16_16816(s0, qa[kk], b0, b1);
-        mma_f16_16816(s1, qa[kk], b2, b3);
+    for (int gi = 0; gi < 3; ++gi)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { s0[gi][e] = 0.f; s1[gi][e] = 0.f; }
+#pragma unroll
+    for (int kk = 0; kk < AU_HD / 16; ++kk) {
+#pragma unroll
+      for (int gi = 0; gi < 3; ++gi) {
+        const int j0 = (warp + 8 * gi) * 16;
+        if (j0 < n16) {                      // warp-uniform
+          uint32_t b0, b1, b2, b3;
+          const int r = j0 + (lane & 7) + (lane >> 4) * 8;
+          const int c = kk * 2 + ((lane >> 3) & 1);
+          ldsm_x4(smem_u32(sK + sw_off<AU_HD>(r, c)), b0, b1, b2, b3);
+          mma_f16_16816(s0[gi], qa[kk], b0, b1);
+          mma_f16_16816(s1[gi], qa[kk], b2, b3);
+        }
       }
-      if (g == 0) {
-        const int j = j0 + 2 * t;
-        x.sc[j] = j < n ? s0[0] * a.scale_log2 : -INFINITY;
-        x.sc[j + 1] = j + 1 < n ? s0[1] * a.scale_log2 : -INFINITY;
-        x.sc[j + 8] = j + 8 < n ? s1[0] * a.scale_log2 : -INFINITY;
-        x.sc[j + 9] = j + 9 < n ? s1[1] * a.scale_log2 : -INFINITY;
+    }
+#pragma unroll
+    for (int gi = 0; gi < 3; ++gi) {
+      const int j = (warp + 8 * gi) * 16 + 2 * t;
+      if (g == 0 && (warp + 8 * gi) * 16 < n16) {
+        x.sc[j] = j < n ? s0[gi][0] * a.scale_log2 : -INFINITY;
+        x.sc[j + 1] = j + 1 < n ? s0[gi][1] * a.scale_log2 : -INFINITY;
+        x.sc[j + 8] = j + 8 < n ? s1[gi][0] * a.scale_log2 : -INFINITY;
+        x.sc[j + 9] = j + 9 < n ? s1[gi][1] * a.scale_log2 : -INFINITY;
       }
     }
   }
+  if (tid == 0) x.next[nx.slot] = nx.u_t0;
   AU_WORKER_BAR();
   AU_STAMP(ts + 3);
+  const int u_next = x.next[nx.slot];
+  au_row_issue_qk(x, L, tiles, a, u_next, nx, tid);   // this unit's q and K are dead: a following row unit's fly during the softmax and p V
   // ---- softmax over the context: thread t holds positions t and t + 256 ----
   const float x0 = tid < n16 ? x.sc[tid] : -INFINITY;
   const float x1 = tid + AU_WORKERS < n16 ? x.sc[tid + AU_WORKERS] : -INFINITY;
@@ -363,7 +409,7 @@ __device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuAr
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
   if (lane == 0) x.red[8 + warp] = sum;
-  cp_async_wait<0>();
+  cp_async_wait<1>();      // V (the look-ahead group may still be in flight)
   AU_WORKER_BAR();
   AU_STAMP(ts + 5);
   float l = x.red[8];
@@ -373,7 +419,19 @@ __device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuAr
   {
     const int cp = tid & 63, sub = tid >> 6;
     float a0 = 0.f, a1 = 0.f;
-    for (int j = sub; j < n; j += 4) {
+    int j = sub;
+    for (; j + 12 < n; j += 16) {      // four positions in flight (loads first), added in position order
+      float pj[4];
+      float2 vv[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        pj[i] = x.sc[j + 4 * i];
+        vv[i] = __half22float2(*reinterpret_cast<const __half2*>(sV + sw_off<AU_HD>(j + 4 * i, cp >> 2) + (cp & 3) * 4));
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { a0 = fmaf(pj[i], vv[i].x, a0); a1 = fmaf(pj[i], vv[i].y, a1); }
+    }
+    for (; j < n; j += 4) {
       const float pj = x.sc[j];
       const float2 vv = __half22float2(*reinterpret_cast<const __half2*>(sV + sw_off<AU_HD>(j, cp >> 2) + (cp & 3) * 4));
       a0 = fmaf(pj, vv.x, a0); a1 = fmaf(pj, vv.y, a1);
@@ -388,54 +446,57 @@ __device__ __forceinline__ void au_row_unit(AuAux& x, uint8_t* tiles, const AuAr
     *reinterpret_cast<uint32_t*>(a.out + static_cast<size_t>(row0) * ldq + h * AU_HD + 2 * tid) = pack_act(o0 * inv, o1 * inv);
   }
   AU_STAMP(ts + 7);
+  return u_next;
 }
 
-// The worker warps' side of a CTA (tid 0..255): segment table -> unit lists, then this CTA's units.  Tensor units come
-// first (the longest).  With a.sched the CTA starts with unit `cta` and pops every further one from a counter - at the START
-// of the current unit, so the atomic's round trip is hidden; otherwise it takes units cta, cta + n_cta, ...  Which CTA runs a
-// unit does not change its result.
-__device__ __forceinline__ void au_workers(AuAux& x, uint8_t* tiles, uint32_t tmem, const AuArgs& a, int cta, int n_cta, int tid) {
-  long long* trace = a.trace;
-  AU_STAMP(0);
-  for (int s = tid; s < a.n_segs; s += AU_WORKERS) {
-    x.seg_req[s] = a.tb.seg_req[s]; x.seg_start[s] = a.tb.seg_start[s]; x.seg_len[s] = a.tb.seg_len[s];
-    x.seg_row0[s] = a.tb.seg_row0[s]; x.seg_base[s] = a.tb.seg_base[s];
+// Segment table -> unit lists, by `nthr` threads (a multiple of 32) that meet at named barrier `bar_id`: (segment, query
+// tile) of every multi-row segment, longest context first, and the one-row segments.
+__device__ __forceinline__ void au_build_lists(AuLists& L, const StepTables& tb, int n_segs, int tid) {
+  for (int s = tid; s < n_segs; s += AU_WORKERS) {
+    L.seg_req[s] = tb.seg_req[s]; L.seg_start[s] = tb.seg_start[s]; L.seg_len[s] = tb.seg_len[s];
+    L.seg_row0[s] = tb.seg_row0[s]; L.seg_base[s] = tb.seg_base[s];
   }
   AU_WORKER_BAR();
-  if (tid == 0) {   // (segment, query tile) of every multi-row segment, longest context first; the one-row segments
+  if (tid == 0) {
     int n_it = 0, n_dec = 0;
-    for (int s = 0; s < a.n_segs; ++s) {
-      const int len = x.seg_len[s];
-      if (len == 1) { x.dec_seg[n_dec++] = s; continue; }
-      for (int q0 = ((len - 1) / AU_BQ) * AU_BQ; q0 >= 0 && n_it < AU_MAX_ITEMS; q0 -= AU_BQ) { x.it_seg[n_it] = s; x.it_q0[n_it] = q0; ++n_it; }
+    for (int s = 0; s < n_segs; ++s) {
+      const int len = L.seg_len[s];
+      if (len == 1) { L.dec_seg[n_dec++] = s; continue; }
+      for (int q0 = ((len - 1) / AU_BQ) * AU_BQ; q0 >= 0 && n_it < AU_MAX_ITEMS; q0 -= AU_BQ) { L.it_seg[n_it] = s; L.it_q0[n_it] = q0; ++n_it; }
     }
-    x.cnt[0] = n_it; x.cnt[1] = n_dec;
+    L.cnt[0] = n_it; L.cnt[1] = n_dec;
   }
   AU_WORKER_BAR();
+}
+
+// The worker warps' side of a CTA (tid 0..255), lists built: this CTA's units.  Tensor units come first (the longest).
+// With a.sched the CTA starts with unit `cta` and pops every further one from a counter - at the START of the current
+// unit, so the atomic's round trip is hidden; otherwise it takes units cta, cta + n_cta, ...  Which CTA runs a unit does not
+// change its result.
+__device__ __forceinline__ void au_workers(AuAux& x, const AuLists& L, uint8_t* tiles, uint32_t tmem, const AuArgs& a, int cta, int n_cta, int tid) {
+  long long* trace = a.trace;
   AU_STAMP(1);
-  const int n_mm = x.cnt[0] * a.H, n_units = n_mm + x.cnt[1] * a.H;
+  const int n_mm = L.cnt[0] * a.H, n_units = n_mm + L.cnt[1] * a.H;
   int n_done = 0;
   uint32_t par = 0;   // phase parity of the tensor units' mbarriers (each completes once per tensor unit)
   int u = cta;
+  bool qk_in_flight = false;   // the current (row) unit's q + K loads were started by the previous unit
   while (u < n_units) {
-    int u_next = u + n_cta;
-    if (a.sched && tid == 0) u_next = n_cta + atomicAdd(&a.sched[0], 1);
+    AuNext nx;
+    nx.u_t0 = u + n_cta; nx.slot = n_done & 1; nx.n_mm = n_mm; nx.n_units = n_units;
+    if (a.sched && tid == 0) nx.u_t0 = n_cta + atomicAdd(&a.sched[0], 1);
+    int u_next;
     if (u < n_mm) {
       const int it = u / a.H;
-      au_tile_unit(x, tiles, tmem, a, x.it_seg[it], x.it_q0[it], u - it * a.H, par, tid, trace, 2 + 8 * n_done);
+      u_next = au_tile_unit(x, L, tiles, tmem, a, L.it_seg[it], L.it_q0[it], u - it * a.H, par, nx, tid, trace, 2 + 8 * n_done);
       par ^= 1u;
     } else {
       const int k = (u - n_mm) / a.H;
-      au_row_unit(x, tiles, a, x.dec_seg[k], (u - n_mm) - k * a.H, tid, trace, 2 + 8 * n_done);
+      u_next = au_row_unit(x, L, tiles, a, L.dec_seg[k], (u - n_mm) - k * a.H, qk_in_flight, nx, tid, trace, 2 + 8 * n_done);
     }
-    if (a.sched) {
-      if (tid == 0) x.next[n_done & 1] = u_next;
-      AU_WORKER_BAR();
-      u = x.next[n_done & 1];
-    } else {
-      AU_WORKER_BAR();   // the unit's shared-memory reads are over before the next unit's loads
-      u = u_next;
-    }
+    AU_WORKER_BAR();   // the unit's shared-memory reads (V, the partial sums) are over before the next unit's loads
+    qk_in_flight = u_next >= n_mm && u_next < n_units;
+    u = u_next;
     ++n_done;
   }
   if (tid == 0) x.kvp[par] = 0;   // tell the MMA thread there is no further tensor unit
@@ -449,6 +510,7 @@ attention_umma_kernel(const AuArgs a) {
   extern __shared__ uint8_t au_smem_raw[];
   uint8_t* tiles = au_smem_raw + ((1024u - (smem_u32(au_smem_raw) & 1023u)) & 1023u);
   __shared__ AuAux x;
+  __shared__ AuLists lists;
   __shared__ uint32_t s_tmem;
   const int tid = threadIdx.x, warp = tid >> 5;
   if (warp == 8) tmem_alloc(&s_tmem, AU_TMEM_COLS);
@@ -462,7 +524,12 @@ attention_umma_kernel(const AuArgs a) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = s_tmem;
-  if (warp < 8) au_workers(x, tiles, tmem, a, blockIdx.x, gridDim.x, tid);
+  if (warp < 8) {
+    long long* trace = a.trace;
+    AU_STAMP(0);
+    au_build_lists(lists, a.tb, a.n_segs, tid);
+    au_workers(x, lists, tiles, tmem, a, blockIdx.x, gridDim.x, tid);
+  }
   else if (tid == AU_WORKERS) au_mma_loop(x, tiles, tmem);
   tc_fence_before();
   __syncthreads();

@@ -300,11 +300,13 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
 // CH_ATTN on the 8 epilogue warps (a function of its own: its register allocation is independent of the GEMM epilogue's)
 // (the shared-memory pointers are rebuilt from the dynamic allocation here, not passed in: through a call boundary they would
 // be generic pointers and every P store / table read a generic access; the arguments travel by value)
-__device__ __noinline__ void chain_attn_phase(uint32_t tmem, const AuArgs a, int cta, int n_cta, int tid) {
+__device__ __noinline__ void chain_attn_phase(uint32_t tmem, const AuArgs a, const AuLists* lists, int cta, int n_cta, int tid) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   AuAux* x = reinterpret_cast<AuAux*>(tiles + AU_TILE_BYTES);
-  au_workers(*x, tiles, tmem, a, cta, n_cta, tid);
+  long long* trace = a.trace;
+  AU_STAMP(0);
+  au_workers(*x, *lists, tiles, tmem, a, cta, n_cta, tid);
 }
 
 // kTwo: 512 < T <= 1024, two token chunks per piece (ChainArgs::T0); a separate instantiation so that the one-chunk kernel
@@ -330,6 +332,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
   __shared__ int deps_done;                         // grid barriers this CTA has passed (published to the producer)
   __shared__ float row_red[CH_ROW_GROUPS][4];
   __shared__ int s_pair_slabs[64];
+  __shared__ AuLists att_lists;                     // CH_ATTN: the step's unit lists, built at kernel start
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cta = blockIdx.x, n_cta = gridDim.x;
@@ -527,6 +530,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
       if (a.ph[ph].kind == CH_ROPE)
         for (int i = etid; i < 3 * a.D / (2 * GEMM_BM) && i < 64; i += GEMM_EPI_WARPS * 32) s_pair_slabs[i] = __ldg(a.ph[ph].pair_slabs + i);
     AF_EPI_BAR();
+    if (a.att_on) au_build_lists(att_lists, a.att.tb, a.att.n_segs, etid);   // (the warps would wait for the first accumulator anyway)
     uint32_t acc_phase = 0, cphase = 0;
     int n_bar = 0, cstage = 0, cunit = 0;
 
@@ -751,7 +755,7 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         chain_rope_phase(reinterpret_cast<const act_t*>(P.src), P.slab_stride, P.q_out, P.kv_layer, a.tb.row_pos, a.tb.row_slot,
                          a.rope_tab, a.H, a.hd, a.R, a.C, a.D, a.T, s_pair_slabs, cta, n_cta, warp, lane);
       } else {
-        chain_attn_phase(tmem_base, a.att, cta, n_cta, etid);
+        chain_attn_phase(tmem_base, a.att, &att_lists, cta, n_cta, etid);
       }
       if (etid == 0 && trace) trace[1 + 2 * ph] = static_cast<long long>(globaltimer_ns());
       // ---- grid barrier: everything this phase wrote is visible to every CTA before the next phase reads it ----

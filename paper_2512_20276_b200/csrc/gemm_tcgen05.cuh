@@ -68,7 +68,7 @@ constexpr int GEMM_MAX_TOK = 512;  // tokens per launch: one UMMA N <= 256, or t
 constexpr int GEMM_TMEM_COLS = 512;
 constexpr int GEMM_MAX_STAGES = 12;
 constexpr int GEMM_XCH_MAX = GEMM_EPI_WARPS * 8192;  // per epilogue warp: two 4 KB (or one 2 KB) staging buffers for TMA stores
-constexpr int GEMM_SMEM_BUDGET = 232448 - 1024;    // dynamic shared memory: 227 KB minus the static part
+constexpr int GEMM_SMEM_BUDGET = 232448 - 1024 - 2304;   // dynamic shared memory: 227 KB minus the static part (layer_chain_kernel: + AuLists)
 
 enum GemmEpilogue : int { EPI_STORE = 0, EPI_SWIGLU = 1 };
 enum GemmSplit : int { SPLIT_STREAMK = 0, SPLIT_K = 1 };
