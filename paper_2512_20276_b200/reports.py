@@ -5,6 +5,7 @@
     python -m paper_2512_20276_b200.reports --sweep --fp8              the same points with AF_WEIGHTS_FP8
     python -m paper_2512_20276_b200.reports --chain-timeline           per-phase timeline of layer_chain_kernel launches
     python -m paper_2512_20276_b200.reports --library-gemm             cuBLAS on the step's projection shapes (context)
+    python -m paper_2512_20276_b200.reports --attention-units          the tcgen05 attention units: timeline and step A/B
 """
 from __future__ import annotations
 
@@ -195,6 +196,81 @@ def run_sweep(args):
 
 
 
+def run_attention_units(args):
+    """The tcgen05 attention units (attention_umma.cuh, af_debug_attention(2)) as the layer chain's last phase: (a) the
+    units' %globaltimer stamps (af_debug_trace(2)) for the steady cfg3 step on a 3-layer slice, by CTA group - CTAs 0..31
+    start with the 20-row query tile (276 keys), 32..63 with rows 128..255, 64..95 with rows 0..127, 96..147 with decode
+    rows; (b) the steady cfg3 step at --layers layers, attention_kernel (mode 1) against the units (mode 2), alternating in
+    one process, CUDA events over 40 steps each."""
+    import numpy as np
+    import torch
+    from . import binding, inputs as I
+    torch.cuda.set_device(0)
+
+    def make(layers):
+        cfg = I.cfg_7b_layers(layers)
+        W = binding.Weights(cfg, I.make_weights(cfg, SEED, threads=16))
+        ring = binding.Ring(cfg, R_REGIONS, CAPACITY, max_rows=288)
+        e_dev = [I.make_embeds(cfg, SEED, t, L_P + K_STAGES - 1).cuda() for t in range(8)]
+        tau = [0]
+
+        def step():
+            t = tau[0]
+            ring.reset_slot(t % R_REGIONS, -1)
+            segs = I.steady_schedule(t, L_P, K_STAGES, R_REGIONS)
+            ring.packed_forward(W, e_dev[t % 8][:I.total_rows(segs)], segs)
+            tau[0] = t + 1
+        return step
+
+    binding.attention_mode(2)
+    step = make(3)
+    for _ in range(12):
+        step()
+    torch.cuda.synchronize()
+    binding.chain_trace(2)
+    step()
+    st, meta, n = binding.chain_trace_read()
+    binding.chain_trace(0)
+    names = ["phase start", "lists", "1st unit: loads issued", "first chunk / K landed", "all landed", "S done / scores", "row maximum",
+             "P written / probabilities", "O done", "unit end", "2nd unit: loads issued", "K landed", "-", "scores", "maximum",
+             "probabilities", "-", "unit end"]
+    print("(a) stamps of worker thread 0, us after the phase's first CTA started, mean over the CTA group; launches:", n)
+    for li in range(min(n, 2)):
+        s = st[li, :int(meta[li][1])].astype(np.float64)
+        t0 = s[:, 0][s[:, 0] > 0].min()
+        print(f"\nlaunch {li}: last stamp {(s.max() - t0) / 1e3:.1f} us\n| stamp | CTAs 0-31 | CTAs 32-63 | CTAs 64-95 | CTAs 96-147 |\n|---|---|---|---|---|")
+        for k in range(18):
+            cells = []
+            for lo, hi in ((0, 32), (32, 64), (64, 96), (96, 148)):
+                col = s[lo:hi, k]
+                col = col[col > 0]
+                cells.append(f"{(col.mean() - t0) / 1e3:.1f}" if len(col) else "-")
+            if names[k] != "-":
+                print(f"| {names[k]} | " + " | ".join(cells) + " |")
+    del step
+    step = make(args.layers)
+    for _ in range(K_STAGES + 10):
+        step()
+    res = {1: [], 2: []}
+    for _ in range(4):
+        for mode in (1, 2):
+            binding.attention_mode(mode)
+            for _ in range(5):
+                step()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(40):
+                step()
+            e1.record()
+            torch.cuda.synchronize()
+            res[mode].append(e0.elapsed_time(e1) / 40)
+    binding.attention_mode(0)
+    print(f"\n(b) steady cfg3 step, {args.layers} layers, ms per step (no LM head), four alternating repetitions:")
+    print("attention_kernel (mma.sync, own launches):", " ".join(f"{x:.3f}" for x in res[1]))
+    print("tcgen05 units (last phase of the chain):  ", " ".join(f"{x:.3f}" for x in res[2]))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=20)
@@ -204,11 +280,14 @@ def main():
     ap.add_argument("--fp8", action="store_true", help="AF_WEIGHTS_FP8 instead of the 16-bit weights")
     ap.add_argument("--chain-timeline", action="store_true")
     ap.add_argument("--library-gemm", action="store_true")
+    ap.add_argument("--attention-units", action="store_true")
     args = ap.parse_args()
     if args.library_gemm:
         return run_library_gemm(args)
     if args.chain_timeline:
         return run_chain_timeline(args)
+    if args.attention_units:
+        return run_attention_units(args)
     return run_sweep(args)
 
 
