@@ -201,7 +201,8 @@ def run_attention_units(args):
     units' %globaltimer stamps (af_debug_trace(2)) for the steady cfg3 step on a 3-layer slice, by CTA group - CTAs 0..31
     start with the 20-row query tile (276 keys), 32..63 with rows 128..255, 64..95 with rows 0..127, 96..147 with decode
     rows; (b) the steady cfg3 step at --layers layers, attention_kernel (mode 1) against the units (mode 2), alternating in
-    one process, CUDA events over 40 steps each."""
+    one process, CUDA events over 40 steps each.  --own-kernel: the per-stage path (AF_WEIGHTS_FP16), where the units run
+    as attention_umma_kernel - the command the ncu capture of that kernel uses."""
     import numpy as np
     import torch
     from . import binding, inputs as I
@@ -209,7 +210,7 @@ def run_attention_units(args):
 
     def make(layers):
         cfg = I.cfg_7b_layers(layers)
-        W = binding.Weights(cfg, I.make_weights(cfg, SEED, threads=16))
+        W = binding.Weights(cfg, I.make_weights(cfg, SEED, threads=16), prepared="fp16" if args.own_kernel else True)
         ring = binding.Ring(cfg, R_REGIONS, CAPACITY, max_rows=288)
         e_dev = [I.make_embeds(cfg, SEED, t, L_P + K_STAGES - 1).cuda() for t in range(8)]
         tau = [0]
@@ -281,6 +282,7 @@ def main():
     ap.add_argument("--chain-timeline", action="store_true")
     ap.add_argument("--library-gemm", action="store_true")
     ap.add_argument("--attention-units", action="store_true")
+    ap.add_argument("--own-kernel", action="store_true", help="with --attention-units: the per-stage path, units as attention_umma_kernel")
     args = ap.parse_args()
     if args.library_gemm:
         return run_library_gemm(args)
