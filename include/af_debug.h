@@ -32,11 +32,13 @@ int af_debug_gemm(const void* a, const void* w, float* out, int32_t n_tok, int32
  * layer chain, so that every stage has a class of its own; 0: off.
  * af_debug_profile_read synchronises, returns summed milliseconds and launch counts since the last read, and clears. */
 int af_debug_profile(int enable);
-/* Which kernel runs the attention stage (a4).  mode 0 (default) / 1: attention_kernel (mma.sync; any head_dim, window,
- * context).  mode 2: the tcgen05 units of attention_umma.cuh wherever they apply - head_dim 128, no window, every segment's
- * context <= 352 - as the last phase of the layer chain, or as attention_umma_kernel on the per-stage path; other steps
- * still take attention_kernel.  Measured slower per step than mode 0 at BASELINE.json's configs, hence not the
- * default.  Process-wide; takes effect at the next af_packed_forward / captured graph. */
+/* Which kernel runs the attention stage (a4).  The units of attention_umma.cuh (tensor units on tcgen05 for multi-row
+ * segments, row units for one-row segments; head_dim 128, no window, every segment's context <= 352) run as the last phase
+ * of the layer chain, or as attention_umma_kernel on the per-stage path; attention_kernel (mma.sync; any head_dim, window,
+ * context) is a kernel of its own.  mode 0 (default): the units for steps made of one-row segments only (decode-only
+ * steps, where they are 2-4 % faster per step), attention_kernel for every other step (1.5 % faster there).
+ * mode 1: attention_kernel always.  mode 2: the units wherever they apply.  Process-wide; takes effect at the next
+ * af_packed_forward / captured graph. */
 int af_debug_attention(int mode);
 int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
 

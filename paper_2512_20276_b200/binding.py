@@ -321,7 +321,8 @@ def profile(enable: bool):
 
 
 def attention_mode(mode: int):
-    """af_debug_attention: 0 / 1 = attention_kernel (mma.sync), 2 = the tcgen05 units of attention_umma.cuh where they apply."""
+    """af_debug_attention: 0 = automatic (units for decode-only steps), 1 = attention_kernel (mma.sync) always, 2 = the units
+    of attention_umma.cuh wherever they apply."""
     L = load_library()
     L.af_debug_attention.argtypes, L.af_debug_attention.restype = [C.c_int], C.c_int
     _check(L.af_debug_attention(int(mode)))

@@ -62,7 +62,7 @@ struct ProfScope {
   }
   ~ProfScope() { if (on) { cudaEventRecord(r.b, st); g_prof.push_back(r); } }
 };
-static int g_att_mode = 0;   // af_debug_attention: 0 / 1 attention_kernel (mma.sync); 2 the tcgen05 units of attention_umma.cuh where they apply
+static int g_att_mode = 0;   // af_debug_attention: 0 automatic, 1 attention_kernel (mma.sync) always, 2 the units of attention_umma.cuh wherever they apply
 extern "C" int af_debug_attention(int mode) {
   if (mode < 0 || mode > 2) return fail(AF_ERR_ARG, "af_debug_attention: mode %d outside [0,2]", mode);
   g_att_mode = mode;
@@ -1069,7 +1069,7 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   const float scale_log2 = 1.4426950408889634f / sqrtf(static_cast<float>(hd));
   const size_t layer_elems = static_cast<size_t>(2) * R * H * C * hd;
   // a4 on tcgen05 (attention_umma.cuh) when every segment's context fits one unit; attention_kernel otherwise
-  bool att_umma = g_att_mode == 2 && hd == AU_HD && g->window == 0;
+  bool att_umma = g_att_mode != 1 && hd == AU_HD && g->window == 0;
   int au_items = 0, au_rows = 0;
   for (int s = 0; s < n_segs; ++s) {
     if (segs[s].start_pos + segs[s].len > AU_KV_MAX) att_umma = false;
@@ -1077,6 +1077,9 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
     else au_items += (segs[s].len + AU_BQ - 1) / AU_BQ;
   }
   if (au_items > AU_MAX_ITEMS) att_umma = false;
+  // default (mode 0): the units take the steps made of one-row segments only (decode-only steps: 2-4 % faster per step,
+  // DESIGN.md 6.2b); a step with a multi-row segment is 1.5 % faster with attention_kernel as a kernel of its own
+  if (g_att_mode == 0 && au_items > 0) att_umma = false;
   const int au_units = (au_items + au_rows) * H;
   auto attn_args = [&](int l) {
     AuArgs aa{};

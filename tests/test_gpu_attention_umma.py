@@ -115,3 +115,21 @@ def test_units_are_deterministic(binding, w2):
             hid = ring.packed_forward(W, I.make_embeds(cfg, 5, t, I.total_rows(segs)).cuda(), segs)
         outs.append(hid.clone())
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+
+
+def test_default_mode_takes_the_units_for_decode_only_steps(binding):
+    """Mode 0 (the default): a step made of one-row segments only runs the units as the chain's last phase - one launch
+    fewer per layer than with attention_kernel - and a step with a multi-row segment does not.  Decode-only steps at contexts
+    100..105 and 300..305 against the fp32 oracle, ring checked."""
+    cfg = I.CFG_7B_1L
+    hw = I.make_weights(cfg, seed=6)
+    binding.attention_mode(0)
+    P = Pair(cfg, hw, R=4, C=384, max_rows=400, bases=[380, 17, 200, 0], oracle_dtype=torch.float32)
+    n0 = binding.launch_count()
+    P.step([(0, 0, 0, 100), (1, 0, 0, 300)], I.make_embeds(cfg, 6, 0, 400))
+    prefill_launches = binding.launch_count() - n0
+    for t in range(6):
+        n0 = binding.launch_count()
+        P.step([(0, 1, 100 + t, 1), (1, 1, 300 + t, 1)], I.make_embeds(cfg, 6, 1 + t, 2))
+        assert binding.launch_count() - n0 == prefill_launches - cfg.n_layers
+    P.check_ring([0, 1])
