@@ -1,11 +1,12 @@
-// Segment-masked causal attention over the Unified KV Ring Buffer (step a4; Alg. 2 line 4) on the
-// 5th-generation tensor cores: the kernel the packed step of the paper's schedule runs (one multi-row prefill segment
-// plus one-row decode segments, contexts of a few hundred positions).  attention_kernel (attention.cuh) stays for
-// everything this one does not take: head_dim != 128, a sliding window, contexts beyond AU_KV_MAX.
+// Segment-masked causal attention over the Unified KV Ring Buffer (step a4; Alg. 2 line 4) as UNITS that
+// run on the warps of a persistent one-CTA-per-SM kernel: the last phase of layer_chain_kernel (chain.cuh), or
+// attention_umma_kernel below on the per-stage path.  For head_dim 128, no window and contexts <= AU_KV_MAX; attention_kernel
+// (attention.cuh) takes every other step - and, by default, the steps with a multi-row segment (there the
+// units are 1.5 % slower per step; decode-only steps are 2-4 % faster with them).
 //
 // Why: on mma.sync a query strip walks its KV tiles one after another - ~2 us per tile step of cp.async wait + block
-// barriers + a dependent chain, 9 steps for the last strip of a 276-row prefill - and the launch takes 20 us for 0.6 GFLOP.
-// Here a unit's WHOLE score matrix fits the tensor memory, so there is no walk:
+// barriers + a dependent chain, 9 steps for the last strip of a 276-row prefill.  Here a unit's WHOLE score matrix fits the
+// tensor memory, so there is no walk:
 //
 //   tensor unit (segment with > 1 row, 128-row query tile, head):  Q, K, V of the visible positions -> shared memory
 //       (cp.async per row: ring wrap and zero fill for free, in the 128-byte-swizzle layout UMMA reads);
@@ -15,12 +16,12 @@
 //       O = P V     tcgen05.mma with V as the MN-major B operand (the ring stores [position][head_dim]: no transpose);
 //       out = O / l TMEM -> registers -> fp16 rows.
 //   row unit (one-row segment, head): the decode rows.  K and V of the whole context -> shared memory, q K^T on
-//       mma.sync (1 of 16 rows used; 35 instructions per warp), softmax over the context by the block, p V on FMAs with
-//       fp32 probabilities (thread = two output columns x a quarter of the positions).
+//       mma.sync (1 of 16 rows used; three 16-position groups per warp in flight), softmax over the context by the block,
+//       p V on FMAs with fp32 probabilities (thread = two output columns x a quarter of the positions).
 //
-// Persistent grid, one CTA per SM (208 KB of tiles): CTA c starts with unit c and pops further units from a counter;
-// tensor units come first (the longest).  Every reduction order is fixed and positions are walked in LOGICAL order: results do not depend on
-// base_r, on the grid size or on timing.
+// CTA c starts with unit c and pops further units from a counter; tensor units come first (the longest).  Every reduction
+// order is fixed and positions are walked in LOGICAL order: results do not depend on base_r, on the grid size, on which CTA
+// ran a unit or on timing.
 #pragma once
 #include "attention.cuh"
 
