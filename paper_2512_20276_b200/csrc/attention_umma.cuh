@@ -120,6 +120,7 @@ struct AuLists {
 // dynamic allocation (behind the tiles) in layer_chain_kernel.
 struct AuAux {
   uint64_t bar_k[3], bar_v, bar_s, bar_p, bar_o;   // K chunks / V landed (256 arrivals), S done (commit), P written (256), O done (commit)
+  uint64_t bar_rv;                                 // row units: V landed (bulk copies, complete_tx)
   int kvp[2];                                      // N extent of the tensor unit the MMA thread runs next, by barrier parity; 0 = no more units
   int next[2];                                     // the CTA's next unit (double-buffered across units)
   float sc[AU_KV_MAX];                             // row units: scores, then probabilities
@@ -144,6 +145,7 @@ __device__ __forceinline__ void au_init_barriers(AuAux& x) {   // one thread, be
   mbar_init(&x.bar_s, 1);
   mbar_init(&x.bar_p, AU_WORKERS);
   mbar_init(&x.bar_o, 1);
+  mbar_init(&x.bar_rv, 1);
 }
 
 // The MMA-issuing thread of a CTA: one pass per tensor unit of the worker warps, in their order; it learns a unit's extent
@@ -322,7 +324,7 @@ __device__ __forceinline__ int au_tile_unit(AuAux& x, const AuLists& L, uint8_t*
 
 // ---- row unit, the 8 worker warps: (one-row segment seg, head h) - a decode row against its whole context ----
 __device__ __forceinline__ int au_row_unit(AuAux& x, const AuLists& L, uint8_t* tiles, const AuArgs& a, int seg, int h, bool qk_in_flight,
-                                           const AuNext& nx, int tid, long long* trace, int ts) {
+                                           uint32_t rpar, const AuNext& nx, int tid, long long* trace, int ts) {
   const int warp = tid >> 5, lane = tid & 31;
   const int req = L.seg_req[seg], start = L.seg_start[seg], row0 = L.seg_row0[seg], base = L.seg_base[seg];
   const int n = start + 1;                      // the row sees positions [0, start]
@@ -338,10 +340,17 @@ __device__ __forceinline__ int au_row_unit(AuAux& x, const AuLists& L, uint8_t* 
     au_load_rows_plain(sK, kbase, base, a.C, n16, n, tid);
     cp_async_commit();
   }
-  au_load_rows_plain(sV, vbase, base, a.C, n, n, tid);
-  cp_async_commit();
+  // V: plain [position][256 B] rows, read row by row in p V - no swizzle needed, so the ring range goes in as one or two
+  // bulk copies (the wrap) instead of 4.6 k cp.async, and the LSU queue is K's alone
+  if (tid == 0) {
+    fence_proxy_async();      // the previous unit's generic reads of this buffer (ordered by the block barrier) before the async writes
+    const int n1 = min(n, a.C - base);
+    mbar_arrive_expect_tx(&x.bar_rv, static_cast<uint32_t>(n) * (AU_HD * 2));
+    bulk_load_1d(sV, vbase + static_cast<size_t>(base) * AU_HD, static_cast<uint32_t>(n1) * (AU_HD * 2), &x.bar_rv);
+    if (n1 < n) bulk_load_1d(sV + n1 * (AU_HD * 2), vbase, static_cast<uint32_t>(n - n1) * (AU_HD * 2), &x.bar_rv);
+  }
   AU_STAMP(ts + 0);
-  cp_async_wait<1>();
+  cp_async_wait<0>();
   AU_WORKER_BAR();
   AU_STAMP(ts + 1);
   // ---- scores: q K^T on mma.sync, the query in row 0 of the A fragment; warp w takes 16-position groups w, w + 8, .. ----
@@ -410,7 +419,7 @@ __device__ __forceinline__ int au_row_unit(AuAux& x, const AuLists& L, uint8_t* 
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
   if (lane == 0) x.red[8 + warp] = sum;
-  cp_async_wait<1>();      // V (the look-ahead group may still be in flight)
+  mbar_wait(&x.bar_rv, rpar);   // V has landed
   AU_WORKER_BAR();
   AU_STAMP(ts + 5);
   float l = x.red[8];
@@ -427,14 +436,14 @@ __device__ __forceinline__ int au_row_unit(AuAux& x, const AuLists& L, uint8_t* 
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         pj[i] = x.sc[j + 4 * i];
-        vv[i] = __half22float2(*reinterpret_cast<const __half2*>(sV + sw_off<AU_HD>(j + 4 * i, cp >> 2) + (cp & 3) * 4));
+        vv[i] = __half22float2(*reinterpret_cast<const __half2*>(sV + (j + 4 * i) * (AU_HD * 2) + cp * 4));
       }
 #pragma unroll
       for (int i = 0; i < 4; ++i) { a0 = fmaf(pj[i], vv[i].x, a0); a1 = fmaf(pj[i], vv[i].y, a1); }
     }
     for (; j < n; j += 4) {
       const float pj = x.sc[j];
-      const float2 vv = __half22float2(*reinterpret_cast<const __half2*>(sV + sw_off<AU_HD>(j, cp >> 2) + (cp & 3) * 4));
+      const float2 vv = __half22float2(*reinterpret_cast<const __half2*>(sV + j * (AU_HD * 2) + cp * 4));
       a0 = fmaf(pj, vv.x, a0); a1 = fmaf(pj, vv.y, a1);
     }
     x.part[sub][2 * cp] = a0; x.part[sub][2 * cp + 1] = a1;
@@ -480,6 +489,7 @@ __device__ __forceinline__ void au_workers(AuAux& x, const AuLists& L, uint8_t* 
   const int n_mm = L.cnt[0] * a.H, n_units = n_mm + L.cnt[1] * a.H;
   int n_done = 0;
   uint32_t par = 0;   // phase parity of the tensor units' mbarriers (each completes once per tensor unit)
+  uint32_t rpar = 0;  // ... of the row units' V barrier
   int u = cta;
   bool qk_in_flight = false;   // the current (row) unit's q + K loads were started by the previous unit
   while (u < n_units) {
@@ -493,7 +503,8 @@ __device__ __forceinline__ void au_workers(AuAux& x, const AuLists& L, uint8_t* 
       par ^= 1u;
     } else {
       const int k = (u - n_mm) / a.H;
-      u_next = au_row_unit(x, L, tiles, a, L.dec_seg[k], (u - n_mm) - k * a.H, qk_in_flight, nx, tid, trace, 2 + 8 * n_done);
+      u_next = au_row_unit(x, L, tiles, a, L.dec_seg[k], (u - n_mm) - k * a.H, qk_in_flight, rpar, nx, tid, trace, 2 + 8 * n_done);
+      rpar ^= 1u;
     }
     AU_WORKER_BAR();   // the unit's shared-memory reads (V, the partial sums) are over before the next unit's loads
     qk_in_flight = u_next >= n_mm && u_next < n_units;
