@@ -212,6 +212,7 @@ __device__ __noinline__ void chain_rows_phase(float* __restrict__ x, const void*
 // sum of the QKV projection's slabs (slab counts per 256-feature tile pair in s_pair_slabs); q and k are rotated at the
 // row's logical position in its own request (rotate-half pairing, table built in fp64); q goes to q_out, k and v straight
 // to the row's ring slot.
+template <bool kSplit>   // kSplit: fewer rows than row groups - a separate instantiation, the full-width step's code is untouched
 __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, long long slab_stride, act_t* __restrict__ q_out,
                                               act_t* __restrict__ kv_layer, const int* __restrict__ row_pos,
                                               const int* __restrict__ row_slot, const float2* __restrict__ rope_tab, int H, int hd,
@@ -219,13 +220,20 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
   const int grp = warp >> 2, gl = (warp & 3) * 32 + lane;
   const int half = hd >> 1, per_head = half / 8;
   const int n_qk = 2 * H * per_head, n_v = D / 8;
-  for (int i = cta * CH_ROW_GROUPS + grp; i < T; i += CH_ROW_GROUPS * n_cta) {
+  // A row's items are walked 256 at a time (two per lane, every load in flight before the first use): D / 2048 passes for
+  // q | k plus as many for v, each an L2 round trip.  With fewer rows than row groups (decode-only steps, short prefills) a
+  // row is split over up to 4 groups, each taking every n_parts-th pass.
+  const int n_grp = CH_ROW_GROUPS * n_cta;
+  const int n_parts = kSplit ? min(4, n_grp / T) : 1;
+  const int qk_passes = (n_qk + 255) / 256;
+  for (int unit = cta * CH_ROW_GROUPS + grp; unit < T * n_parts; unit += n_grp) {
+    const int i = unit / n_parts, part = unit - i * n_parts;
     const int pos = __ldg(row_pos + i), gslot = __ldg(row_slot + i);
     const int req = gslot / C, slot = gslot - req * C;
     const act_t* src = qkv + static_cast<size_t>(i) * 3 * D;
     const float2* tab = rope_tab + static_cast<size_t>(pos) * half;
     const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
-    for (int w0 = gl; w0 < n_qk; w0 += 256) {           // q, k: two (head, 8-element) items per lane at a time
+    for (int w0 = gl + 256 * part; w0 < n_qk; w0 += 256 * n_parts) {   // q, k: two (head, 8-element) items per lane at a time
       uint4 rlo[2][QKV_MAX_SLABS_K], rhi[2][QKV_MAX_SLABS_K];
       float4 cs[2][4];
       int colv[2], hv[2], cv[2];
@@ -270,7 +278,8 @@ __device__ __noinline__ void chain_rope_phase(const act_t* __restrict__ qkv, lon
         }
       }
     }
-    for (int w0 = gl; w0 < n_v; w0 += 256) {          // v: two 8-element items per lane at a time
+    const int v_first = ((part - qk_passes) % n_parts + n_parts) % n_parts;   // v's pass k is pass qk_passes + k of the row
+    for (int w0 = gl + 256 * v_first; w0 < n_v; w0 += 256 * n_parts) {   // v: two 8-element items per lane at a time
       uint4 rv[2][QKV_MAX_SLABS_K];
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
@@ -752,8 +761,12 @@ layer_chain_kernel(const __grid_constant__ ChainArgs a) {
         if (P.embed) chain_rows_phase<true>(a.x, P.src, 0, 0, P.gain, P.xn, a.D, a.eps, a.T, row_red, cta, n_cta, warp, lane);
         else chain_rows_phase<false>(a.x, P.src ? P.src : a.x, ns, P.slab_stride, P.gain, P.xn, a.D, a.eps, a.T, row_red, cta, n_cta, warp, lane);
       } else if (P.kind == CH_ROPE) {
-        chain_rope_phase(reinterpret_cast<const act_t*>(P.src), P.slab_stride, P.q_out, P.kv_layer, a.tb.row_pos, a.tb.row_slot,
-                         a.rope_tab, a.H, a.hd, a.R, a.C, a.D, a.T, s_pair_slabs, cta, n_cta, warp, lane);
+        if (2 * a.T <= CH_ROW_GROUPS * n_cta)
+          chain_rope_phase<true>(reinterpret_cast<const act_t*>(P.src), P.slab_stride, P.q_out, P.kv_layer, a.tb.row_pos, a.tb.row_slot,
+                                 a.rope_tab, a.H, a.hd, a.R, a.C, a.D, a.T, s_pair_slabs, cta, n_cta, warp, lane);
+        else
+          chain_rope_phase<false>(reinterpret_cast<const act_t*>(P.src), P.slab_stride, P.q_out, P.kv_layer, a.tb.row_pos, a.tb.row_slot,
+                                  a.rope_tab, a.H, a.hd, a.R, a.C, a.D, a.T, s_pair_slabs, cta, n_cta, warp, lane);
       } else {
         chain_attn_phase(tmem_base, a.att, &att_lists, cta, n_cta, etid);
       }
