@@ -133,3 +133,48 @@ def test_default_mode_takes_the_units_for_decode_only_steps(binding):
         P.step([(0, 1, 100 + t, 1), (1, 1, 300 + t, 1)], I.make_embeds(cfg, 6, 1 + t, 2))
         assert binding.launch_count() - n0 == prefill_launches - cfg.n_layers
     P.check_ring([0, 1])
+
+
+def test_random_schedules_units_vs_mma_sync(binding):
+    """150 random packed steps on one 7B-shaped layer - requests appear, grow by chunks of 1..180 rows or by single decode
+    rows, and are recycled at random bases before they pass 352 positions - run twice, with the units (mode 2) and with
+    attention_kernel (mode 1).  Every step's hidden states agree to rounding; the units' unit lists, look-ahead loads,
+    dynamic hand-out and wrap handling see shapes no fixed schedule has."""
+    cfg = I.CFG_7B_1L
+    hw = I.make_weights(cfg, seed=12)
+    W = binding.Weights(cfg, hw)
+    Rr, Cc, LIM = 8, 400, 352
+    worst = 0.0
+    outs = {}
+    for mode in (2, 1):
+        binding.attention_mode(mode)
+        rng = np.random.default_rng(123)
+        ring = binding.Ring(cfg, Rr, Cc, max_rows=512)
+        length = [0] * Rr
+        outs[mode] = []
+        for t in range(150):
+            segs, rows = [], 0
+            for r in rng.permutation(Rr):
+                r = int(r)
+                if length[r] >= LIM - 1 or (length[r] > 0 and rng.random() < 0.05):
+                    ring.reset_slot(r, int(rng.integers(0, Cc)))
+                    length[r] = 0
+                    continue
+                kind = rng.random()
+                if kind < 0.35:
+                    continue
+                ln = 1 if (kind < 0.7 and length[r] > 0) else int(min(rng.integers(1, 181), LIM - length[r]))
+                if rows + ln > 512:
+                    continue
+                segs.append((r, 1 if (ln == 1 and length[r] > 0) else 0, length[r], ln))
+                length[r] += ln
+                rows += ln
+            if not segs:
+                continue
+            hid = ring.packed_forward(W, I.make_embeds(cfg, 12, t, rows).cuda(), segs)
+            outs[mode].append(hid.clone())
+    assert len(outs[1]) == len(outs[2]) and len(outs[1]) > 100
+    for a, b in zip(outs[2], outs[1]):
+        assert not torch.isnan(a).any()
+        worst = max(worst, relmax(a, b))
+    assert worst <= 2e-3, f"units vs attention_kernel over random schedules: {worst:.3e}"
