@@ -45,7 +45,8 @@ int af_debug_profile_read(double* ms_sum, int64_t* counts, int32_t n_slots);
 /* The work lists of the GEMM kernel (pure host logic, needs no GPU): for `n_tile_pairs` pairs of 128-row weight tiles and
  * `n_kblocks` 64-wide k-blocks on at most `max_clusters` 2-CTA clusters: stream-K ranges (split_k == 0), split-K (split_k ==
  * 1: `splits` equal slabs per tile pair) or the layer chain's slab ranges (split_k == 2: equal unit ranges, every piece a
- * plain piece stored as slab `slab` = its ordinal inside its tile pair, at most `splits` per pair).  pieces = HOST int32 [max_clusters_out][16][8]; piece = {pair, kb0, kb1, kind (0 plain,
+ * plain piece stored as slab `slab` = its ordinal inside its tile pair, at most `splits` per pair) or the skewed split-K of a
+ * launch's first phase (split_k == 3: clusters numbered split-major, k-ranges shrinking from the first split to the last).  pieces = HOST int32 [max_clusters_out][16][8]; piece = {pair, kb0, kb1, kind (0 plain,
  * 1 contributor, 2 owner), slot, n_contrib, slab, 0}, a cluster's list ends at pair = -1.  Returns the number of
  * clusters used, or a negative AF_ERR_*. */
 int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int32_t n_kblocks, int32_t max_clusters, int32_t splits,

@@ -396,6 +396,11 @@ static int streamk_partition(int total, int nkb, int n_max, int* ub) {
 // (Two hand-made schedules for the QKV and gate/up shapes - owners with a single piece plus clusters made of
 //  contributor pieces only - were built on this table and measured no faster than the ranges; removed.)
 constexpr int SPLIT_SLABS = 2;
+// SPLIT_K for the FIRST phase of a launch: the CTAs with the highest indices become resident last (on the SMs the previous
+// kernel frees last) and have had no time to prefetch weights before griddepcontrol.wait lets the phase start - measured 1.5-2 us
+// behind at T = 282, 4 us at T = 6.  So clusters are numbered split-major (the last split of every tile pair sits on the
+// last clusters) and the k-ranges shrink linearly from 19/16 of an even share (first split) to 13/16 (last split).
+constexpr int SPLIT_K_SKEW = 3;
 
 // Pure host part: the flat [n_cl][GEMM_MAX_PIECES] table (also what af_debug_gemm_schedule returns, for CPU tests).
 static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits, std::vector<GemmPiece>* flat_out, int* n_cl_out,
@@ -412,6 +417,22 @@ static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits
       const int t = c / splits, s = c % splits;
       cl[c].push_back(piece(t, static_cast<int>(1LL * s * nkb / splits), static_cast<int>(1LL * (s + 1) * nkb / splits),
                             PK_PLAIN, 0, 0, s));
+    }
+    pair_slabs.assign(n_pairs, splits);
+  } else if (split == SPLIT_K_SKEW) {
+    // split s takes a share of 1 + 3/16 (s = 0) ... 1 - 3/16 (s = splits - 1) of an even one: boundaries from the cumulative shares
+    if (nkb < 2 * splits && splits > 1) return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: %d k-blocks cannot feed %d skewed splits", nkb, splits);
+    auto kb_at = [&](int sp) {
+      if (sp <= 0) return 0;
+      if (sp >= splits) return nkb;
+      // sum_{i < sp} (16 + 3 - 6 i / (splits - 1)) / (16 splits), in integers
+      const long long num = 19LL * sp * (splits - 1) - 3LL * sp * (sp - 1);
+      return static_cast<int>((num * nkb + 8LL * splits * (splits - 1)) / (16LL * splits * (splits - 1)));
+    };
+    cl.resize(static_cast<size_t>(n_pairs) * splits);
+    for (int c = 0; c < n_pairs * splits; ++c) {
+      const int t = c % n_pairs, sp = c / n_pairs;
+      cl[c].push_back(piece(t, kb_at(sp), kb_at(sp + 1), PK_PLAIN, 0, 0, sp));
     }
     pair_slabs.assign(n_pairs, splits);
   } else if (split == SPLIT_SLABS) {
@@ -640,7 +661,10 @@ static int chain_add_gemm(ChainBuilder& b, const void* const* w, const float* co
   P->n_tiles = n_tiles; P->num_kb = (K + GEMM_BK - 1) / GEMM_BK; P->epi = epi;
   const int n_pairs = (n_tiles + 1) / 2;
   int splits = max_slabs;
-  if (split == SPLIT_K) splits = gemm_split_count(b.ctx, n_tiles, K);
+  if (split == SPLIT_K) {
+    splits = gemm_split_count(b.ctx, n_tiles, K);
+    if (P == &b.a.ph[0] && splits > 1 && P->num_kb >= 4 * splits) split = SPLIT_K_SKEW;   // the launch's first phase: late-resident clusters get the short pieces
+  }
   Sched sc;
   int rc = build_schedule(b.ctx, split, n_pairs, P->num_kb, b.ctx->max_clusters, split == SPLIT_STREAMK ? 1 : splits, &sc, b.chunks);
   if (rc) return rc;
@@ -956,7 +980,7 @@ extern "C" int af_debug_gemm_schedule(int32_t split_k, int32_t n_tile_pairs, int
   if (!pieces) return fail(AF_ERR_ARG, "null output");
   std::vector<GemmPiece> flat;
   int n_cl = 0;
-  const int rc = make_schedule(split_k == 2 ? SPLIT_SLABS : (split_k ? SPLIT_K : SPLIT_STREAMK), n_tile_pairs, n_kblocks, max_clusters, splits, &flat, &n_cl);
+  const int rc = make_schedule(split_k == 3 ? SPLIT_K_SKEW : split_k == 2 ? SPLIT_SLABS : (split_k ? SPLIT_K : SPLIT_STREAMK), n_tile_pairs, n_kblocks, max_clusters, splits, &flat, &n_cl);
   if (rc) return rc;
   if (n_cl > max_clusters_out) return fail(AF_ERR_ARG, "%d clusters do not fit the output (%d)", n_cl, max_clusters_out);
   memcpy(pieces, flat.data(), flat.size() * sizeof(GemmPiece));
@@ -1115,9 +1139,10 @@ static int packed_forward_impl(const af_weights* w, const void* packed_embeds, c
   auto chain_schedulable = [&]() {
     const int kd = (D + GEMM_BK - 1) / GEMM_BK, kf = (F + GEMM_BK - 1) / GEMM_BK;
     const int d_pairs = ((D + GEMM_BM - 1) / GEMM_BM + 1) / 2, gu_pairs = ((F + 63) / 64 + 1) / 2;
+    const int o_splits = gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, D);
     Sched sc;
     return build_schedule(ctx, SPLIT_SLABS, (3 * ((D + GEMM_BM - 1) / GEMM_BM) + 1) / 2, kd, ctx->max_clusters, QKV_MAX_SLABS, &sc, t_chunks) == AF_OK &&
-           build_schedule(ctx, SPLIT_K, d_pairs, kd, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, D), &sc, t_chunks) == AF_OK &&
+           build_schedule(ctx, (o_splits > 1 && kd >= 4 * o_splits) ? SPLIT_K_SKEW : SPLIT_K, d_pairs, kd, ctx->max_clusters, o_splits, &sc, t_chunks) == AF_OK &&
            build_schedule(ctx, SPLIT_K, d_pairs, kf, ctx->max_clusters, gemm_split_count(ctx, (D + GEMM_BM - 1) / GEMM_BM, F), &sc, t_chunks) == AF_OK &&
            build_schedule(ctx, SPLIT_STREAMK, gu_pairs, kd, ctx->max_clusters, 1, &sc, t_chunks) == AF_OK;
   };

@@ -114,6 +114,33 @@ def test_splitk_schedules(n_pairs, nkb, splits):
     assert (cover == 1).all() and len(slabs) == n_pairs * splits
 
 
+@pytest.mark.parametrize("n_pairs,nkb,splits", [(16, 64, 4), (16, 172, 4), (1, 8, 4), (3, 11, 2), (2, 9, 3)])
+def test_skewed_splitk_schedules(n_pairs, nkb, splits):
+    """split_k = 3, the first phase of a layer-chain launch: as split-K, but clusters are numbered split-major (the last
+    clusters - resident last, nothing prefetched - hold the LAST split of every tile pair) and the k-ranges shrink from the
+    first split to the last."""
+    cl = schedule(3, n_pairs, nkb, 74, splits)
+    assert len(cl) == n_pairs * splits
+    cover = np.zeros((n_pairs, nkb), dtype=np.int32)
+    slabs = set()
+    lens = {}
+    for c, pieces in enumerate(cl):
+        assert len(pieces) == 1 and pieces[0]["kind"] == PLAIN and pieces[0]["kb1"] > pieces[0]["kb0"]
+        p = pieces[0]
+        assert (p["pair"], p["mid"]) == (c % n_pairs, c // n_pairs)
+        cover[p["pair"], p["kb0"]:p["kb1"]] += 1
+        slabs.add((p["pair"], p["mid"]))
+        lens.setdefault(p["mid"], set()).add(p["kb1"] - p["kb0"])
+    assert (cover == 1).all() and len(slabs) == n_pairs * splits
+    assert all(len(v) == 1 for v in lens.values())                         # a split has one length for every pair
+    ln = [next(iter(lens[m])) for m in range(splits)]
+    assert sum(ln) == nkb and min(ln) >= 1
+    if nkb >= 16 * splits:                                                 # shares fall linearly from 19/16 to 13/16 of an even one
+        assert all(a >= b for a, b in zip(ln, ln[1:])) and ln[0] > ln[-1]
+        even = nkb / splits
+        assert abs(ln[0] - 19 / 16 * even) <= 1 and abs(ln[-1] - 13 / 16 * even) <= 1
+
+
 def check_slabs(n_pairs, nkb, max_cl, splits):
     """Layer-chain slab ranges (split_k = 2): every (tile pair, k-block) exactly once, every piece plain, a pair's pieces
     carry slab ordinals 0, 1, 2, .. in k order (the row stage adds them in that order), never more than `splits`."""
