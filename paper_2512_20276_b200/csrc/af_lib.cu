@@ -436,18 +436,47 @@ static int make_schedule(int split, int n_pairs, int nkb, int max_cl, int splits
     }
     pair_slabs.assign(n_pairs, splits);
   } else if (split == SPLIT_SLABS) {
-    // range length: all clusters busy, but never more than `splits` pieces of one tile pair
+    // Ranges of equal COST over all clusters: a range pays its k-blocks plus kSlabCharge k-blocks for every tile pair it
+    // touches (each piece ends in an accumulator drain and a pipeline refill, ~9 k-blocks' worth at T = 282; with equal LENGTHS the two
+    // thirds of the clusters whose range crosses a pair boundary finished 3 us after the others).  Never shorter than
+    // lmin, so that a tile pair is cut into at most `splits` pieces.
     const int total = n_pairs * nkb;
-    int len = (total + max_cl - 1) / max_cl;
-    if (splits > 1) { const int lmin = (nkb - 1 + splits - 2) / (splits - 1); if (len < lmin) len = lmin; }
-    else len = nkb > len ? nkb : (len + nkb - 1) / nkb * nkb;
-    if (len < 1) len = 1;
-    const int n = (total + len - 1) / len;
+    constexpr int kSlabCharge = 9;
+    int lmin = 1;
+    if (splits > 1) lmin = (nkb - 1 + splits - 2) / (splits - 1);
+    else lmin = nkb;
+    if (lmin < 1) lmin = 1;
+    std::vector<int> ub;   // range c = [ub[c], ub[c + 1])
+    auto cut = [&](long long cap, std::vector<int>* out) {   // greedy: every range as long as `cap` allows
+      out->assign(1, 0);
+      int a = 0;
+      while (a < total) {
+        int b = a + lmin < total ? a + lmin : total;
+        if (splits == 1) { b = (b + nkb - 1) / nkb * nkb; if (b > total) b = total; }
+        auto cost = [&](int e) { return static_cast<long long>(e - a) + kSlabCharge * ((e - 1) / nkb - a / nkb + 1); };
+        while (b < total) {
+          const int nb = splits == 1 ? (b + nkb < total ? b + nkb : total) : b + 1;
+          if (cost(nb) > cap) break;
+          b = nb;
+        }
+        out->push_back(b);
+        a = b;
+      }
+      return static_cast<int>(out->size()) - 1;
+    };
+    long long lo = 1, hi = static_cast<long long>(total) + kSlabCharge * (n_pairs + 1);
+    while (lo < hi) {   // the smallest cap that fits max_cl ranges
+      const long long mid_cap = (lo + hi) / 2;
+      std::vector<int> tmp;
+      if (cut(mid_cap, &tmp) <= max_cl) hi = mid_cap; else lo = mid_cap + 1;
+    }
+    const int n = cut(lo, &ub);
+    if (n > max_cl) return fail(AF_ERR_UNSUPPORTED, "GEMM schedule: %d ranges for %d clusters", n, max_cl);
     cl.resize(n);
     pair_slabs.assign(n_pairs, 0);
     for (int c = 0; c < n; ++c) {
-      int u = c * len;
-      const int end = (c + 1) * len < total ? (c + 1) * len : total;
+      int u = ub[c];
+      const int end = ub[c + 1];
       while (u < end) {
         const int t = u / nkb, kb0 = u - t * nkb;
         const int kb1 = end - t * nkb < nkb ? end - t * nkb : nkb;
