@@ -178,3 +178,15 @@ def test_random_schedules_units_vs_mma_sync(binding):
         assert not torch.isnan(a).any()
         worst = max(worst, relmax(a, b))
     assert worst <= 2e-3, f"units vs attention_kernel over random schedules: {worst:.3e}"
+
+
+def test_units_on_a_two_chunk_step(binding):
+    """A packed step of 800 rows (eight 100-row prefills) runs the layer chain with two token chunks per weight tile; its
+    last phase is still the attention units (256 tensor units on 148 CTAs: every CTA takes two).  Then 8 decode rows."""
+    cfg = I.CFG_7B_1L
+    hw = I.make_weights(cfg, seed=8)
+    binding.attention_mode(2)
+    P = Pair(cfg, hw, R=8, C=256, max_rows=1024, bases=[250, 0, 13, 100, 255, 77, 200, 31], oracle_dtype=torch.float32)
+    P.step([(r, 0, 0, 100) for r in range(8)], I.make_embeds(cfg, 8, 0, 800))
+    P.step([(r, 1, 100, 1) for r in range(8)], I.make_embeds(cfg, 8, 1, 8))
+    P.check_ring(list(range(8)))
