@@ -190,3 +190,23 @@ def test_units_on_a_two_chunk_step(binding):
     P.step([(r, 0, 0, 100) for r in range(8)], I.make_embeds(cfg, 8, 0, 800))
     P.step([(r, 1, 100, 1) for r in range(8)], I.make_embeds(cfg, 8, 1, 8))
     P.check_ring(list(range(8)))
+
+
+def test_units_with_fp8_weights(binding):
+    """AF_WEIGHTS_FP8 runs on the layer chain only, so with mode 2 its attention is the chain's last phase too
+    (layer_chain_kernel<true, *>): the steady schedule's first 8 steps, units against attention_kernel, same weights."""
+    cfg = I.cfg_7b_layers(2, vocab=512)
+    W = binding.WeightsFP8(cfg, I.quantize_weights_fp8(I.make_weights(cfg, seed=5, threads=16)))
+    outs = {}
+    for mode in (2, 1):
+        binding.attention_mode(mode)
+        ring = binding.Ring(cfg, R, C, max_rows=288)
+        for r in range(R):
+            ring.reset_slot(r, (r * 131 + 290) % C)
+        outs[mode] = []
+        for t in range(8):
+            ring.reset_slot(t % R, -1)
+            segs = I.steady_schedule(t, L_P, K, R)
+            outs[mode].append(ring.packed_forward(W, I.make_embeds(cfg, 5, t, I.total_rows(segs)).cuda(), segs).clone())
+    worst = max(relmax(a, b) for a, b in zip(outs[2], outs[1]))
+    assert worst <= 2e-3, f"FP8 weights, units vs attention_kernel: {worst:.3e}"
